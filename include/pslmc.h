@@ -1,0 +1,182 @@
+/*
+ * pslmc.h — C ABI of libpslmc: phase-space-let (PSL) source sampling + Monte Carlo dose on one B200.
+ *
+ * The operations are those of Tian et al., "An Analytic Linear Accelerator Source Model for Monte
+ * Carlo dose calculations. II", in the reading fixed by DESIGN.md:
+ *   psl_build          PAPER.md:35-57  §2.1.1 (PSR→PSL conversion, Eq. 1-2),
+ *                      PAPER.md:61-69  §2.1.2 (sampling areas), :75-80 S1-S2 (Eq. 3)
+ *   mc_sample_debug    PAPER.md:82-92  S3 (Eq. 4-5), :94-116 S4-S5, jaw rejection :65/:92, set-up :173
+ *   mc_dose            PAPER.md:118-120 §2.1.3 (iterated source kernel / transport kernel, M per
+ *                      launch, type-major / energy-ascending order), :161 (cut-offs 50 keV / 200 keV)
+ *   mc_stats           PAPER.md:177-191 Table 1 (per-phase timing breakdown)
+ *
+ * Conventions
+ *   - Plain C structs, `extern "C"`, no exceptions cross the boundary, no torch types.
+ *   - Every pointer says HOST or DEVICE.  The caller owns every array it passes and keeps it alive
+ *     for the duration of the call.  The library owns `psl_t` (host + device tables) until psl_free.
+ *   - Units: cm, MeV, g/cm^3.  Beam frame: origin at the primary source, +z downstream, isocentre at
+ *     (0,0,sad).  Phantom frame: pos_ph = iso + R * (pos_beam - (0,0,sad)), dir_ph = R * dir_beam.
+ *   - All entry points return 0 on success or a negative MC_E_* code; mc_last_error() returns a
+ *     thread-local message.  Outputs are unspecified after an error.
+ *   - Calls on one psl_t are not re-entrant.  mc_dose is synchronous with respect to the given
+ *     stream when it returns.
+ *   - Determinism: for fixed inputs and seed, dose, ledgers and counters are bitwise identical for
+ *     every `batch`, every `order` and every partition [history_begin,history_end) summed.
+ *   - There is no CPU fallback: every entry point that computes needs a CUDA device (sm_100a).
+ */
+#ifndef PSLMC_H
+#define PSLMC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MC_OK             0
+#define MC_E_INVALID_ARG -1
+#define MC_E_EMPTY_FIELD -2  /* no let survives the jaw selection                              */
+#define MC_E_WORKSPACE   -3  /* caller-supplied workspace too small                            */
+#define MC_E_CUDA        -4  /* a CUDA runtime call or kernel failed                           */
+#define MC_E_OVERFLOW    -5  /* a secondary queue could not be drained / ledger overflow       */
+
+/* PSR analytic source model (paper layer L0).                           */
+typedef struct {
+  int32_t n_ebin, n_ring;          /* energy bins, rings                                         */
+  double  e_min, e_bin_width;      /* MeV; bin e spans e_min + e*w .. e_min + (e+1)*w            */
+  double  ring_width, z_phsp;      /* cm; ring i spans i*w .. (i+1)*w on the plane z = z_phsp    */
+  const double *W;                 /* HOST [3][n_ebin][n_ring] relative ring weights, row-major  */
+  double  sigma_src[3], z_src[3];  /* per sub-source Gaussian virtual source: sigma, plane z (cm)*/
+  int32_t particle_type[3];        /* 0 photon, 1 electron                                       */
+} psr_params_t;
+
+/* Thin rectangular jaws.  Edges are given by their projection on the isocentre
+ * plane z = sad; the X pair sits at z_jx, the Y pair at z_jy (beam frame, cm).  x1 < x2, y1 < y2. */
+typedef struct { double x1, x2, y1, y2; double z_jx, z_jy, sad; } jaws_t;
+
+/* Voxel phantom.  Voxel (i,j,k) spans o + i*d .. o + (i+1)*d per axis; linear index
+ * (k*ny + j)*nx + i (x fastest).  Outside the grid is vacuum.                                   */
+typedef struct {
+  int32_t nx, ny, nz;
+  double  dx, dy, dz, ox, oy, oz;
+  const float   *density;          /* DEVICE (mc_dose) / HOST (mc_dose_host); g/cm^3             */
+  const uint8_t *material;         /* DEVICE / HOST likewise; 0 water, 1 lung, 2 bone            */
+} phantom_t;
+
+/* Beam set-up ("translating and rotating").  R is row-major 3x3.                   */
+typedef struct { double iso[3]; double R[9]; double sad; } beam_geom_t;
+
+typedef struct psl psl_t;          /* opaque: active lets, alias tables, group weights           */
+
+#define MC_ORDER_SORTED 0          /* sub-source major, energy bin ascending  */
+#define MC_ORDER_MIXED  1          /* histories permuted, one combined launch over mixed types   */
+
+#define MC_FLAG_ELECTRONS_LOCAL 1  /* debug physics: deposit every charged secondary on the spot */
+#define MC_FLAG_STATS           2  /* fill the event counters of mc_stats_t (ledgers are always) */
+#define MC_FLAG_TIMING          4  /* CUDA-event time per kernel class into mc_stats_t           */
+#define MC_FLAG_STATIC_LANES    8  /* ablation: one particle per thread, no lane refill          */
+
+typedef struct {
+  void     *workspace;             /* DEVICE scratch or NULL (library-managed, cached in psl_t)  */
+  size_t    workspace_bytes;
+  void     *cuda_stream;           /* cudaStream_t or NULL (legacy default stream)               */
+  int64_t  *dose_acc;              /* DEVICE int64[nx*ny*nz] or NULL.  When given, deposits are  */
+                                   /* ADDED to it (multi-beam plans) and dose_out may be NULL    */
+  int32_t   order;                 /* MC_ORDER_*                                                 */
+  int32_t   flags;                 /* MC_FLAG_* bits                                             */
+  uint64_t *fingerprints;          /* DEVICE u64[history_end-history_begin] or NULL; ADDED to    */
+  uint64_t  history_begin;         /* sub-range of history ids to run (sharding) ...             */
+  uint64_t  history_end;           /* ... 0 means n_histories                                    */
+} mc_opts_t;
+
+/* Ledger / kernel-class indices of mc_stats_t.                                                  */
+enum { MC_LEDGER_INCIDENT = 0, MC_LEDGER_DEPOSITED = 1, MC_LEDGER_ESCAPED = 2, MC_LEDGER_JAW = 3 };
+enum { MC_K_SAMPLE = 0, MC_K_PHOTON = 1, MC_K_ELECTRON = 2, MC_K_FINALISE = 3, MC_K_AUX = 4 };
+
+typedef struct {
+  /* energy ledgers in quanta of 2^-32 MeV, exact 128-bit sums as (hi:int64, lo:uint64)          */
+  int64_t  ledger_hi[4];
+  uint64_t ledger_lo[4];
+  uint64_t n_hist[3];              /* histories sampled per sub-source                           */
+  uint64_t n_jaw_rejected;
+  /* event counters (MC_FLAG_STATS)                                                              */
+  uint64_t n_missed;               /* tracks that never entered the phantom                      */
+  uint64_t n_flights, n_virtual, n_compton, n_photo, n_pair;
+  uint64_t n_photon_cutoff, n_photon_escape, n_uncollided_escape;
+  uint64_t n_sec_electrons, n_sec_photons;
+  uint64_t n_electron_tracks, n_electron_steps, n_electron_escape;
+  uint64_t n_deposits;
+  uint64_t queue_high_water[2];    /* electron queue, photon queue (entries)                     */
+  uint64_t launches[5];            /* per MC_K_* class                                           */
+  float    ms[5];                  /* per MC_K_* class (MC_FLAG_TIMING)                          */
+  float    ms_total;               /* whole mc_dose on its stream, CUDA events (always)          */
+} mc_stats_t;
+
+/* psl_build — host.  Cuts every ring into n_sectors equal angular lets (weight W_ring/n_sectors,
+ * Eq. 1-2 integrated over a sector), computes the sampling rectangle of each sub-source
+ * (PAPER.md:65), keeps lets whose bounding box touches it, builds one alias table per
+ * (sub-source, energy bin) group and uploads the tables to the current CUDA device.
+ * Returns MC_E_EMPTY_FIELD if no let is active.                                                 */
+int  psl_build(const psr_params_t *psr, const jaws_t *jaws, int32_t n_sectors, psl_t **out);
+void psl_free(psl_t *psl);
+
+/* psl_export — host.  Serialises the tables for inspection:
+ *   u64 n_groups; then per group: i32 stype, i32 ebin, u64 n, f64 W_g,
+ *   u16 ring[n], u16 sector[n], u32 thresh[n], u32 alias[n]   (each array padded to 8 bytes);
+ *   finally f64 rect[3][4] = (xlo,xhi,ylo,yhi) sampling rectangle per sub-source.
+ * Call with host_buf = NULL to get the size in *bytes.                                          */
+int  psl_export(const psl_t *psl, void *host_buf, size_t *bytes);
+
+/* psl_allocate — host.  Eq. 3 at group level: N_g = N*W_g/sum(W_g), largest-remainder rounding.
+ * off_out: HOST u64[n_groups+1], prefix offsets of the contiguous history-id ranges.            */
+int  psl_allocate(const psl_t *psl, uint64_t n_histories, uint64_t *off_out);
+
+/* Workspace bytes mc_dose needs for this batch size (0 on invalid arguments).                   */
+size_t mc_workspace_bytes(const psl_t *psl, const phantom_t *ph, uint64_t batch);
+
+/* mc_dose — the hot path.  Runs histories [history_begin,history_end) of an n_histories-history
+ * allocation in batches of `batch` through k_sample → k_photon / k_electron (+ secondary queues)
+ * with int64 fixed-point scoring, then writes
+ *   dose_out[v] = acc[v] * 2^-32 / (rho_v * V_voxel * n_histories)   (MeV/g per history; 0 if rho=0)
+ * dose_out: DEVICE double[nx*ny*nz], overwritten (may be NULL if opts->dose_acc is given).      */
+int  mc_dose(const psl_t *psl, const phantom_t *ph, const beam_geom_t *beam,
+             uint64_t n_histories, uint64_t seed, uint64_t batch,
+             double *dose_out, const mc_opts_t *opts);
+
+/* mc_dose_host — same, end to end from HOST buffers: ph->density / ph->material and dose_out are
+ * HOST pointers; the call uploads the phantom, runs mc_dose, and downloads the dose.            */
+int  mc_dose_host(const psl_t *psl, const phantom_t *ph_host, const beam_geom_t *beam,
+                  uint64_t n_histories, uint64_t seed, uint64_t batch,
+                  double *dose_out_host, const mc_opts_t *opts);
+
+/* Counters, ledgers and timings of the last mc_dose / mc_transport_debug on this thread.        */
+int  mc_stats(mc_stats_t *out);
+const char *mc_last_error(void);
+
+/* ---- parity / debug exports ------------------------------------------------------------------ */
+
+/* Source sampling only.  soa_out: DEVICE float[8*count] as two float4 planes,
+ *   plane 0 [i] = (x, y, z, E), plane 1 [i] = (u, v, w, status), i = history - first_history,
+ * status = group index (>= 0) if the particle passed the jaws, -(group index) - 1 if rejected.  */
+int  mc_sample_debug(const psl_t *psl, const beam_geom_t *beam, uint64_t first_history,
+                     uint64_t count, uint64_t n_histories, uint64_t seed, float *soa_out,
+                     void *cuda_stream);
+
+/* Transport only.  Takes `count` particles in the layout of mc_sample_debug (status < 0 entries
+ * are skipped), particle_type 0 photon / 1 electron, as track 0 of histories first_history + i
+ * with the stream positioned at draw 8, and scores into opts->dose_acc (required).  Ledgers and
+ * counters go to mc_stats; the incident ledger counts the particles given.                      */
+int  mc_transport_debug(const phantom_t *ph, int32_t particle_type, const float *soa_in,
+                        uint64_t first_history, uint64_t count, uint64_t seed,
+                        const mc_opts_t *opts);
+
+/* One Philox4x32-10 block computed ON THE DEVICE: key = seed, counter = (block, track, h_lo, h_hi).
+ * out: HOST u32[4].                                                                             */
+int  mc_philox_debug(uint64_t seed, uint64_t history, uint32_t track, uint32_t block,
+                     uint32_t *out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PSLMC_H */
