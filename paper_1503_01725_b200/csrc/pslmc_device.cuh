@@ -1,0 +1,190 @@
+// pslmc_device.cuh — device-side building blocks of libpslmc (sm_100a): counter-based RNG,
+// physics in fp32, geometry, int64 fixed-point scoring.  Definitions: DESIGN.md R1, P1-P9, S1, F1.
+// Shares nothing with oracle/ (which is test infrastructure); constants are typed here on their own.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace pslmc {
+
+// ------------------------------------------------------------------ model constants
+constexpr float  kMe      = 0.51099895f;      // electron rest energy (MeV)
+constexpr double kMeD     = 0.51099895;
+constexpr double kTwoPiRe2 = 2.0 * 3.14159265358979323846 * 7.940787e-26;   // 2 pi r_e^2 (cm^2)
+constexpr float  kEPair   = 1.022f;           // pair threshold / annihilation total (MeV)
+constexpr float  kEAnnih  = 0.511f;
+constexpr float  kPcut    = 0.05f;            // photon cut-off
+constexpr float  kEcut    = 0.2f;             // electron cut-off
+constexpr float  kEpsB    = 1e-4f;            // boundary nudge (cm)
+constexpr float  kFe      = 0.12f;            // energy-loss fraction per condensed-history step
+constexpr float  kPi      = 3.14159265358979323846f;
+
+struct Materials {       // index: 0 water, 1 lung, 2 bone
+  float ne[3];           // electrons per gram
+  float cphoto[3];       // cm^2 g^-1 MeV^3
+  float ppair[3];        // cm^2 g^-1
+  float sscale[3];       // stopping-power scale
+  float inv_x0[3];       // 1 / radiation length (cm^2/g)
+};
+__constant__ Materials c_mat = {
+    {3.343e23f, 3.343e23f, 3.100e23f},
+    {2.77e-6f, 2.77e-6f, 2.2e-5f},
+    {9.6e-4f, 9.6e-4f, 1.3e-3f},
+    {1.0f, 1.0f, 0.92f},
+    {1.0f / 36.08f, 1.0f / 36.08f, 1.0f / 27.2f}};
+
+// ------------------------------------------------------------------ R1: Philox4x32-10
+struct Philox {
+  uint32_t k0, k1;             // key = seed
+  uint32_t track, hlo, hhi;    // counter words 1..3
+  uint32_t n;                  // next draw number of this stream (block n>>2, word n&3)
+  uint32_t w0, w1, w2, w3;     // cached block
+
+  __device__ __forceinline__ void block(uint32_t j) {
+    uint32_t c0 = j, c1 = track, c2 = hlo, c3 = hhi, a = k0, b = k1;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+      uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+      uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+      c0 = h1 ^ c1 ^ a; c1 = l1; c2 = h0 ^ c3 ^ b; c3 = l0;
+      a += 0x9E3779B9u; b += 0xBB67AE85u;
+    }
+    w0 = c0; w1 = c1; w2 = c2; w3 = c3;
+  }
+  __device__ __forceinline__ void init(uint64_t seed, uint64_t h, uint32_t trk, uint32_t ndraw) {
+    k0 = (uint32_t)seed; k1 = (uint32_t)(seed >> 32);
+    hlo = (uint32_t)h; hhi = (uint32_t)(h >> 32); track = trk; n = ndraw;
+    if (ndraw & 3u) block(ndraw >> 2);
+  }
+  __device__ __forceinline__ uint32_t next() {
+    uint32_t i = n & 3u;
+    if (i == 0) block(n >> 2);
+    ++n;
+    return i == 0 ? w0 : (i == 1 ? w1 : (i == 2 ? w2 : w3));
+  }
+};
+__device__ __forceinline__ float u_co(uint32_t x) { return (float)(x >> 8) * (1.0f / 16777216.0f); }          // [0,1)
+__device__ __forceinline__ float u_oc(uint32_t x) { return (float)((x >> 8) + 1u) * (1.0f / 16777216.0f); }   // (0,1]
+
+__device__ __forceinline__ uint32_t child_track(uint32_t parent, uint32_t n, uint32_t c) {
+  return (((parent ^ 0x9E3779B9u) * 0x01000193u) ^ ((n << 2) | c)) * 0x01000193u;
+}
+
+// ------------------------------------------------------------------ F1: FNV-1a-64
+struct Fnv {
+  uint64_t v;
+  __device__ __forceinline__ void init(uint32_t track) { v = 0xcbf29ce484222325ull; u32(track); }
+  __device__ __forceinline__ void byte(uint32_t b) { v = (v ^ (uint64_t)b) * 0x100000001b3ull; }
+  __device__ __forceinline__ void u32(uint32_t x) { byte(x & 255u); byte((x >> 8) & 255u); byte((x >> 16) & 255u); byte(x >> 24); }
+};
+
+// ------------------------------------------------------------------ phantom + scoring
+struct Grid {
+  int nx, ny, nz;
+  float ox, oy, oz, dx, dy, dz, idx, idy, idz;      // origin, voxel size, reciprocal voxel size
+  const float   *density;
+  const uint8_t *material;
+  unsigned long long *acc;                           // int64 fixed-point dose accumulator (2^-32 MeV)
+};
+
+__device__ __forceinline__ long long quanta(float e) { return __float2ll_rn(e * 4294967296.0f); }
+
+__device__ __forceinline__ bool locate(const Grid &g, float x, float y, float z, int &i, int &j, int &k) {
+  float fi = floorf((x - g.ox) * g.idx), fj = floorf((y - g.oy) * g.idy), fk = floorf((z - g.oz) * g.idz);
+  bool in = fi >= 0.0f && fi < (float)g.nx && fj >= 0.0f && fj < (float)g.ny && fk >= 0.0f && fk < (float)g.nz;
+  i = (int)fi; j = (int)fj; k = (int)fk;
+  return in;
+}
+__device__ __forceinline__ int vox_index(const Grid &g, int i, int j, int k) { return (k * g.ny + j) * g.nx + i; }
+
+// Ray/box entry for a track that starts outside the grid.  false = misses the phantom.
+__device__ __forceinline__ bool enter(const Grid &g, float &x, float &y, float &z, float u, float v, float w,
+                                      int &i, int &j, int &k) {
+  const float lo[3] = {g.ox, g.oy, g.oz};
+  const float hi[3] = {g.ox + g.nx * g.dx, g.oy + g.ny * g.dy, g.oz + g.nz * g.dz};
+  const float p[3] = {x, y, z}, d[3] = {u, v, w};
+  float tmin = -INFINITY, tmax = INFINITY;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    if (d[a] == 0.0f) { if (p[a] < lo[a] || p[a] >= hi[a]) return false; continue; }
+    float t1 = (lo[a] - p[a]) / d[a], t2 = (hi[a] - p[a]) / d[a];
+    tmin = fmaxf(tmin, fminf(t1, t2)); tmax = fminf(tmax, fmaxf(t1, t2));
+  }
+  if (tmin > tmax || tmax <= 0.0f) return false;
+  float s = fmaxf(tmin, 0.0f) + kEpsB;
+  x += s * u; y += s * v; z += s * w;
+  return locate(g, x, y, z, i, j, k);
+}
+
+// ------------------------------------------------------------------ physics
+// Klein–Nishina total cross-section per electron (cm^2).  The bracket cancels ~1.5/alpha^2-fold at low
+// energy, so it is evaluated in double (once per photon energy change, not per flight).
+__device__ __forceinline__ float sigma_kn(float E) {
+  double a = (double)E / kMeD, L = log1p(2.0 * a), t = 1.0 + 2.0 * a;
+  double s = (1.0 + a) / (a * a) * (2.0 * (1.0 + a) / t - L / a) + L / (2.0 * a) - (1.0 + 3.0 * a) / (t * t);
+  return (float)(kTwoPiRe2 * s);
+}
+
+// Per-energy photon data, recomputed after every energy change.
+struct PhotonXs {
+  float skn, inv_e3, lp2, mu_max;     // sigma_KN, 1/E^3, ln^2(E/1.022) (0 below threshold), Woodcock majorant
+  __device__ __forceinline__ void set(float E, const float rhomax[3]) {
+    skn = sigma_kn(E);
+    inv_e3 = 1.0f / (E * E * E);
+    float l = E > kEPair ? logf(E / kEPair) : 0.0f;
+    lp2 = l * l;
+    float m = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+      m = fmaxf(m, rhomax[k] * (c_mat.ne[k] * skn + c_mat.cphoto[k] * inv_e3 + c_mat.ppair[k] * lp2));
+    mu_max = m;
+  }
+};
+
+// Rotate unit vector d by polar angle (ct, st) and azimuth phi = 2*pi*uphi.
+__device__ __forceinline__ void rotate(float &u, float &v, float &w, float ct, float st, float uphi) {
+  float sp, cp;
+  sincospif(2.0f * uphi, &sp, &cp);
+  float nx, ny, nz;
+  if (fabsf(w) < 0.99999f) {
+    float s = sqrtf(1.0f - w * w), is = 1.0f / s;
+    nx = u * ct + st * (u * w * cp - v * sp) * is;
+    ny = v * ct + st * (v * w * cp + u * sp) * is;
+    nz = w * ct - s * st * cp;
+  } else {
+    nx = st * cp; ny = st * sp; nz = w > 0.0f ? ct : -ct;
+  }
+  float inv = rsqrtf(nx * nx + ny * ny + nz * nz);
+  u = nx * inv; v = ny * inv; w = nz * inv;
+}
+
+// Kahn's rejection for Klein–Nishina: returns eta = E/E'.  3 draws per trial.
+__device__ __forceinline__ float kahn(float alpha, Philox &rng) {
+  const float ta = 2.0f * alpha, pb = (ta + 1.0f) / (ta + 9.0f);
+  for (;;) {
+    float r1 = u_co(rng.next()), r2 = u_co(rng.next()), r3 = u_co(rng.next());
+    if (r1 <= pb) {
+      float eta = 1.0f + ta * r2, ie = 1.0f / eta;
+      if (r3 <= 4.0f * (ie - ie * ie)) return eta;
+    } else {
+      float eta = (ta + 1.0f) / (1.0f + ta * r2);
+      float ct = 1.0f - (eta - 1.0f) / alpha;
+      if (r3 <= 0.5f * (ct * ct + 1.0f / eta)) return eta;
+    }
+  }
+}
+
+// ------------------------------------------------------------------ warp helpers
+__device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+// 128-bit unsigned accumulate into (lo, hi) words in global memory.
+__device__ __forceinline__ void add128(unsigned long long *lohi, unsigned long long q) {
+  if (q == 0) return;
+  unsigned long long old = atomicAdd(lohi, q);
+  if (old + q < old) atomicAdd(lohi + 1, 1ull);
+}
+
+}  // namespace pslmc

@@ -1,0 +1,471 @@
+// pslmc_dose.cu — the batching driver and the C ABI of the hot path: iterated k_sample → k_photon /
+// k_electron launches per sub-source type and energy order, secondary
+// queues, int64 scoring, finalise, stats.  No CPU fallback: every entry point here needs a device.
+#include "pslmc_host.h"
+#include "pslmc_transport.cuh"
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+
+namespace pslmc {
+
+#define CUDA_TRY(expr)                                                                         \
+  do {                                                                                         \
+    cudaError_t e_ = (expr);                                                                   \
+    if (e_ != cudaSuccess) {                                                                   \
+      char b_[512];                                                                            \
+      snprintf(b_, sizeof b_, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+      return fail(MC_E_CUDA, b_);                                                              \
+    }                                                                                          \
+  } while (0)
+
+thread_local mc_stats_t g_stats;
+
+// Library-managed scratch (used when the caller passes no workspace).  One per process; calls are
+// not re-entrant (see pslmc.h).
+struct Scratch { void *ptr = nullptr; size_t bytes = 0; };
+static Scratch g_scratch, g_hostio;
+
+static int scratch_get(Scratch &s, size_t bytes, void **out) {
+  if (s.bytes < bytes) {
+    if (s.ptr) cudaFree(s.ptr);
+    s.ptr = nullptr; s.bytes = 0;
+    CUDA_TRY(cudaMalloc(&s.ptr, bytes));
+    s.bytes = bytes;
+  }
+  *out = s.ptr;
+  return MC_OK;
+}
+
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// Workspace layout for a batch of B primaries: control block, group offsets, the particle buffer
+// (2 planes), the electron queue (capacity 4B) and the photon queue (capacity B), each 3 planes,
+// then (optionally) the int64 dose grid.
+struct Layout {
+  size_t ctl, off, p0, p1, eq[3], pq[3], acc, total;
+  unsigned eq_cap, pq_cap;
+};
+static Layout make_layout(uint64_t batch, size_t nvox, bool with_acc) {
+  Layout L; size_t o = 0;
+  auto take = [&](size_t b) { size_t at = o; o += align_up(b); return at; };
+  L.eq_cap = (unsigned)std::min<uint64_t>(4 * batch, 0x7fffffffu); L.pq_cap = (unsigned)batch;
+  L.ctl = take(sizeof(Control)); L.off = take(sizeof(uint64_t) * 160);
+  L.p0 = take(16 * batch); L.p1 = take(16 * batch);
+  for (int k = 0; k < 3; ++k) L.eq[k] = take((size_t)16 * L.eq_cap);
+  for (int k = 0; k < 3; ++k) L.pq[k] = take((size_t)16 * L.pq_cap);
+  L.acc = take(with_acc ? 8 * nvox : 0);
+  L.total = o;
+  return L;
+}
+
+int upload_tables(psl *P) {
+  CUDA_TRY(cudaGetDevice(&P->device));
+  const size_t G = P->groups.size();
+  std::vector<uint32_t> let_off(G), n_let(G);
+  std::vector<AliasEntry> table;
+  for (size_t g = 0; g < G; ++g) {
+    const HostGroup &hg = P->groups[g];
+    let_off[g] = (uint32_t)table.size(); n_let[g] = (uint32_t)hg.ring.size();
+    for (size_t i = 0; i < hg.ring.size(); ++i) {
+      AliasEntry e; e.thresh = hg.thresh[i]; e.ring_c = hg.ring[i]; e.sector_c = hg.sector[i];
+      e.ring_a = hg.ring[hg.alias[i]]; e.sector_a = hg.sector[hg.alias[i]]; e.pad = 0;
+      table.push_back(e);
+    }
+  }
+  P->total_lets = table.size();
+  CUDA_TRY(cudaMalloc(&P->d_table, sizeof(AliasEntry) * std::max<size_t>(1, table.size())));
+  CUDA_TRY(cudaMalloc((void **)&P->d_let_off, sizeof(uint32_t) * G));
+  CUDA_TRY(cudaMalloc((void **)&P->d_n_let, sizeof(uint32_t) * G));
+  CUDA_TRY(cudaMemcpy(P->d_table, table.data(), sizeof(AliasEntry) * table.size(), cudaMemcpyHostToDevice));
+  CUDA_TRY(cudaMemcpy(P->d_let_off, let_off.data(), sizeof(uint32_t) * G, cudaMemcpyHostToDevice));
+  CUDA_TRY(cudaMemcpy(P->d_n_let, n_let.data(), sizeof(uint32_t) * G, cudaMemcpyHostToDevice));
+  return MC_OK;
+}
+
+static SourceModel source_model(const psl &P) {
+  SourceModel m{};
+  m.table = (const AliasEntry *)P.d_table; m.let_off = P.d_let_off; m.n_let = P.d_n_let;
+  m.n_groups = (int)P.groups.size(); m.n_ebin = P.n_ebin; m.n_sectors = P.n_sectors;
+  m.e_min = (float)P.psr.e_min; m.e_bin_width = (float)P.psr.e_bin_width; m.ring_width = (float)P.psr.ring_width;
+  m.z_phsp = (float)P.psr.z_phsp; m.inv_nsec = (float)(1.0 / P.n_sectors);
+  const jaws_t &j = P.jaws;
+  for (int s = 0; s < 3; ++s) {
+    m.sigma_src[s] = (float)P.psr.sigma_src[s]; m.z_src[s] = (float)P.psr.z_src[s]; m.particle_type[s] = P.psr.particle_type[s];
+    m.jaw_tx[s] = (float)((j.z_jx - P.psr.z_src[s]) / (P.psr.z_phsp - P.psr.z_src[s]));
+    m.jaw_ty[s] = (float)((j.z_jy - P.psr.z_src[s]) / (P.psr.z_phsp - P.psr.z_src[s]));
+  }
+  m.jx_lo = (float)(j.x1 * j.z_jx / j.sad); m.jx_hi = (float)(j.x2 * j.z_jx / j.sad);
+  m.jy_lo = (float)(j.y1 * j.z_jy / j.sad); m.jy_hi = (float)(j.y2 * j.z_jy / j.sad);
+  return m;
+}
+
+static BeamXf beam_xf(const beam_geom_t &b) {
+  BeamXf x{};
+  for (int i = 0; i < 3; ++i) x.iso[i] = (float)b.iso[i];
+  for (int i = 0; i < 9; ++i) x.R[i] = (float)b.R[i];
+  x.sad = (float)b.sad;
+  return x;
+}
+
+static Grid make_grid(const phantom_t &ph, long long *acc) {
+  Grid g{};
+  g.nx = ph.nx; g.ny = ph.ny; g.nz = ph.nz;
+  g.ox = (float)ph.ox; g.oy = (float)ph.oy; g.oz = (float)ph.oz;
+  g.dx = (float)ph.dx; g.dy = (float)ph.dy; g.dz = (float)ph.dz;
+  g.idx = (float)(1.0 / ph.dx); g.idy = (float)(1.0 / ph.dy); g.idz = (float)(1.0 / ph.dz);
+  g.density = ph.density; g.material = ph.material; g.acc = (unsigned long long *)acc;
+  return g;
+}
+
+static bool phantom_ok(const phantom_t *ph) {
+  return ph && ph->nx > 0 && ph->ny > 0 && ph->nz > 0 && ph->dx > 0 && ph->dy > 0 && ph->dz > 0 && ph->density && ph->material &&
+         (uint64_t)ph->nx * ph->ny * ph->nz < 0x7fffffffull;
+}
+
+// Persistent-grid size: every SM filled to the kernel's occupancy.
+template <typename K>
+static int persistent_blocks(K kernel) {
+  int dev = 0, sms = 0, per = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kernel, kThreads, 0);
+  return std::max(1, sms * std::max(1, per));
+}
+
+struct Timer {                                  // per-kernel-class CUDA-event timing (MC_FLAG_TIMING)
+  bool on = false; cudaStream_t st = nullptr;
+  std::vector<cudaEvent_t> ev[5];
+  void begin(int cls) { if (!on) return; cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, st); ev[cls].push_back(e); }
+  void end(int cls) { begin(cls); }
+  void collect(float ms[5]) {
+    for (int c = 0; c < 5; ++c) {
+      ms[c] = 0;
+      for (size_t i = 0; i + 1 < ev[c].size(); i += 2) { float t = 0; cudaEventElapsedTime(&t, ev[c][i], ev[c][i + 1]); ms[c] += t; }
+      for (cudaEvent_t e : ev[c]) cudaEventDestroy(e);
+      ev[c].clear();
+    }
+  }
+};
+
+// Everything the launch helpers need.
+struct Run {
+  cudaStream_t st; char *ws; Layout L; Grid g; Control *ctl;
+  uint64_t seed, n_total, perm_a; int flags; bool dbg;
+  unsigned long long *fp; uint64_t fp_base;
+  Timer tm; uint64_t launches[5] = {0, 0, 0, 0, 0};
+  int blocks_photon[2], blocks_electron[2];
+
+  Queue queue(const size_t off[3], unsigned *count, unsigned cap) const {
+    Queue q; q.a = (float4 *)(ws + off[0]); q.b = (float4 *)(ws + off[1]); q.c = (uint4 *)(ws + off[2]); q.count = count; q.cap = cap;
+    return q;
+  }
+  TransportArgs base_args() const {
+    TransportArgs a{};
+    a.g = g; a.ctl = ctl; a.seed = seed; a.n_total = n_total; a.perm_a = perm_a;
+    a.p0 = (const float4 *)(ws + L.p0); a.p1 = (const float4 *)(ws + L.p1);
+    a.eq = queue(L.eq, &ctl->n_eq, L.eq_cap); a.pq = queue(L.pq, &ctl->n_pq, L.pq_cap);
+    a.fp = fp; a.fp_base = fp_base;
+    a.electrons_local = (flags & MC_FLAG_ELECTRONS_LOCAL) ? 1 : 0;
+    a.static_lanes = (flags & MC_FLAG_STATIC_LANES) ? 1 : 0;
+    return a;
+  }
+  void photon(const TransportArgs &a) {
+    tm.begin(MC_K_PHOTON);
+    if (dbg) k_photon<true><<<blocks_photon[1], kThreads, 0, st>>>(a); else k_photon<false><<<blocks_photon[0], kThreads, 0, st>>>(a);
+    tm.end(MC_K_PHOTON); ++launches[MC_K_PHOTON];
+  }
+  void electron(const TransportArgs &a) {
+    tm.begin(MC_K_ELECTRON);
+    if (dbg) k_electron<true><<<blocks_electron[1], kThreads, 0, st>>>(a); else k_electron<false><<<blocks_electron[0], kThreads, 0, st>>>(a);
+    tm.end(MC_K_ELECTRON); ++launches[MC_K_ELECTRON];
+  }
+  void init_blocks() {
+    blocks_photon[0] = persistent_blocks(k_photon<false>); blocks_photon[1] = persistent_blocks(k_photon<true>);
+    blocks_electron[0] = persistent_blocks(k_electron<false>); blocks_electron[1] = persistent_blocks(k_electron<true>);
+  }
+  // photons of the particle buffer, then annihilation photons, then every queued electron
+  void transport_photon_batch(uint64_t first, bool debug_buffer, const unsigned *count_ptr) {
+    TransportArgs a = base_args();
+    a.src_kind = SRC_BUFFER; a.buffer_is_debug = debug_buffer; a.first = first; a.want_type = 0;
+    a.src_count = count_ptr; a.src_head = &ctl->head_pb;
+    photon(a);
+    TransportArgs b = base_args();
+    b.src_kind = SRC_QUEUE; b.src = b.pq; b.src_count = &ctl->n_pq; b.src_head = &ctl->head_pq;
+    b.pq.cap = 0;                              // 0.511 MeV photons cannot pair-produce; a push would flag overflow
+    photon(b);
+    drain_electrons();
+  }
+  void drain_electrons() {
+    TransportArgs c = base_args();
+    c.src_kind = SRC_QUEUE; c.src = c.eq; c.src_count = &ctl->n_eq; c.src_head = &ctl->head_eq;
+    electron(c);
+  }
+  void transport_electron_buffer(uint64_t first, bool debug_buffer, const unsigned *count_ptr, unsigned *head) {
+    TransportArgs a = base_args();
+    a.src_kind = SRC_BUFFER; a.buffer_is_debug = debug_buffer; a.first = first; a.want_type = 1;
+    a.src_count = count_ptr; a.src_head = head;
+    electron(a);
+  }
+};
+
+static void fold_stats(const Control &c, const Run &r, mc_stats_t *s) {
+  for (int k = 0; k < 4; ++k) {
+    unsigned __int128 tot = 0;
+    for (int sl = 0; sl < kLedgerSlots; ++sl) tot += ((unsigned __int128)c.ledger[sl][k][1] << 64) | c.ledger[sl][k][0];
+    s->ledger_hi[k] = (int64_t)(uint64_t)(tot >> 64); s->ledger_lo[k] = (uint64_t)tot;
+  }
+  s->n_missed = c.stat[ST_MISSED]; s->n_flights = c.stat[ST_FLIGHTS]; s->n_virtual = c.stat[ST_VIRTUAL];
+  s->n_compton = c.stat[ST_COMPTON]; s->n_photo = c.stat[ST_PHOTO]; s->n_pair = c.stat[ST_PAIR];
+  s->n_photon_cutoff = c.stat[ST_PCUT]; s->n_photon_escape = c.stat[ST_PESC]; s->n_uncollided_escape = c.stat[ST_UNCOLLIDED];
+  s->n_sec_electrons = c.stat[ST_SEC_E]; s->n_sec_photons = c.stat[ST_SEC_P];
+  s->n_electron_tracks = c.stat[ST_ETRACKS]; s->n_electron_steps = c.stat[ST_ESTEPS]; s->n_electron_escape = c.stat[ST_EESC];
+  s->n_deposits = c.stat[ST_DEPOSITS];
+  s->queue_high_water[0] = c.hw_eq; s->queue_high_water[1] = c.hw_pq;
+  for (int k = 0; k < 5; ++k) s->launches[k] = r.launches[k];
+}
+
+}  // namespace pslmc
+
+using namespace pslmc;
+
+static uint64_t gcd_u64(uint64_t a, uint64_t b) { while (b) { uint64_t t = a % b; a = b; b = t; } return a; }
+
+// Mixed order (ablation): thread t handles history (a*t) mod N, a = smallest integer >= floor(0.618...N) coprime to N.
+static uint64_t mixed_multiplier(uint64_t N) {
+  if (N < 3) return 1;
+  uint64_t a = (uint64_t)(0.6180339887 * (double)N);
+  if (a < 1) a = 1;
+  while (gcd_u64(a, N) != 1) ++a;
+  return a;
+}
+
+// The driver proper.  All pointers inside `ph` are DEVICE pointers here.
+static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam, uint64_t N, uint64_t seed, uint64_t batch,
+                    double *dose_out, const mc_opts_t *opts) {
+  static const mc_opts_t kDefaults = {};
+  if (!opts) opts = &kDefaults;
+  if (!P || !beam || !phantom_ok(ph) || N == 0 || batch == 0 || batch > (1ull << 30) || (!dose_out && !opts->dose_acc))
+    return fail(MC_E_INVALID_ARG, "mc_dose: invalid argument");
+  const uint64_t hb = opts->history_begin, he = opts->history_end ? opts->history_end : N;
+  if (hb > he || he > N) return fail(MC_E_INVALID_ARG, "mc_dose: history range outside [0, n_histories]");
+  const bool mixed = opts->order == MC_ORDER_MIXED;
+  if (mixed && (N >> 32)) return fail(MC_E_INVALID_ARG, "mc_dose: mixed order needs n_histories < 2^32");
+  if (mixed && opts->fingerprints && (hb != 0 || he != N)) return fail(MC_E_INVALID_ARG, "mc_dose: mixed order + fingerprints needs the full range");
+  int dev = 0; CUDA_TRY(cudaGetDevice(&dev));
+  if (dev != P->device) return fail(MC_E_INVALID_ARG, "mc_dose: psl_t was built on another device");
+
+  const size_t nvox = (size_t)ph->nx * ph->ny * ph->nz;
+  const Layout L = make_layout(batch, nvox, opts->dose_acc == nullptr);
+  void *ws = opts->workspace;
+  if (ws) { if (opts->workspace_bytes < L.total) return fail(MC_E_WORKSPACE, "mc_dose: workspace too small (see mc_workspace_bytes)"); }
+  else { int rc = scratch_get(g_scratch, L.total, &ws); if (rc) return rc; }
+
+  Run r{};
+  r.st = (cudaStream_t)opts->cuda_stream; r.ws = (char *)ws; r.L = L; r.ctl = (Control *)(r.ws + L.ctl);
+  long long *acc = opts->dose_acc ? (long long *)opts->dose_acc : (long long *)(r.ws + L.acc);
+  r.g = make_grid(*ph, acc);
+  r.seed = seed; r.n_total = N; r.perm_a = mixed ? mixed_multiplier(N) : 0; r.flags = opts->flags;
+  r.fp = (unsigned long long *)opts->fingerprints; r.fp_base = hb;
+  r.dbg = (opts->flags & MC_FLAG_STATS) || opts->fingerprints;
+  r.tm.on = (opts->flags & MC_FLAG_TIMING) != 0; r.tm.st = r.st;
+  r.init_blocks();
+
+  std::vector<uint64_t> off(P->groups.size() + 1);
+  allocate_host(*P, N, off.data());
+  unsigned long long *d_off = (unsigned long long *)(r.ws + L.off);
+
+  cudaEvent_t ev0, ev1;
+  CUDA_TRY(cudaEventCreate(&ev0)); CUDA_TRY(cudaEventCreate(&ev1));
+  CUDA_TRY(cudaEventRecord(ev0, r.st));
+  CUDA_TRY(cudaMemsetAsync(r.ctl, 0, sizeof(Control), r.st));
+  CUDA_TRY(cudaMemcpyAsync(d_off, off.data(), sizeof(uint64_t) * off.size(), cudaMemcpyHostToDevice, r.st));
+  if (!opts->dose_acc) CUDA_TRY(cudaMemsetAsync(acc, 0, 8 * nvox, r.st));
+  r.tm.begin(MC_K_AUX);
+  k_rhomax<<<296, 256, 0, r.st>>>(ph->density, ph->material, nvox, r.ctl);
+  r.tm.end(MC_K_AUX); ++r.launches[MC_K_AUX];
+
+  SampleArgs sa{};
+  sa.m = source_model(*P); sa.beam = beam_xf(*beam); sa.off_g = d_off; sa.seed = seed; sa.n_total = N; sa.perm_a = r.perm_a;
+  sa.p0 = (float4 *)(r.ws + L.p0); sa.p1 = (float4 *)(r.ws + L.p1); sa.ctl = r.ctl; sa.fp = r.fp; sa.fp_base = hb; sa.compact = 1;
+
+  memset(&g_stats, 0, sizeof g_stats);
+  auto sample_batch = [&](uint64_t first, uint64_t count) {
+    r.tm.begin(MC_K_AUX); k_next_batch<<<1, 1, 0, r.st>>>(r.ctl); r.tm.end(MC_K_AUX); ++r.launches[MC_K_AUX];
+    sa.first = first; sa.count = (unsigned)count;
+    r.tm.begin(MC_K_SAMPLE);
+    k_sample<<<(unsigned)((count + kThreads - 1) / kThreads), kThreads, 0, r.st>>>(sa);
+    r.tm.end(MC_K_SAMPLE); ++r.launches[MC_K_SAMPLE];
+  };
+  const int ne = P->n_ebin;
+  if (!mixed) {
+    // one sub-source type at a time, energy bins ascending, M histories per launch
+    for (int s = 0; s < 3; ++s) {
+      const uint64_t lo = std::max(hb, off[(size_t)s * ne]), hi = std::min(he, off[(size_t)(s + 1) * ne]);
+      if (lo >= hi) continue;
+      g_stats.n_hist[s] = hi - lo;
+      for (uint64_t first = lo; first < hi; first += batch) {
+        sample_batch(first, std::min(batch, hi - first));
+        if (P->psr.particle_type[s] == 0) r.transport_photon_batch(first, false, &r.ctl->n_pb);
+        else r.transport_electron_buffer(first, false, &r.ctl->n_pb, &r.ctl->head_pb);
+      }
+    }
+  } else {
+    for (int s = 0; s < 3; ++s) g_stats.n_hist[s] = 0;     // mixed: per-type counts are not tracked per range
+    for (uint64_t first = hb; first < he; first += batch) {
+      sample_batch(first, std::min(batch, he - first));
+      r.transport_electron_buffer(first, false, &r.ctl->n_pb, &r.ctl->pad0);
+      r.transport_photon_batch(first, false, &r.ctl->n_pb);
+    }
+    if (hb == 0 && he == N) for (int s = 0; s < 3; ++s) g_stats.n_hist[s] = off[(size_t)(s + 1) * ne] - off[(size_t)s * ne];
+  }
+  k_next_batch<<<1, 1, 0, r.st>>>(r.ctl); ++r.launches[MC_K_AUX];
+  if (dose_out) {
+    r.tm.begin(MC_K_FINALISE);
+    const double inv_vn = 1.0 / (ph->dx * ph->dy * ph->dz * (double)N);
+    k_finalise<<<592, 256, 0, r.st>>>(acc, ph->density, nvox, inv_vn, dose_out);
+    r.tm.end(MC_K_FINALISE); ++r.launches[MC_K_FINALISE];
+  }
+  CUDA_TRY(cudaEventRecord(ev1, r.st));
+  CUDA_TRY(cudaGetLastError());
+  Control hc;
+  CUDA_TRY(cudaMemcpyAsync(&hc, r.ctl, sizeof(Control), cudaMemcpyDeviceToHost, r.st));
+  CUDA_TRY(cudaStreamSynchronize(r.st));
+  CUDA_TRY(cudaEventElapsedTime(&g_stats.ms_total, ev0, ev1));
+  cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+  r.tm.collect(g_stats.ms);
+  fold_stats(hc, r, &g_stats);
+  g_stats.n_jaw_rejected = (he - hb) - hc.n_accepted;
+  if (hc.overflow) return fail(MC_E_OVERFLOW, "mc_dose: a secondary queue overflowed; use a larger batch workspace");
+  return MC_OK;
+}
+
+extern "C" void psl_free(psl_t *P) {
+  if (!P) return;
+  if (P->d_table) cudaFree(P->d_table);
+  if (P->d_let_off) cudaFree(P->d_let_off);
+  if (P->d_n_let) cudaFree(P->d_n_let);
+  delete P;
+}
+
+extern "C" size_t mc_workspace_bytes(const psl_t *P, const phantom_t *ph, uint64_t batch) {
+  if (!P || !ph || ph->nx <= 0 || ph->ny <= 0 || ph->nz <= 0 || batch == 0 || batch > (1ull << 30)) return 0;
+  return make_layout(batch, (size_t)ph->nx * ph->ny * ph->nz, true).total;
+}
+
+extern "C" int mc_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam, uint64_t n_histories, uint64_t seed,
+                       uint64_t batch, double *dose_out, const mc_opts_t *opts) {
+  return run_dose(P, ph, beam, n_histories, seed, batch, dose_out, opts);
+}
+
+extern "C" int mc_dose_host(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam, uint64_t n_histories, uint64_t seed,
+                            uint64_t batch, double *dose_out_host, const mc_opts_t *opts) {
+  if (!ph || ph->nx <= 0 || ph->ny <= 0 || ph->nz <= 0 || !ph->density || !ph->material || !dose_out_host)
+    return fail(MC_E_INVALID_ARG, "mc_dose_host: invalid argument");
+  const size_t nvox = (size_t)ph->nx * ph->ny * ph->nz;
+  const size_t o_rho = 0, o_mat = align_up(4 * nvox), o_dose = o_mat + align_up(nvox), total = o_dose + 8 * nvox;
+  void *io = nullptr;
+  int rc = scratch_get(g_hostio, total, &io); if (rc) return rc;
+  cudaStream_t st = opts ? (cudaStream_t)opts->cuda_stream : nullptr;
+  char *b = (char *)io;
+  CUDA_TRY(cudaMemcpyAsync(b + o_rho, ph->density, 4 * nvox, cudaMemcpyHostToDevice, st));
+  CUDA_TRY(cudaMemcpyAsync(b + o_mat, ph->material, nvox, cudaMemcpyHostToDevice, st));
+  phantom_t d = *ph; d.density = (const float *)(b + o_rho); d.material = (const uint8_t *)(b + o_mat);
+  rc = run_dose(P, &d, beam, n_histories, seed, batch, (double *)(b + o_dose), opts);
+  if (rc) return rc;
+  CUDA_TRY(cudaMemcpyAsync(dose_out_host, b + o_dose, 8 * nvox, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return MC_OK;
+}
+
+extern "C" int mc_stats(mc_stats_t *out) {
+  if (!out) return fail(MC_E_INVALID_ARG, "mc_stats: null argument");
+  *out = g_stats;
+  return MC_OK;
+}
+
+// ---------------------------------------------------------------- parity / debug exports
+extern "C" int mc_sample_debug(const psl_t *P, const beam_geom_t *beam, uint64_t first_history, uint64_t count,
+                               uint64_t n_histories, uint64_t seed, float *soa_out, void *cuda_stream) {
+  if (!P || !beam || !soa_out || n_histories == 0 || first_history + count > n_histories || count > 0x7fffffffull)
+    return fail(MC_E_INVALID_ARG, "mc_sample_debug: invalid argument");
+  if (count == 0) return MC_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::vector<uint64_t> off(P->groups.size() + 1);
+  allocate_host(*P, n_histories, off.data());
+  void *d_off = nullptr;
+  CUDA_TRY(cudaMalloc(&d_off, sizeof(uint64_t) * off.size()));
+  CUDA_TRY(cudaMemcpyAsync(d_off, off.data(), sizeof(uint64_t) * off.size(), cudaMemcpyHostToDevice, st));
+  SampleArgs sa{};
+  sa.m = source_model(*P); sa.beam = beam_xf(*beam); sa.off_g = (const unsigned long long *)d_off;
+  sa.seed = seed; sa.first = first_history; sa.n_total = n_histories; sa.perm_a = 0; sa.count = (unsigned)count;
+  sa.p0 = (float4 *)soa_out; sa.p1 = (float4 *)soa_out + count; sa.ctl = nullptr; sa.fp = nullptr; sa.compact = 0;
+  k_sample<<<(unsigned)((count + kThreads - 1) / kThreads), kThreads, 0, st>>>(sa);
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaStreamSynchronize(st));
+  cudaFree(d_off);
+  return MC_OK;
+}
+
+extern "C" int mc_transport_debug(const phantom_t *ph, int32_t particle_type, const float *soa_in, uint64_t first_history,
+                                  uint64_t count, uint64_t seed, const mc_opts_t *opts) {
+  if (!phantom_ok(ph) || !soa_in || !opts || !opts->dose_acc || (particle_type != 0 && particle_type != 1) || count > (1ull << 30))
+    return fail(MC_E_INVALID_ARG, "mc_transport_debug: invalid argument (opts->dose_acc is required)");
+  memset(&g_stats, 0, sizeof g_stats);
+  if (count == 0) return MC_OK;
+  const size_t nvox = (size_t)ph->nx * ph->ny * ph->nz;
+  const Layout L = make_layout(count, nvox, false);
+  void *ws = opts->workspace;
+  if (ws) { if (opts->workspace_bytes < L.total) return fail(MC_E_WORKSPACE, "mc_transport_debug: workspace too small"); }
+  else { int rc = scratch_get(g_scratch, L.total, &ws); if (rc) return rc; }
+  Run r{};
+  r.st = (cudaStream_t)opts->cuda_stream; r.ws = (char *)ws; r.L = L; r.ctl = (Control *)(r.ws + L.ctl);
+  r.g = make_grid(*ph, (long long *)opts->dose_acc);
+  r.seed = seed; r.n_total = first_history + count; r.perm_a = 0; r.flags = opts->flags;
+  r.fp = (unsigned long long *)opts->fingerprints; r.fp_base = first_history;
+  r.dbg = true; r.tm.on = false; r.init_blocks();
+  cudaEvent_t ev0, ev1;
+  CUDA_TRY(cudaEventCreate(&ev0)); CUDA_TRY(cudaEventCreate(&ev1));
+  CUDA_TRY(cudaEventRecord(ev0, r.st));
+  CUDA_TRY(cudaMemsetAsync(r.ctl, 0, sizeof(Control), r.st));
+  k_rhomax<<<296, 256, 0, r.st>>>(ph->density, ph->material, nvox, r.ctl);
+  // the caller's planes stand in for the particle buffer; n_pb = count
+  const unsigned cnt = (unsigned)count;
+  CUDA_TRY(cudaMemcpyAsync(&r.ctl->n_pb, &cnt, sizeof cnt, cudaMemcpyHostToDevice, r.st));
+  TransportArgs a = r.base_args();
+  a.p0 = (const float4 *)soa_in; a.p1 = (const float4 *)soa_in + count;
+  a.src_kind = SRC_BUFFER; a.buffer_is_debug = 1; a.first = first_history; a.want_type = particle_type;
+  a.src_count = &r.ctl->n_pb; a.src_head = &r.ctl->head_pb;
+  if (particle_type == 0) {
+    r.photon(a);
+    TransportArgs b = r.base_args();
+    b.src_kind = SRC_QUEUE; b.src = b.pq; b.src_count = &r.ctl->n_pq; b.src_head = &r.ctl->head_pq; b.pq.cap = 0;
+    r.photon(b);
+    r.drain_electrons();
+  } else {
+    r.electron(a);
+  }
+  k_next_batch<<<1, 1, 0, r.st>>>(r.ctl);
+  CUDA_TRY(cudaEventRecord(ev1, r.st));
+  CUDA_TRY(cudaGetLastError());
+  Control hc;
+  CUDA_TRY(cudaMemcpyAsync(&hc, r.ctl, sizeof(Control), cudaMemcpyDeviceToHost, r.st));
+  CUDA_TRY(cudaStreamSynchronize(r.st));
+  CUDA_TRY(cudaEventElapsedTime(&g_stats.ms_total, ev0, ev1));
+  cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+  fold_stats(hc, r, &g_stats);
+  if (hc.overflow) return fail(MC_E_OVERFLOW, "mc_transport_debug: a secondary queue overflowed");
+  return MC_OK;
+}
+
+extern "C" int mc_philox_debug(uint64_t seed, uint64_t history, uint32_t track, uint32_t block, uint32_t *out) {
+  if (!out) return fail(MC_E_INVALID_ARG, "mc_philox_debug: null argument");
+  uint32_t *d = nullptr;
+  CUDA_TRY(cudaMalloc((void **)&d, 16));
+  k_philox_debug<<<1, 1>>>(seed, history, track, block, d);
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaMemcpy(out, d, 16, cudaMemcpyDeviceToHost));
+  cudaFree(d);
+  return MC_OK;
+}

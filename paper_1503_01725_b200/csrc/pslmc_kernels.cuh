@@ -1,0 +1,207 @@
+// pslmc_kernels.cuh — the kernels of the hot path: k_sample (PAPER.md:82-116 S3-S5), k_photon,
+// k_electron (physics DESIGN.md P1-P9), secondary queues, finalise.
+#pragma once
+#include "pslmc_device.cuh"
+
+namespace pslmc {
+
+constexpr int kThreads = 256;
+constexpr int kLedgerSlots = 32;
+constexpr unsigned kFull = 0xffffffffu;
+
+enum Stat {
+  ST_MISSED = 0, ST_FLIGHTS, ST_VIRTUAL, ST_COMPTON, ST_PHOTO, ST_PAIR, ST_PCUT, ST_PESC, ST_UNCOLLIDED,
+  ST_SEC_E, ST_SEC_P, ST_ETRACKS, ST_ESTEPS, ST_EESC, ST_DEPOSITS, ST_COUNT
+};
+
+// Device-resident control block.  `batch` part is reset by k_next_batch, the rest once per call.
+struct Control {
+  // per batch
+  unsigned n_pb, head_pb;          // particle buffer: entries written by k_sample, consume cursor
+  unsigned n_eq, head_eq;          // electron queue
+  unsigned n_pq, head_pq;          // photon queue (annihilation photons)
+  unsigned pad0, pad1;
+  // per call
+  unsigned overflow;               // a queue was full: result invalid → MC_E_OVERFLOW
+  unsigned hw_eq, hw_pq;           // queue high-water marks
+  unsigned pad2;
+  unsigned long long n_accepted;   // primaries that passed the jaws
+  unsigned long long ledger[kLedgerSlots][4][2];   // [slot][incident,deposited,escaped,jaw][lo,hi] quanta
+  unsigned long long stat[ST_COUNT];
+  float rhomax[4];                 // largest density per material (as float, written via atomicMax on bits)
+};
+
+// One alias-table entry, 16 B: everything k_sample needs after picking a column.
+struct __align__(16) AliasEntry {
+  uint32_t thresh;                 // accept column if frac < thresh
+  uint16_t ring_c, sector_c;       // the column's own let
+  uint16_t ring_a, sector_a;       // the alias let
+  uint32_t pad;
+};
+
+struct SourceModel {               // read-only, uploaded once by psl_build
+  const AliasEntry *table;         // all groups back to back
+  const uint32_t *let_off;         // [G] first entry of group g
+  const uint32_t *n_let;           // [G]
+  int n_groups, n_ebin, n_sectors;
+  float e_min, e_bin_width, ring_width, z_phsp, inv_nsec;
+  float sigma_src[3], z_src[3];
+  int particle_type[3];
+  float jaw_tx[3], jaw_ty[3];      // (z_jx - z_s)/(z_p - z_s), (z_jy - z_s)/(z_p - z_s)
+  float jx_lo, jx_hi, jy_lo, jy_hi;   // jaw edges on their own planes
+};
+
+struct BeamXf { float iso[3]; float R[9]; float sad; };
+
+struct SampleArgs {
+  SourceModel m;
+  BeamXf beam;
+  const unsigned long long *off_g;   // [G+1] device
+  unsigned long long seed, first, n_total, perm_a;   // perm_a != 0 → mixed order: h = (perm_a * t) mod n_total
+  unsigned count;
+  float4 *p0, *p1;                   // outputs (two float4 planes)
+  Control *ctl;
+  unsigned long long *fp;            // fingerprints or null
+  unsigned long long fp_base;
+  int compact;                       // 1: survivors packed, p1.w = local index bits; 0: indexed by t, p1.w = status
+};
+
+__device__ __forceinline__ unsigned long long history_of(unsigned long long t, unsigned long long perm_a, unsigned long long n_total) {
+  return perm_a ? (perm_a * t) % n_total : t;
+}
+
+// ------------------------------------------------------------------ k_sample
+__global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ SampleArgs a) {
+  __shared__ unsigned long long s_off[160];
+  __shared__ unsigned long long s_led[kThreads / 32][2];
+  const SourceModel &m = a.m;
+  for (int i = threadIdx.x; i <= m.n_groups; i += kThreads) s_off[i] = a.off_g[i];
+  __syncthreads();
+  const unsigned t = blockIdx.x * kThreads + threadIdx.x;
+  const unsigned lane = threadIdx.x & 31u;
+  const bool live = t < a.count;
+  unsigned long long q_inc = 0, q_jaw = 0;
+  bool pass = false;
+  float4 o0 = make_float4(0.f, 0.f, 0.f, 0.f), o1 = o0;
+  int g = 0;
+  if (live) {
+    const unsigned long long h = history_of(a.first + t, a.perm_a, a.n_total);
+    // group of h: last g with off[g] <= h (empty groups have off[g] == off[g+1] and are skipped by "last")
+    int lo = 0, hi = m.n_groups;           // invariant: off[lo] <= h < off[hi]
+    while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (s_off[mid] <= h) lo = mid; else hi = mid; }
+    g = lo;
+    const int stype = g / m.n_ebin, ebin = g - stype * m.n_ebin;
+    Philox rng; rng.init(a.seed, h, 0u, 0u);
+    const uint32_t x0 = rng.next(), x1 = rng.next(), x2 = rng.next(), x3 = rng.next();
+    const uint32_t y0 = rng.next(), y1 = rng.next();
+    // 1. let through the alias table
+    const unsigned long long mm = (unsigned long long)x0 * m.n_let[g];
+    const uint32_t col = (uint32_t)(mm >> 32), frac = (uint32_t)mm;
+    const AliasEntry e = m.table[m.let_off[g] + col];
+    const bool own = frac < e.thresh;
+    const float ring = (float)(own ? e.ring_c : e.ring_a), sector = (float)(own ? e.sector_c : e.sector_a);
+    // 2. position uniform in the let's area
+    const float r0 = ring * m.ring_width, r1 = (ring + 1.0f) * m.ring_width;
+    const float r = sqrtf(r0 * r0 + u_co(x1) * (r1 * r1 - r0 * r0));
+    float sn, cs;
+    sincospif(2.0f * (sector + u_co(x2)) * m.inv_nsec, &sn, &cs);
+    const float px = r * cs, py = r * sn, pz = m.z_phsp;
+    // 3. energy uniform in the bin
+    const float E = (m.e_min + (float)ebin * m.e_bin_width) + u_oc(x3) * m.e_bin_width;
+    // 4. source point on the sub-source's Gaussian (Eq. 4)
+    const float rho = m.sigma_src[stype] * sqrtf(-2.0f * logf(u_oc(y0)));
+    sincospif(2.0f * u_co(y1), &sn, &cs);
+    const float qx = rho * cs, qy = rho * sn, qz = m.z_src[stype];
+    // 5. direction (Eq. 5)
+    float dx = px - qx, dy = py - qy, dz = pz - qz;
+    const float il = rsqrtf(dx * dx + dy * dy + dz * dz);
+    dx *= il; dy *= il; dz *= il;
+    // 6. thin-jaw test
+    const float xj = qx + (px - qx) * m.jaw_tx[stype], yj = qy + (py - qy) * m.jaw_ty[stype];
+    pass = xj >= m.jx_lo && xj <= m.jx_hi && yj >= m.jy_lo && yj <= m.jy_hi;
+    // 7. beam set-up
+    const float *R = a.beam.R;
+    const float bz = pz - a.beam.sad;
+    o0.x = a.beam.iso[0] + R[0] * px + R[1] * py + R[2] * bz;
+    o0.y = a.beam.iso[1] + R[3] * px + R[4] * py + R[5] * bz;
+    o0.z = a.beam.iso[2] + R[6] * px + R[7] * py + R[8] * bz;
+    o0.w = E;
+    o1.x = R[0] * dx + R[1] * dy + R[2] * dz;
+    o1.y = R[3] * dx + R[4] * dy + R[5] * dz;
+    o1.z = R[6] * dx + R[7] * dy + R[8] * dz;
+    q_inc = (unsigned long long)quanta(E);
+    if (!pass) {
+      q_jaw = q_inc;
+      if (a.fp) {
+        Fnv f; f.init(0u); f.byte('J');
+        atomicAdd(a.fp + (h - a.fp_base), f.v);
+      }
+    }
+  }
+  if (a.compact) {
+    // survivors packed with one queue-tail atomic per warp
+    const unsigned keep = __ballot_sync(kFull, live && pass);
+    unsigned base = 0;
+    if (lane == 0 && keep) base = atomicAdd(&a.ctl->n_pb, __popc(keep));
+    base = __shfl_sync(kFull, base, 0);
+    if (live && pass) {
+      const unsigned dst = base + __popc(keep & ((1u << lane) - 1u));
+      o1.w = __uint_as_float(t | ((unsigned)m.particle_type[g / m.n_ebin] << 31));
+      a.p0[dst] = o0; a.p1[dst] = o1;
+    }
+  } else if (live) {
+    o1.w = pass ? (float)g : -(float)g - 1.0f;
+    a.p0[t] = o0; a.p1[t] = o1;
+  }
+  // ledgers: incident and jaw-rejected energy, block-reduced, spread over slots
+  if (a.ctl) {
+    q_inc = warp_sum_u64(q_inc); q_jaw = warp_sum_u64(q_jaw);
+    if (lane == 0) { s_led[threadIdx.x >> 5][0] = q_inc; s_led[threadIdx.x >> 5][1] = q_jaw; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      unsigned long long si = 0, sj = 0;
+      for (int w = 0; w < kThreads / 32; ++w) { si += s_led[w][0]; sj += s_led[w][1]; }
+      unsigned long long (*L)[2] = a.ctl->ledger[blockIdx.x % kLedgerSlots];
+      add128(L[0], si); add128(L[3], sj);
+    }
+  }
+}
+
+// ------------------------------------------------------------------ small helpers
+// Folds the finished batch's counters into the per-call totals and resets them.
+__global__ void k_next_batch(Control *c) {
+  c->n_accepted += c->n_pb;
+  c->hw_eq = max(c->hw_eq, c->n_eq); c->hw_pq = max(c->hw_pq, c->n_pq);
+  c->n_pb = c->head_pb = c->n_eq = c->head_eq = c->n_pq = c->head_pq = c->pad0 = c->pad1 = 0;
+}
+
+// Largest density per material (Woodcock majorant input).  Densities are >= 0, so float order = uint order.
+__global__ void k_rhomax(const float *density, const uint8_t *material, size_t n, Control *c) {
+  float best[3] = {0.f, 0.f, 0.f};
+  for (size_t v = blockIdx.x * (size_t)blockDim.x + threadIdx.x; v < n; v += (size_t)gridDim.x * blockDim.x) {
+    const float d = density[v]; const int mt = material[v];
+    if (mt == 0) best[0] = fmaxf(best[0], d); else if (mt == 1) best[1] = fmaxf(best[1], d); else best[2] = fmaxf(best[2], d);
+  }
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    float b = best[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) b = fmaxf(b, __shfl_xor_sync(kFull, b, o));
+    if ((threadIdx.x & 31) == 0 && b > 0.f) atomicMax((unsigned *)&c->rhomax[k], __float_as_uint(b));
+  }
+}
+
+// dose[v] = acc[v] 2^-32 / (rho_v V N)
+__global__ void k_finalise(const long long *acc, const float *density, size_t n, double inv_vn, double *dose) {
+  for (size_t v = blockIdx.x * (size_t)blockDim.x + threadIdx.x; v < n; v += (size_t)gridDim.x * blockDim.x) {
+    const float rho = density[v];
+    dose[v] = rho > 0.f ? (double)acc[v] * (1.0 / 4294967296.0) * inv_vn / (double)rho : 0.0;
+  }
+}
+
+__global__ void k_philox_debug(unsigned long long seed, unsigned long long h, uint32_t track, uint32_t block, uint32_t *out) {
+  Philox r; r.init(seed, h, track, 0u); r.block(block);
+  out[0] = r.w0; out[1] = r.w1; out[2] = r.w2; out[3] = r.w3;
+}
+
+}  // namespace pslmc

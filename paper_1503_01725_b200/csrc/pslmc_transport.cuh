@@ -1,0 +1,333 @@
+// pslmc_transport.cuh — k_photon and k_electron: persistent warps with lane refill, Woodcock photon
+// flights with Klein–Nishina/Kahn Compton, condensed-history electrons, warp-compacted secondary
+// queues, int64 fixed-point scoring.  PAPER.md:118-120 (iterated kernels), :161 (cut-offs);
+// physics per DESIGN.md P1-P9.
+#pragma once
+#include "pslmc_kernels.cuh"
+
+namespace pslmc {
+
+// A queue of tracks: three 16-byte planes so every lane store/load is one 128-bit access.
+struct Queue {
+  float4 *a;            // x, y, z, E
+  float4 *b;            // u, v, w, (unused)
+  uint4  *c;            // hist_lo, hist_hi, track, (unused)
+  unsigned *count;      // tail (device)
+  unsigned cap;
+};
+
+enum { SRC_BUFFER = 0, SRC_QUEUE = 1 };
+
+struct TransportArgs {
+  Grid g;
+  Control *ctl;
+  unsigned long long seed;
+  // source
+  int src_kind;                       // SRC_BUFFER: p0/p1 planes from k_sample;  SRC_QUEUE: src queue
+  int buffer_is_debug;                // SRC_BUFFER only: 1 = indexed by history, p1.w = status (skip < 0)
+  const float4 *p0, *p1;
+  Queue src;
+  const unsigned *src_count;          // entries available (device)
+  unsigned *src_head;                 // consume cursor (device)
+  unsigned long long first, n_total, perm_a;
+  // sinks
+  Queue eq, pq;
+  // options
+  unsigned long long *fp; unsigned long long fp_base;
+  int electrons_local, static_lanes;
+  int want_type;                      // SRC_BUFFER, compact: take only entries of this particle type (bit 31 of p1.w)
+};
+
+struct Tally {                         // per-thread running sums, flushed once at kernel exit
+  unsigned long long inc, dep, esc;
+  unsigned st[ST_COUNT];
+};
+
+template <bool DBG>
+__device__ __forceinline__ void tally_flush(const TransportArgs &a, Tally &t) {
+  unsigned long long inc = warp_sum_u64(t.inc), dep = warp_sum_u64(t.dep), esc = warp_sum_u64(t.esc);
+  if ((threadIdx.x & 31) == 0) {
+    unsigned long long (*L)[2] = a.ctl->ledger[(blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5)) % kLedgerSlots];
+    add128(L[0], inc); add128(L[1], dep); add128(L[2], esc);
+  }
+  if (DBG) {
+#pragma unroll
+    for (int s = 0; s < ST_COUNT; ++s) {
+      unsigned v = __reduce_add_sync(kFull, t.st[s]);
+      if ((threadIdx.x & 31) == 0 && v) atomicAdd(&a.ctl->stat[s], (unsigned long long)v);
+    }
+  }
+}
+
+// Pending deposit: consecutive deposits into one voxel are merged before the atomic (integers: exact).
+struct Pending {
+  int v; long long q;
+  __device__ __forceinline__ void flush(const Grid &g) { if (q) atomicAdd(g.acc + v, (unsigned long long)q); q = 0; }
+  __device__ __forceinline__ void add(const Grid &g, int vox, long long dq) {
+    if (vox != v) { flush(g); v = vox; }
+    q += dq;
+  }
+};
+
+template <bool DBG>
+__device__ __forceinline__ void finish_track(const TransportArgs &a, unsigned long long h, const Fnv &f) {
+  if (DBG && a.fp) atomicAdd(a.fp + (h - a.fp_base), f.v);
+}
+
+// Warp-aggregated push: lanes with `want` get consecutive slots behind one atomic.  Convergent call.
+__device__ __forceinline__ bool queue_reserve(const Queue &q, Control *ctl, bool want, unsigned &slot) {
+  const unsigned m = __ballot_sync(kFull, want);
+  if (!m) return false;
+  const unsigned lane = threadIdx.x & 31u;
+  unsigned base = 0;
+  if (lane == (unsigned)(__ffs(m) - 1)) base = atomicAdd(q.count, __popc(m));
+  base = __shfl_sync(kFull, base, __ffs(m) - 1);
+  slot = base + __popc(m & ((1u << lane) - 1u));
+  if (want && slot >= q.cap) { ctl->overflow = 1u; return false; }
+  return want;
+}
+// Divergent-context push of one track (rare paths: pair production).
+__device__ __forceinline__ void queue_push1(const Queue &q, Control *ctl, float x, float y, float z, float E,
+                                            float u, float v, float w, unsigned long long h, uint32_t track) {
+  const unsigned slot = atomicAdd(q.count, 1u);
+  if (slot >= q.cap) { ctl->overflow = 1u; return; }
+  q.a[slot] = make_float4(x, y, z, E); q.b[slot] = make_float4(u, v, w, 0.f);
+  q.c[slot] = make_uint4((uint32_t)h, (uint32_t)(h >> 32), track, 0u);
+}
+
+// Refill protocol shared by both kernels: lanes without a track take the next source indices.
+// Returns the source index for this lane or 0xffffffff.  `exhausted` becomes true (warp-uniform)
+// once the cursor passed the end.
+__device__ __forceinline__ unsigned refill_index(const TransportArgs &a, bool idle, unsigned count, bool &exhausted) {
+  const unsigned need = __ballot_sync(kFull, idle);
+  if (!need || exhausted) return 0xffffffffu;
+  if (a.static_lanes && need != kFull) return 0xffffffffu;       // ablation: a warp refills only when all lanes are done
+  const unsigned lane = threadIdx.x & 31u, leader = __ffs(need) - 1;
+  unsigned base = 0;
+  if (lane == leader) base = atomicAdd(a.src_head, __popc(need));
+  base = __shfl_sync(kFull, base, leader);
+  if (base + __popc(need) >= count) exhausted = true;
+  const unsigned idx = base + __popc(need & ((1u << lane) - 1u));
+  return (idle && idx < count) ? idx : 0xffffffffu;
+}
+
+struct TrackIn { float x, y, z, u, v, w, E; unsigned long long h; uint32_t track, ndraw; bool ok; };
+
+__device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned idx) {
+  TrackIn t;
+  if (a.src_kind == SRC_BUFFER) {
+    const float4 A = a.p0[idx], B = a.p1[idx];
+    t.x = A.x; t.y = A.y; t.z = A.z; t.E = A.w; t.u = B.x; t.v = B.y; t.w = B.z;
+    unsigned long long tt;
+    if (a.buffer_is_debug) { tt = idx; t.ok = B.w >= 0.0f; }
+    else { const unsigned bits = __float_as_uint(B.w); tt = bits & 0x7fffffffu; t.ok = (int)(bits >> 31) == a.want_type; }
+    t.h = history_of(a.first + tt, a.perm_a, a.n_total);
+    t.track = 0u; t.ndraw = 8u;
+  } else {
+    const float4 A = a.src.a[idx], B = a.src.b[idx]; const uint4 C = a.src.c[idx];
+    t.x = A.x; t.y = A.y; t.z = A.z; t.E = A.w; t.u = B.x; t.v = B.y; t.w = B.z;
+    t.h = ((unsigned long long)C.y << 32) | C.x; t.track = C.z; t.ndraw = 0u; t.ok = true;
+  }
+  return t;
+}
+
+// ------------------------------------------------------------------ k_photon
+template <bool DBG>
+__global__ void __launch_bounds__(kThreads) k_photon(const __grid_constant__ TransportArgs a) {
+  const Grid &g = a.g;
+  const float rhomax[3] = {a.ctl->rhomax[0], a.ctl->rhomax[1], a.ctl->rhomax[2]};
+  const unsigned count = *a.src_count;
+  Tally tl; tl.inc = tl.dep = tl.esc = 0;
+  if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
+  Pending pend; pend.v = 0; pend.q = 0;
+  bool active = false, exhausted = false, collided = false;
+  float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, E = 0;
+  int vi = 0, vj = 0, vk = 0;
+  unsigned long long h = 0; uint32_t nchild = 0;
+  Philox rng; rng.n = 0; rng.track = 0; rng.k0 = rng.k1 = rng.hlo = rng.hhi = 0; rng.w0 = rng.w1 = rng.w2 = rng.w3 = 0;
+  PhotonXs xs; xs.skn = xs.inv_e3 = xs.lp2 = xs.mu_max = 0;
+  Fnv fnv; fnv.v = 0;
+
+  for (;;) {
+    // ---- refill idle lanes
+    const unsigned idx = refill_index(a, !active, count, exhausted);
+    if (idx != 0xffffffffu) {
+      const TrackIn t = load_track(a, idx);
+      if (t.ok) {
+        x = t.x; y = t.y; z = t.z; u = t.u; v = t.v; w = t.w; E = t.E; h = t.h; nchild = 0; collided = false;
+        rng.init(a.seed, h, t.track, t.ndraw);
+        if (DBG) fnv.init(t.track);
+        if (a.src_kind == SRC_BUFFER && a.buffer_is_debug) tl.inc += (unsigned long long)quanta(E);
+        active = true;
+        if (!locate(g, x, y, z, vi, vj, vk) && !enter(g, x, y, z, u, v, w, vi, vj, vk)) {
+          tl.esc += (unsigned long long)quanta(E);
+          if (DBG) { fnv.byte('M'); ++tl.st[ST_MISSED]; finish_track<DBG>(a, h, fnv); }
+          active = false;
+        } else xs.set(E, rhomax);
+      }
+    }
+    if (!__any_sync(kFull, active)) { if (exhausted) break; else continue; }
+
+    // ---- one Woodcock flight (+ interaction) per active lane
+    bool push_e = false; float ex = 0, ey = 0, ez = 0, eT = 0; uint32_t etrack = 0;
+    if (active) {
+      bool done = false;
+      if (E < kPcut) {                                   // below cut-off: absorbed on the spot
+        const long long q = quanta(E); pend.add(g, vox_index(g, vi, vj, vk), q); tl.dep += (unsigned long long)q;
+        if (DBG) { fnv.byte('A'); ++tl.st[ST_PCUT]; ++tl.st[ST_DEPOSITS]; }
+        done = true;
+      } else if (!(xs.mu_max > 0.0f)) {
+        tl.esc += (unsigned long long)quanta(E);
+        if (DBG) { fnv.byte('E'); ++tl.st[ST_PESC]; if (!collided && rng.track == 0u) ++tl.st[ST_UNCOLLIDED]; }
+        done = true;
+      } else {
+        const float s = -logf(u_oc(rng.next())) / xs.mu_max;
+        x += s * u; y += s * v; z += s * w;
+        if (DBG) ++tl.st[ST_FLIGHTS];
+        if (!locate(g, x, y, z, vi, vj, vk)) {
+          tl.esc += (unsigned long long)quanta(E);
+          if (DBG) { fnv.byte('E'); ++tl.st[ST_PESC]; if (!collided && rng.track == 0u) ++tl.st[ST_UNCOLLIDED]; }
+          done = true;
+        } else {
+          const int vox = vox_index(g, vi, vj, vk);
+          const float rho = __ldg(g.density + vox); const int mt = __ldg(g.material + vox);
+          const float muC = rho * (c_mat.ne[mt] * xs.skn), muT = rho * (c_mat.cphoto[mt] * xs.inv_e3), muK = rho * (c_mat.ppair[mt] * xs.lp2);
+          const float tt = u_co(rng.next()) * xs.mu_max;
+          if (tt < muC) {                                // Compton
+            collided = true;
+            if (DBG) { fnv.byte('C'); ++tl.st[ST_COMPTON]; }
+            const float alpha = E / kMe, eta = kahn(alpha, rng);
+            const float k = (eta - 1.0f) / alpha, ct = 1.0f - k, sn = sqrtf(fmaxf(0.0f, k * (2.0f - k)));
+            const float uphi = u_co(rng.next());
+            const float Ep = E / eta, T = E - Ep, u0 = u, v0 = v, w0 = w;
+            rotate(u, v, w, ct, sn, uphi);
+            if (T >= kEcut && !a.electrons_local) {
+              float dxe = E * u0 - Ep * u, dye = E * v0 - Ep * v, dze = E * w0 - Ep * w;
+              const float n2 = dxe * dxe + dye * dye + dze * dze;
+              if (n2 > 0.0f) { const float inv = rsqrtf(n2); ex = dxe * inv; ey = dye * inv; ez = dze * inv; }
+              else { ex = u0; ey = v0; ez = w0; }
+              eT = T; etrack = child_track(rng.track, nchild, 0u); push_e = true;
+              if (DBG) ++tl.st[ST_SEC_E];
+            } else {
+              const long long q = quanta(T); pend.add(g, vox, q); tl.dep += (unsigned long long)q;
+              if (DBG) ++tl.st[ST_DEPOSITS];
+            }
+            ++nchild; E = Ep; xs.set(E, rhomax);
+          } else if (tt < muC + muT) {                   // photo-electric: local absorption
+            const long long q = quanta(E); pend.add(g, vox, q); tl.dep += (unsigned long long)q;
+            if (DBG) { fnv.byte('P'); ++tl.st[ST_PHOTO]; ++tl.st[ST_DEPOSITS]; }
+            done = true;
+          } else if (tt < muC + muT + muK) {             // pair production (rare: plain per-lane pushes)
+            if (DBG) { fnv.byte('X'); ++tl.st[ST_PAIR]; }
+            const float Tsum = E - kEPair, Tm = u_co(rng.next()) * Tsum, Tp = Tsum - Tm;
+            const float Tc[2] = {Tm, Tp};
+#pragma unroll
+            for (int sl = 0; sl < 2; ++sl) {
+              if (Tc[sl] >= kEcut && !a.electrons_local) {
+                queue_push1(a.eq, a.ctl, x, y, z, Tc[sl], u, v, w, h, child_track(rng.track, nchild, sl));
+                if (DBG) ++tl.st[ST_SEC_E];
+              } else {
+                const long long q = quanta(Tc[sl]); pend.add(g, vox, q); tl.dep += (unsigned long long)q;
+                if (DBG) ++tl.st[ST_DEPOSITS];
+              }
+            }
+            const float cz = 2.0f * u_co(rng.next()) - 1.0f, sz = sqrtf(fmaxf(0.0f, 1.0f - cz * cz));
+            float sa, ca; sincospif(2.0f * u_co(rng.next()), &sa, &ca);
+            const float nx = sz * ca, ny = sz * sa;
+            queue_push1(a.pq, a.ctl, x, y, z, kEAnnih, nx, ny, cz, h, child_track(rng.track, nchild, 2u));
+            queue_push1(a.pq, a.ctl, x, y, z, kEAnnih, -nx, -ny, -cz, h, child_track(rng.track, nchild, 3u));
+            if (DBG) tl.st[ST_SEC_P] += 2;
+            done = true;
+          } else if (DBG) { fnv.byte('V'); ++tl.st[ST_VIRTUAL]; }
+        }
+      }
+      if (done) { if (DBG) finish_track<DBG>(a, h, fnv); active = false; }
+    }
+    // ---- Compton electrons: warp ballot + prefix sum, one tail atomic per warp
+    unsigned slot;
+    if (queue_reserve(a.eq, a.ctl, push_e, slot)) {
+      a.eq.a[slot] = make_float4(x, y, z, eT); a.eq.b[slot] = make_float4(ex, ey, ez, 0.f);
+      a.eq.c[slot] = make_uint4((uint32_t)h, (uint32_t)(h >> 32), etrack, 0u);
+    }
+  }
+  pend.flush(g);
+  tally_flush<DBG>(a, tl);
+}
+
+// ------------------------------------------------------------------ k_electron
+template <bool DBG>
+__global__ void __launch_bounds__(kThreads) k_electron(const __grid_constant__ TransportArgs a) {
+  const Grid &g = a.g;
+  const unsigned count = *a.src_count;
+  Tally tl; tl.inc = tl.dep = tl.esc = 0;
+  if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
+  Pending pend; pend.v = 0; pend.q = 0;
+  bool active = false, exhausted = false;
+  float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, T = 0;
+  int vi = 0, vj = 0, vk = 0;
+  unsigned long long h = 0; uint32_t steps = 0;
+  Philox rng; rng.n = 0; rng.track = 0; rng.k0 = rng.k1 = rng.hlo = rng.hhi = 0; rng.w0 = rng.w1 = rng.w2 = rng.w3 = 0;
+  Fnv fnv; fnv.v = 0;
+
+  for (;;) {
+    const unsigned idx = refill_index(a, !active, count, exhausted);
+    if (idx != 0xffffffffu) {
+      const TrackIn t = load_track(a, idx);
+      if (t.ok) {
+        x = t.x; y = t.y; z = t.z; u = t.u; v = t.v; w = t.w; T = t.E; h = t.h; steps = 0;
+        rng.init(a.seed, h, t.track, t.ndraw);
+        if (DBG) { fnv.init(t.track); ++tl.st[ST_ETRACKS]; }
+        if (a.src_kind == SRC_BUFFER && a.buffer_is_debug) tl.inc += (unsigned long long)quanta(T);
+        active = true;
+        if (!locate(g, x, y, z, vi, vj, vk) && !enter(g, x, y, z, u, v, w, vi, vj, vk)) {
+          tl.esc += (unsigned long long)quanta(T);
+          if (DBG) { fnv.u32(0u); fnv.byte('M'); ++tl.st[ST_MISSED]; finish_track<DBG>(a, h, fnv); }
+          active = false;
+        }
+      }
+    }
+    if (!__any_sync(kFull, active)) { if (exhausted) break; else continue; }
+
+    if (active) {                                        // one condensed-history step
+      const int vox = vox_index(g, vi, vj, vk);
+      const float rho = __ldg(g.density + vox); const int mt = __ldg(g.material + vox);
+      const float D = c_mat.sscale[mt] * (1.52f + 0.25f / T + 0.078f * T) * rho;
+      const float sE = D > 0.0f ? kFe * T / D : INFINITY;
+      float sv = INFINITY;
+      if (u > 0.0f) sv = fminf(sv, (g.ox + (float)(vi + 1) * g.dx - x) / u); else if (u < 0.0f) sv = fminf(sv, (g.ox + (float)vi * g.dx - x) / u);
+      if (v > 0.0f) sv = fminf(sv, (g.oy + (float)(vj + 1) * g.dy - y) / v); else if (v < 0.0f) sv = fminf(sv, (g.oy + (float)vj * g.dy - y) / v);
+      if (w > 0.0f) sv = fminf(sv, (g.oz + (float)(vk + 1) * g.dz - z) / w); else if (w < 0.0f) sv = fminf(sv, (g.oz + (float)vk * g.dz - z) / w);
+      sv = fmaxf(sv, 0.0f);
+      const float s = fminf(sE, sv + kEpsB), dT = D * s;
+      ++steps;
+      if (DBG) { ++tl.st[ST_ESTEPS]; ++tl.st[ST_DEPOSITS]; }
+      bool done = false;
+      if (T - dT <= kEcut) {
+        const long long q = quanta(T); pend.add(g, vox, q); tl.dep += (unsigned long long)q;
+        if (DBG) { fnv.u32(steps); fnv.byte('A'); }
+        done = true;
+      } else {
+        const long long q = quanta(dT); pend.add(g, vox, q); tl.dep += (unsigned long long)q;
+        const float Tpre = T;
+        x += s * u; y += s * v; z += s * w; T -= dT;
+        if (!locate(g, x, y, z, vi, vj, vk)) {
+          tl.esc += (unsigned long long)quanta(T);
+          if (DBG) { fnv.u32(steps); fnv.byte('E'); ++tl.st[ST_EESC]; }
+          done = true;
+        } else {
+          const float pbeta = Tpre * (Tpre + 2.0f * kMe) / (Tpre + kMe);
+          const float th0 = 13.6f / pbeta * sqrtf(rho * s * c_mat.inv_x0[mt]);
+          const float a1 = u_oc(rng.next()), b1 = u_co(rng.next());
+          const float th = fminf(kPi, th0 * sqrtf(-2.0f * logf(a1)));
+          float st, ct; sincosf(th, &st, &ct);
+          rotate(u, v, w, ct, st, b1);
+        }
+      }
+      if (done) { if (DBG) finish_track<DBG>(a, h, fnv); active = false; }
+    }
+  }
+  pend.flush(g);
+  tally_flush<DBG>(a, tl);
+}
+
+}  // namespace pslmc

@@ -1,0 +1,174 @@
+"""Whole-path mc_dose parity with the oracle, determinism and edge cases (python -m pytest tests -m gpu)."""
+import numpy as np
+import pytest
+
+from test_gpu_parity import B, gpsl, COUNTERS          # noqa: F401  (fixtures)
+
+pytestmark = pytest.mark.gpu
+
+
+def gpu_dose(B, psl, dph, beam, N, seed, batch, want_fp=True, **opt):
+    import torch
+    hb, he = opt.get("history_begin", 0), opt.get("history_end", 0) or N
+    fp = torch.zeros(he - hb, dtype=torch.int64, device="cuda") if want_fp else None
+    acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
+    dose = torch.empty(dph.nvox, dtype=torch.float64, device="cuda")
+    psl.dose(dph, beam, N, seed, batch=batch, dose_out=dose, dose_acc=acc, fingerprints=fp, **opt)
+    st = B.stats()
+    return acc.cpu().numpy(), dose.cpu().numpy(), st, (fp.cpu().numpy().view(np.uint64) if want_fp else None)
+
+
+def compare_with_oracle(B, orc, g, o, ph_dict, beam, N, seed, batch, min_same=0.999, dose_tol=5e-3, frac_vox=0.995):
+    dph, oph = B.DevicePhantom(ph_dict), orc.Phantom(ph_dict)
+    acc, dose, st, fp = gpu_dose(B, g, dph, beam, N, seed, batch, flags=B.MC_FLAG_STATS)
+    oacc, ores, ofp = o.dose(oph, beam, N, seed, fingerprints=True)
+    ref = orc.finalise(oph, oacc, N)
+    same = float((fp == ofp).mean())
+    assert same >= min_same, same
+    # integer bookkeeping
+    assert st["n_hist"] == ores["n_hist"]
+    assert abs(st["n_jaw_rejected"] - ores["n_jaw_rejected"]) <= max(2, 1e-4 * N)
+    for k in COUNTERS:
+        assert abs(st[k] - ores[k]) <= max(3, 2e-3 * ores[k]), (k, st[k], ores[k])
+    L, OL = st["ledger"], ores["ledger"]
+    assert int(acc.sum()) == L["deposited"]
+    assert abs(L["deposited"] + L["escaped"] + L["jaw"] - L["incident"]) <= 1e-5 * L["incident"]
+    for k in OL:
+        assert abs(L[k] - OL[k]) <= 1e-3 * OL["incident"], k
+    # dose: 0.5 % of local dose in voxels above 10 % of Dmax
+    big = ref > 0.1 * ref.max()
+    err = np.abs(dose[big] - ref[big]) / ref[big]
+    assert np.median(err) < 1e-4
+    assert (err <= dose_tol).mean() >= frac_vox, (float((err <= dose_tol).mean()), float(err.max()))
+    # finalise: dose_out is exactly the scaled accumulator
+    rho = np.asarray(ph_dict["density"], np.float64)
+    V = ph_dict["dx"] * ph_dict["dy"] * ph_dict["dz"]
+    exp = np.where(rho > 0, acc / 2.0 ** 32 / (np.where(rho > 0, rho, 1) * V * N), 0.0)
+    assert np.allclose(dose, exp, rtol=1e-14, atol=0)
+    return same, float(err.max()), float((err <= dose_tol).mean())
+
+
+def test_dose_parity_c0_full(B, orc, gpsl, opsl, cfg):
+    c = cfg("C0")
+    compare_with_oracle(B, orc, gpsl("C0"), opsl("C0"), c["phantom"], c["beams"][0], c["n_histories"], c["seed"], batch=1 << 14)
+
+
+def test_dose_parity_c1(B, orc, gpsl, opsl, cfg):
+    c = cfg("C1")
+    compare_with_oracle(B, orc, gpsl("C1"), opsl("C1"), c["phantom"], c["beams"][0], 2_000_000, c["seed"], batch=1 << 18)
+
+
+def test_dose_parity_c2_heterogeneous(B, orc, gpsl, opsl, cfg):
+    c = cfg("C2")
+    compare_with_oracle(B, orc, gpsl("C2"), opsl("C2"), c["phantom"], c["beams"][0], 1_000_000, c["seed"], batch=300_000)
+
+
+def test_dose_parity_c3_rotated_beam(B, orc, opsl, cfg):
+    c = cfg("C3")
+    g = B.Psl(c["psr"], c["jaws"], c["n_sectors"])
+    compare_with_oracle(B, orc, g, opsl("C3"), c["phantom"], c["beams"][2], 500_000, 42, batch=1 << 17, frac_vox=0.98)
+
+
+def test_dose_parity_c4_large_field(B, orc, gpsl, opsl, cfg):
+    c = cfg("C4")
+    compare_with_oracle(B, orc, gpsl("C4"), opsl("C4"), c["phantom"], c["beams"][0], 1_000_000, c["seed"], batch=1 << 20, frac_vox=0.98)
+
+
+# ---------------------------------------------------------------- determinism contract (bit-exact)
+def test_bitwise_identity_under_batch_order_partition(B, gpsl, cfg):
+    c = cfg("C0")
+    dph = B.DevicePhantom(c["phantom"])
+    g, beam, N, seed = gpsl("C0"), c["beams"][0], 100_000, 1
+    ref_acc, ref_dose, ref_st, ref_fp = gpu_dose(B, g, dph, beam, N, seed, 1 << 16)
+    for batch, opt in ((1000, {}), (33_333, {}), (1 << 20, {}), (1 << 13, dict(order=B.MC_ORDER_MIXED)),
+                       (1 << 15, dict(flags=B.MC_FLAG_STATIC_LANES)), (1 << 15, dict(flags=B.MC_FLAG_STATS | B.MC_FLAG_TIMING))):
+        acc, dose, st, fp = gpu_dose(B, g, dph, beam, N, seed, batch, **opt)
+        assert np.array_equal(acc, ref_acc), (batch, opt)
+        assert np.array_equal(dose, ref_dose) and np.array_equal(fp, ref_fp)
+        assert st["ledger"] == ref_st["ledger"] and st["n_jaw_rejected"] == ref_st["n_jaw_rejected"]
+    # partitions of the history range, accumulated into one int64 grid
+    import torch
+    acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
+    led = {k: 0 for k in ref_st["ledger"]}
+    for a, b in ((60_000, 100_000), (0, 1), (1, 25_000), (25_000, 60_000)):
+        g.dose(dph, beam, N, seed, batch=9000, dose_acc=acc, history_begin=a, history_end=b)
+        for k in led:
+            led[k] += B.stats()["ledger"][k]
+    assert np.array_equal(acc.cpu().numpy(), ref_acc) and led == ref_st["ledger"]
+
+
+def test_mixed_order_is_bitwise_equal_on_c4(B, gpsl, cfg):
+    c = cfg("C4")
+    dph = B.DevicePhantom(c["phantom"])
+    a0, _, s0, _ = gpu_dose(B, gpsl("C4"), dph, c["beams"][0], 3_000_000, 5, 1 << 20, want_fp=False)
+    a1, _, s1, _ = gpu_dose(B, gpsl("C4"), dph, c["beams"][0], 3_000_000, 5, 1 << 18, want_fp=False, order=B.MC_ORDER_MIXED)
+    assert np.array_equal(a0, a1) and s0["ledger"] == s1["ledger"]
+
+
+def test_multi_beam_accumulation_and_conservation_c3(B, cfg):
+    import torch
+    c = cfg("C3")
+    g = B.Psl(c["psr"], c["jaws"], c["n_sectors"])
+    dph = B.DevicePhantom(c["phantom"])
+    acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
+    dep = 0
+    for b, beam in enumerate(c["beams"]):
+        g.dose(dph, beam, 300_000, c["seed"] + b, batch=1 << 17, dose_acc=acc)
+        L = B.stats()["ledger"]
+        assert abs(L["deposited"] + L["escaped"] + L["jaw"] - L["incident"]) <= 1e-5 * L["incident"]
+        dep += L["deposited"]
+        assert int(acc.sum().item()) == dep
+    d = acc.cpu().numpy().reshape(120, 256, 256)
+    assert d[50:70, 118:138, 118:138].mean() > 5 * d[50:70, :20, :20].mean()     # beams cross at the isocentre
+
+
+# ---------------------------------------------------------------- edge cases and errors
+def test_edge_cases(B, gpsl, cfg):
+    import torch
+    c = cfg("C0")
+    dph = B.DevicePhantom(c["phantom"])
+    g, beam = gpsl("C0"), c["beams"][0]
+    d = g.dose(dph, beam, 1, 3, batch=1)                                           # a single history
+    assert d.shape[0] == dph.nvox and torch.isfinite(d).all()
+    acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
+    g.dose(dph, beam, 1000, 3, batch=64, dose_acc=acc, history_begin=500, history_end=500)      # empty range
+    assert int(acc.abs().sum().item()) == 0 and B.stats()["ledger"]["incident"] == 0
+    with pytest.raises(B.PslmcError):
+        g.dose(dph, beam, 1000, 3, batch=0)
+    with pytest.raises(B.PslmcError):
+        g.dose(dph, beam, 1000, 3, batch=64, history_begin=10, history_end=2000)
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.PslmcError) as e:
+        g.dose(dph, beam, 1000, 3, batch=1 << 16, workspace=small)
+    assert e.value.code == -3
+    ws = torch.empty(g.workspace_bytes(dph, 1 << 12), dtype=torch.uint8, device="cuda")
+    a = g.dose(dph, beam, 20_000, 3, batch=1 << 12, workspace=ws).clone()
+    b = g.dose(dph, beam, 20_000, 3, batch=1 << 12)
+    assert torch.equal(a, b)
+    # a side stream
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        c2 = g.dose(dph, beam, 20_000, 3, batch=1 << 12, stream=s)
+    assert torch.equal(a, c2)
+
+
+def test_host_entry_point_matches_device_entry_point(B, gpsl, cfg):
+    c = cfg("C0")
+    dph = B.DevicePhantom(c["phantom"])
+    d_dev = gpsl("C0").dose(dph, c["beams"][0], 50_000, 1, batch=1 << 14).cpu().numpy()
+    d_host = gpsl("C0").dose_host(c["phantom"], c["beams"][0], 50_000, 1, batch=1 << 14)
+    assert np.array_equal(d_dev, d_host)
+
+
+def test_vacuum_and_queue_stats(B, orc, cfg, wl):
+    """A phantom with a vacuum gap (rho = 0): parity still holds; queue high-water marks are reported."""
+    c = cfg("C1", False)
+    n = 32
+    rho = np.ones((n, n, n), np.float32); mat = np.zeros((n, n, n), np.uint8)
+    rho[8:12] = 0.0
+    rho[12:16], mat[12:16] = 1.85, 2
+    ph = dict(nx=n, ny=n, nz=n, dx=0.5, dy=0.5, dz=0.5, ox=-8.0, oy=-8.0, oz=0.0, density=rho.reshape(-1), material=mat.reshape(-1))
+    g, o = B.Psl(c["psr"], c["jaws"], 16), orc.Psl(c["psr"], c["jaws"], 16)
+    compare_with_oracle(B, orc, g, o, ph, c["beams"][0], 300_000, 8, batch=1 << 16, frac_vox=0.98)
+    st = B.stats()
+    assert 0 < st["queue_high_water"][0] < 4 * (1 << 16) and st["launches"]["photon"] > 0

@@ -1,0 +1,180 @@
+"""GPU ↔ oracle parity through the C ABI (python -m pytest tests -m gpu).
+
+Bars (BASELINE.json north_star): sampled buffers within 1e-6 (scale-relative, fp32);
+>= 99.9 % of histories with an identical interaction sequence (fingerprint); same-seed dose within
+0.5 % of local dose in voxels above 10 % of Dmax; integer results (tables, allocation, ledger
+identities, determinism under batch/order/partition) bit-exact.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+SCALE = np.array([16.0, 16.0, 16.0, 1.0, 1.0, 1.0, 6.0])     # G16: positions 16 cm, cosines 1, energy 6 MeV
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1503_01725_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def gpsl(B, cfg):
+    cache = {}
+
+    def get(name):
+        if name not in cache:
+            c = cfg(name, with_phantom=False)
+            cache[name] = B.Psl(c["psr"], c["jaws"], c["n_sectors"])
+        return cache[name]
+    return get
+
+
+def soa_to_rows(t):
+    a = t.cpu().numpy().astype(np.float64)                     # (2, n, 4)
+    return np.concatenate([a[0, :, :3], a[1, :, :3], a[0, :, 3:4], a[1, :, 3:4]], axis=1)   # x y z u v w E status
+
+
+# ---------------------------------------------------------------- integer / table parity
+def test_philox_on_device(B, orc):
+    for seed, h, t, b in ((0, 0, 0, 0), (1, 5, 0, 2), (0x0123456789ABCDEF, 2 ** 40 + 17, 0xDEADBEEF, 123456)):
+        assert B.philox_debug(seed, h, t, b).tolist() == orc.philox(seed, h, t, b).tolist()
+
+
+@pytest.mark.parametrize("name", ["C0", "C1", "C2", "C4"])
+def test_tables_and_allocation_bit_exact(name, B, gpsl, opsl, cfg):
+    ex = gpsl(name).export()
+    o = opsl(name)
+    assert len(ex["groups"]) == o.n_groups
+    assert np.array_equal(ex["rect"], o.rect())
+    for gi, g in enumerate(ex["groups"]):
+        og = o.group(gi)
+        assert (g["stype"], g["ebin"]) == (og["stype"], og["ebin"]) and g["W"] == og["W"]
+        for k in ("ring", "sector", "thresh", "alias"):
+            assert np.array_equal(g[k], og[k]), (name, gi, k)
+    for N in (1, 1000, cfg(name, False)["n_histories"]):
+        assert np.array_equal(gpsl(name).allocate(N), o.allocate(N))
+
+
+# ---------------------------------------------------------------- k_sample
+def check_samples(B, g, o, beam, N, seed, first, count):
+    got = soa_to_rows(g.sample_debug(beam, N, seed, first, count))
+    ref = o.sample(beam, N, seed, first, count)
+    same_status = got[:, 7] == ref[:, 7]
+    assert same_status.mean() >= 1 - 1e-4                      # a jaw decision may flip on an fp32 tie
+    err = np.abs(got[:, :7] - ref[:, :7])
+    tol = 1e-6 * np.maximum(np.maximum(np.abs(got[:, :7]), np.abs(ref[:, :7])), SCALE)
+    assert np.all(err <= tol), float((err / tol).max())
+    return float((err / tol).max())
+
+
+def test_sample_parity_c0_full(B, gpsl, opsl, cfg):
+    c = cfg("C0", False)
+    check_samples(B, gpsl("C0"), opsl("C0"), c["beams"][0], 100_000, 1, 0, 100_000)
+
+
+def test_sample_parity_c1_windows(B, gpsl, opsl, cfg):
+    c = cfg("C1", False)
+    N = c["n_histories"]
+    off = opsl("C1").allocate(N).astype(np.int64)
+    # windows across group boundaries of all three sub-sources, a ragged tail, the last histories
+    for first, count in ((0, 70_001), (int(off[24]) - 3000, 6001), (int(off[48]) - 501, 1003), (N - 4097, 4097),
+                         (int(off[30]), 1)):
+        check_samples(B, gpsl("C1"), opsl("C1"), c["beams"][0], N, c["seed"], first, count)
+
+
+def test_sample_parity_rotated_beam_and_c4(B, gpsl, opsl, cfg, wl):
+    c3 = cfg("C3", False)
+    g, o = B.Psl(c3["psr"], c3["jaws"], 16), opsl("C3")
+    for b in (1, 4):
+        check_samples(B, g, o, c3["beams"][b], 1_000_000, 40 + b, 123_456, 30_000)
+    c4 = cfg("C4", False)
+    N = c4["n_histories"]
+    off = opsl("C4").allocate(N).astype(np.int64)
+    for first in (0, int(off[70]), int(off[100]) - 10_000, N - 50_000):
+        check_samples(B, gpsl("C4"), opsl("C4"), c4["beams"][0], N, 5, first, 50_000)
+
+
+def test_sample_empty_and_invalid(B, gpsl, cfg):
+    c = cfg("C0", False)
+    assert gpsl("C0").sample_debug(c["beams"][0], 100, 1, 0, 0).shape[1] == 0
+    with pytest.raises(B.PslmcError):
+        gpsl("C0").sample_debug(c["beams"][0], 100, 1, 90, 11)
+    with pytest.raises(B.PslmcError):
+        B.Psl(c["psr"], dict(c["jaws"], x1=1.0, x2=-1.0), 8)
+    # a field that no let can see: far off-axis sliver
+    with pytest.raises(B.PslmcError) as e:
+        B.Psl(c["psr"], dict(c["jaws"], x1=60.0, x2=61.0, y1=60.0, y2=61.0), 8)
+    assert e.value.code == -2
+
+
+# ---------------------------------------------------------------- transport only
+def run_transport(B, orc, ph_dict, ptype, rows, first, seed, flags=0):
+    import torch
+    dph, oph = B.DevicePhantom(ph_dict), orc.Phantom(ph_dict)
+    n = rows.shape[0]
+    soa = np.zeros((2, n, 4), np.float32)
+    soa[0, :, :3], soa[0, :, 3] = rows[:, 0:3], rows[:, 6]
+    soa[1, :, :3], soa[1, :, 3] = rows[:, 3:6], rows[:, 7]
+    acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
+    fp = torch.zeros(n, dtype=torch.int64, device="cuda")
+    B.transport_debug(dph, ptype, torch.as_tensor(soa).cuda(), first, seed, acc, fingerprints=fp, flags=flags)
+    st = B.stats()
+    rows64 = soa_to_rows(torch.as_tensor(soa))                 # the oracle sees the same fp32-rounded inputs
+    oacc, ores, ofp = orc.transport(oph, ptype, rows64, first, seed, flags=flags & 1, fingerprints=True)
+    return acc.cpu().numpy(), st, fp.cpu().numpy().view(np.uint64), oacc, ores, ofp
+
+
+COUNTERS = ("n_missed", "n_flights", "n_virtual", "n_compton", "n_photo", "n_pair", "n_photon_cutoff", "n_photon_escape",
+            "n_uncollided_escape", "n_sec_electrons", "n_sec_photons", "n_electron_tracks", "n_electron_steps",
+            "n_electron_escape", "n_deposits")
+
+
+def assert_close_run(acc, st, fp, oacc, ores, ofp, min_same=0.999, rel_counts=2e-3):
+    assert (fp == ofp).mean() >= min_same, float((fp == ofp).mean())
+    for k in COUNTERS:
+        assert abs(st[k] - ores[k]) <= max(3, rel_counts * ores[k]), (k, st[k], ores[k])
+    L, OL = st["ledger"], ores["ledger"]
+    assert int(acc.sum()) == L["deposited"]                                    # integer identity on the GPU side
+    assert abs(L["deposited"] + L["escaped"] + L["jaw"] - L["incident"]) <= 1e-5 * L["incident"]
+    for k in OL:
+        assert abs(L[k] - OL[k]) <= 2e-3 * max(OL["incident"], 1), k
+
+
+def test_transport_photon_pencil_layered(B, orc):
+    from test_oracle_physics import pencil
+    n = 24
+    rho = np.ones((n, n, n), np.float32)
+    mat = np.zeros((n, n, n), np.uint8)
+    rho[6:10], mat[6:10] = 1.85, 2
+    rho[10:16], mat[10:16] = 0.26, 1
+    ph = dict(nx=n, ny=n, nz=n, dx=0.5, dy=0.5, dz=0.5, ox=-6.0, oy=-6.0, oz=0.0, density=rho.reshape(-1), material=mat.reshape(-1))
+    rows = pencil(200_003, 6.0)
+    rows[::7, 7] = -1.0                                                      # skipped entries
+    rows[:, 0] = 0.13
+    rows[:, 1] = -0.21
+    out = run_transport(B, orc, ph, 0, rows, 1000, 77)
+    assert_close_run(*out)
+    assert out[1]["n_pair"] > 100 and out[1]["n_virtual"] > 1000 and out[1]["n_sec_photons"] == 2 * out[1]["n_pair"]
+    out = run_transport(B, orc, ph, 0, rows[:50_000], 0, 78, flags=1)          # electrons deposited locally
+    assert_close_run(*out)
+    assert out[1]["n_electron_steps"] == 0
+
+
+def test_transport_electron_beam(B, orc, wl):
+    rng = np.random.default_rng(4)
+    n = 100_001
+    rows = np.zeros((n, 8))
+    rows[:, 0:2] = rng.uniform(-2, 2, (n, 2))
+    rows[:, 2] = -5.0                                                          # starts outside, enters through k = 0
+    d = rng.normal(0, 0.05, (n, 3)); d[:, 2] = 1.0
+    rows[:, 3:6] = d / np.linalg.norm(d, axis=1)[:, None]
+    rows[:, 6] = rng.uniform(0.1, 6.0, n)
+    rows[:5, 3:6] = (1.0, 0.0, 0.0)                                            # these miss the phantom
+    out = run_transport(B, orc, wl.slab_phantom(48, 0.25), 1, rows, 0, 9)
+    assert_close_run(*out)
+    assert out[1]["n_missed"] == 5 and out[1]["n_electron_tracks"] == n
