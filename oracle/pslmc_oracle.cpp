@@ -303,8 +303,9 @@ double stopping(int m, double T) { return SSCALE[m] * (1.52 + 0.25 / T + 0.078 *
 
 void rotate(double d[3], double ct, double st, double phi) {
   double cp = std::cos(phi), sp = std::sin(phi), nx, ny, nz;
-  if (std::fabs(d[2]) < 0.99999) {
-    double s = std::sqrt(1.0 - d[2] * d[2]);
+  double s2 = d[0] * d[0] + d[1] * d[1];               // = 1 - d_z^2 for a unit vector (P8)
+  if (s2 > 1e-20) {
+    double s = std::sqrt(s2);
     nx = d[0] * ct + st * (d[0] * d[2] * cp - d[1] * sp) / s;
     ny = d[1] * ct + st * (d[1] * d[2] * cp + d[0] * sp) / s;
     nz = d[2] * ct - s * st * cp;

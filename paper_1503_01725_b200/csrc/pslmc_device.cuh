@@ -146,8 +146,9 @@ __device__ __forceinline__ void rotate(float &u, float &v, float &w, float ct, f
   float sp, cp;
   sincospif(2.0f * uphi, &sp, &cp);
   float nx, ny, nz;
-  if (fabsf(w) < 0.99999f) {
-    float s = sqrtf(1.0f - w * w), is = 1.0f / s;
+  const float s2 = u * u + v * v;                         // = 1 - w^2 for a unit vector, without the cancellation
+  if (s2 > 1e-20f) {
+    float s = sqrtf(s2), is = 1.0f / s;
     nx = u * ct + st * (u * w * cp - v * sp) * is;
     ny = v * ct + st * (v * w * cp + u * sp) * is;
     nz = w * ct - s * st * cp;
