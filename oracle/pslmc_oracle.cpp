@@ -444,30 +444,38 @@ struct Ctx {
     int ijk[3]; uint32_t steps = 0;
     if (!locate(t.pos, ijk) && !enter(t, ijk)) { escape(t.E); f.u32(0); f.byte('M'); ev(t, 'M'); ++res->n_missed; fp += f.v; return; }
     const double lo[3] = {ph.ox, ph.oy, ph.oz}, dd[3] = {ph.dx, ph.dy, ph.dz};
+    // One condensed-history step loses the fraction fE of the energy it starts with (budget); it is cut
+    // into sub-steps at voxel faces.  The Gaussian deflection is applied once per condensed step, over
+    // the rho*s/X0 accumulated along it (P7).
+    double budget = 0, tacc = 0, Tms = t.E; bool fresh = true;
     for (;;) {
+      if (fresh) { budget = fE * t.E; Tms = t.E; tacc = 0; fresh = false; }
       size_t v = vox(ijk); double rho = ph.density[v]; int m = ph.material[v];
       double D = stopping(m, t.E) * rho;
-      double sE = D > 0 ? fE * t.E / D : std::numeric_limits<double>::infinity();
+      double sE = D > 0 ? budget / D : std::numeric_limits<double>::infinity();
       double sv = std::numeric_limits<double>::infinity();
       for (int a = 0; a < 3; ++a) {
         if (t.dir[a] > 0) sv = std::fmin(sv, (lo[a] + (ijk[a] + 1) * dd[a] - t.pos[a]) / t.dir[a]);
         else if (t.dir[a] < 0) sv = std::fmin(sv, (lo[a] + ijk[a] * dd[a] - t.pos[a]) / t.dir[a]);
       }
       if (sv < 0) sv = 0;
-      double s = std::fmin(sE, sv + EPS_B), dT = D * s;
+      bool turn = sE <= sv + EPS_B;                       // the sub-step ends the condensed step
+      double s = turn ? sE : sv + EPS_B, dT = turn ? budget : D * s;
       ++steps; ++res->n_electron_steps;
       if (t.E - dT <= ECUT) { deposit(v, t.E); ev(t, 'A', s); f.u32(steps); f.byte('A'); break; }
       deposit(v, dT);
-      double Tpre = t.E;
       for (int a = 0; a < 3; ++a) t.pos[a] += s * t.dir[a];
-      t.E -= dT;
+      t.E -= dT; budget -= dT; tacc += rho * s / X0[m];
       if (!locate(t.pos, ijk)) { escape(t.E); ev(t, 'E', s); ++res->n_electron_escape; f.u32(steps); f.byte('E'); break; }
-      double pbeta = Tpre * (Tpre + 2.0 * ME) / (Tpre + ME);
-      double th0 = 13.6 / pbeta * std::sqrt(rho * s / X0[m]);
-      double a1 = U_oc(st.next()), b1 = U_co(st.next());
-      double th = std::fmin(PI, th0 * std::sqrt(-2.0 * std::log(a1)));
-      rotate(t.dir, std::cos(th), std::sin(th), 2.0 * PI * b1);
-      ev(t, 'S', s);
+      if (turn) {
+        double pbeta = Tms * (Tms + 2.0 * ME) / (Tms + ME);
+        double th0 = 13.6 / pbeta * std::sqrt(tacc);
+        double a1 = U_oc(st.next()), b1 = U_co(st.next());
+        double th = std::fmin(PI, th0 * std::sqrt(-2.0 * std::log(a1)));
+        rotate(t.dir, std::cos(th), std::sin(th), 2.0 * PI * b1);
+        fresh = true;
+        ev(t, 'T', s);
+      } else ev(t, 'S', s);
     }
     fp += f.v;
   }

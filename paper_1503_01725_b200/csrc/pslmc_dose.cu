@@ -388,9 +388,10 @@ extern "C" int mc_stats(mc_stats_t *out) {
 // ---------------------------------------------------------------- parity / debug exports
 extern "C" int mc_sample_debug(const psl_t *P, const beam_geom_t *beam, uint64_t first_history, uint64_t count,
                                uint64_t n_histories, uint64_t seed, float *soa_out, void *cuda_stream) {
-  if (!P || !beam || !soa_out || n_histories == 0 || first_history + count > n_histories || count > 0x7fffffffull)
+  if (!P || !beam || n_histories == 0 || first_history + count > n_histories || count > 0x7fffffffull)
     return fail(MC_E_INVALID_ARG, "mc_sample_debug: invalid argument");
   if (count == 0) return MC_OK;
+  if (!soa_out) return fail(MC_E_INVALID_ARG, "mc_sample_debug: soa_out is null");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   std::vector<uint64_t> off(P->groups.size() + 1);
   allocate_host(*P, n_histories, off.data());

@@ -255,6 +255,10 @@ __global__ void __launch_bounds__(kThreads) k_photon(const __grid_constant__ Tra
 }
 
 // ------------------------------------------------------------------ k_electron
+// Electrons carry (voxel index, offset inside the voxel) instead of global coordinates: fp32 then
+// resolves positions to ~3e-8 cm relative to the voxel faces that decide every step, instead of the
+// ~1e-6 cm of a global coordinate.  In exact arithmetic this is the
+// same walk as floor((pos - o)/d) on global coordinates.
 template <bool DBG>
 __global__ void __launch_bounds__(kThreads) k_electron(const __grid_constant__ TransportArgs a) {
   const Grid &g = a.g;
@@ -263,9 +267,11 @@ __global__ void __launch_bounds__(kThreads) k_electron(const __grid_constant__ T
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
   Pending pend; pend.v = 0; pend.q = 0;
   bool active = false, exhausted = false;
-  float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, T = 0;
+  float lx = 0, ly = 0, lz = 0, u = 0, v = 0, w = 1, T = 0;      // offset inside voxel (vi,vj,vk), direction, energy
   int vi = 0, vj = 0, vk = 0;
   unsigned long long h = 0; uint32_t steps = 0;
+  // condensed step (P7): energy still to lose in it, rho*s/X0 accumulated, energy at its start
+  float budget = 0, tacc = 0, Tms = 0; bool fresh = true;
   Philox rng; rng.n = 0; rng.track = 0; rng.k0 = rng.k1 = rng.hlo = rng.hhi = 0; rng.w0 = rng.w1 = rng.w2 = rng.w3 = 0;
   Fnv fnv; fnv.v = 0;
 
@@ -274,7 +280,8 @@ __global__ void __launch_bounds__(kThreads) k_electron(const __grid_constant__ T
     if (idx != 0xffffffffu) {
       const TrackIn t = load_track(a, idx);
       if (t.ok) {
-        x = t.x; y = t.y; z = t.z; u = t.u; v = t.v; w = t.w; T = t.E; h = t.h; steps = 0;
+        float x = t.x, y = t.y, z = t.z;
+        u = t.u; v = t.v; w = t.w; T = t.E; h = t.h; steps = 0; fresh = true;
         rng.init(a.seed, h, t.track, t.ndraw);
         if (DBG) { fnv.init(t.track); ++tl.st[ST_ETRACKS]; }
         if (a.src_kind == SRC_BUFFER && a.buffer_is_debug) tl.inc += (unsigned long long)quanta(T);
@@ -283,6 +290,8 @@ __global__ void __launch_bounds__(kThreads) k_electron(const __grid_constant__ T
           tl.esc += (unsigned long long)quanta(T);
           if (DBG) { fnv.u32(0u); fnv.byte('M'); ++tl.st[ST_MISSED]; finish_track<DBG>(a, h, fnv); }
           active = false;
+        } else {
+          lx = (x - g.ox) - (float)vi * g.dx; ly = (y - g.oy) - (float)vj * g.dy; lz = (z - g.oz) - (float)vk * g.dz;
         }
       }
     }
@@ -291,14 +300,16 @@ __global__ void __launch_bounds__(kThreads) k_electron(const __grid_constant__ T
     if (active) {                                        // one condensed-history step
       const int vox = vox_index(g, vi, vj, vk);
       const float rho = __ldg(g.density + vox); const int mt = __ldg(g.material + vox);
+      if (fresh) { budget = kFe * T; Tms = T; tacc = 0.0f; fresh = false; }
       const float D = c_mat.sscale[mt] * (1.52f + 0.25f / T + 0.078f * T) * rho;
-      const float sE = D > 0.0f ? kFe * T / D : INFINITY;
+      const float sE = D > 0.0f ? budget / D : INFINITY;
       float sv = INFINITY;
-      if (u > 0.0f) sv = fminf(sv, (g.ox + (float)(vi + 1) * g.dx - x) / u); else if (u < 0.0f) sv = fminf(sv, (g.ox + (float)vi * g.dx - x) / u);
-      if (v > 0.0f) sv = fminf(sv, (g.oy + (float)(vj + 1) * g.dy - y) / v); else if (v < 0.0f) sv = fminf(sv, (g.oy + (float)vj * g.dy - y) / v);
-      if (w > 0.0f) sv = fminf(sv, (g.oz + (float)(vk + 1) * g.dz - z) / w); else if (w < 0.0f) sv = fminf(sv, (g.oz + (float)vk * g.dz - z) / w);
+      if (u > 0.0f) sv = fminf(sv, (g.dx - lx) / u); else if (u < 0.0f) sv = fminf(sv, -lx / u);
+      if (v > 0.0f) sv = fminf(sv, (g.dy - ly) / v); else if (v < 0.0f) sv = fminf(sv, -ly / v);
+      if (w > 0.0f) sv = fminf(sv, (g.dz - lz) / w); else if (w < 0.0f) sv = fminf(sv, -lz / w);
       sv = fmaxf(sv, 0.0f);
-      const float s = fminf(sE, sv + kEpsB), dT = D * s;
+      const bool turn = sE <= sv + kEpsB;              // this sub-step ends the condensed step
+      const float s = turn ? sE : sv + kEpsB, dT = turn ? budget : D * s;
       ++steps;
       if (DBG) { ++tl.st[ST_ESTEPS]; ++tl.st[ST_DEPOSITS]; }
       bool done = false;
@@ -308,19 +319,23 @@ __global__ void __launch_bounds__(kThreads) k_electron(const __grid_constant__ T
         done = true;
       } else {
         const long long q = quanta(dT); pend.add(g, vox, q); tl.dep += (unsigned long long)q;
-        const float Tpre = T;
-        x += s * u; y += s * v; z += s * w; T -= dT;
-        if (!locate(g, x, y, z, vi, vj, vk)) {
+        lx += s * u; ly += s * v; lz += s * w; T -= dT; budget -= dT; tacc += rho * s * c_mat.inv_x0[mt];
+        // re-home: a step ends at most eps beyond the face it was limited by
+        if (lx >= g.dx) { lx -= g.dx; ++vi; } else if (lx < 0.0f) { lx += g.dx; --vi; }
+        if (ly >= g.dy) { ly -= g.dy; ++vj; } else if (ly < 0.0f) { ly += g.dy; --vj; }
+        if (lz >= g.dz) { lz -= g.dz; ++vk; } else if (lz < 0.0f) { lz += g.dz; --vk; }
+        if ((unsigned)vi >= (unsigned)g.nx || (unsigned)vj >= (unsigned)g.ny || (unsigned)vk >= (unsigned)g.nz) {
           tl.esc += (unsigned long long)quanta(T);
           if (DBG) { fnv.u32(steps); fnv.byte('E'); ++tl.st[ST_EESC]; }
           done = true;
-        } else {
-          const float pbeta = Tpre * (Tpre + 2.0f * kMe) / (Tpre + kMe);
-          const float th0 = 13.6f / pbeta * sqrtf(rho * s * c_mat.inv_x0[mt]);
+        } else if (turn) {
+          const float pbeta = Tms * (Tms + 2.0f * kMe) / (Tms + kMe);
+          const float th0 = 13.6f / pbeta * sqrtf(tacc);
           const float a1 = u_oc(rng.next()), b1 = u_co(rng.next());
           const float th = fminf(kPi, th0 * sqrtf(-2.0f * logf(a1)));
           float st, ct; sincosf(th, &st, &ct);
           rotate(u, v, w, ct, st, b1);
+          fresh = true;
         }
       }
       if (done) { if (DBG) finish_track<DBG>(a, h, fnv); active = false; }

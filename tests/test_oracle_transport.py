@@ -98,8 +98,8 @@ def csda_range(T0, m=0, rho=1.0, Tend=0.2):
 
 def electron_path(orc, ph, T0, h, fE):
     ev = orc.trace(ph, 1, [0, 0, 0, 0, 0, 1, T0, 0], h, 5, f_e=fE, max_events=100000)
-    steps = [e for e in ev if e["code"] in "SAE"]
-    return sum(e["aux"] for e in steps if e["code"] == "S"), steps[-1]["aux"], len(steps), ev
+    steps = [e for e in ev if e["code"] in "STAE"]
+    return sum(e["aux"] for e in steps if e["code"] in "ST"), steps[-1]["aux"], len(steps), ev
 
 
 def test_csda_path_length_converges_to_closed_form(orc):
@@ -118,23 +118,56 @@ def test_csda_path_length_converges_to_closed_form(orc):
 
 
 def test_energy_loss_and_voxel_limited_steps(orc):
-    """In a 0.25 cm grid the step is min(f_E T / D, s_voxel + eps): energy lost = D * s exactly."""
+    """DESIGN.md P7: a condensed step loses 12 % of its starting energy and is cut into sub-steps at voxel
+    faces ('S', nudged 1e-4 cm past the face); the deflection happens at its end ('T')."""
     n = 24
     d = 0.25
     ph = orc.Phantom(dict(nx=n, ny=n, nz=n, dx=d, dy=d, dz=d, ox=-3.0, oy=-3.0, oz=0.0,
                           density=np.full(n ** 3, 1.0, np.float32), material=np.zeros(n ** 3, np.uint8)))
     ev = orc.trace(ph, 1, [0.1, 0.1, 0.05, 0, 0, 1, 6.0, 0], 3, 8)
-    st = [e for e in ev if e["code"] == "S"]
-    # first step: straight along z from z=0.05 to the face at 0.25 plus eps (s_E = 0.355 > 0.2)
-    assert st[0]["aux"] == pytest.approx(0.2 + 1e-4, abs=1e-12)
+    st = [e for e in ev if e["code"] in "ST"]
+    # first sub-step: straight along z from z=0.05 to the face at 0.25 plus eps (s_E = 0.355 > 0.2)
+    assert st[0]["code"] == "S" and st[0]["aux"] == pytest.approx(0.2 + 1e-4, abs=1e-12)
     D = 1.52 + 0.25 / 6.0 + 0.078 * 6.0
     assert st[0]["E"] == pytest.approx(6.0 - D * st[0]["aux"], abs=1e-12)
     assert st[0]["pos"][2] == pytest.approx(0.25 + 1e-4, abs=1e-12)
+    assert st[0]["dir"] == pytest.approx([0, 0, 1], abs=0)                       # no deflection inside a condensed step
+    # second sub-step finishes the 12 % budget with the stopping power at the current energy
+    D1 = 1.52 + 0.25 / st[0]["E"] + 0.078 * st[0]["E"]
+    assert st[1]["code"] == "T" and st[1]["E"] == pytest.approx(6.0 * 0.88, abs=1e-12)
+    assert st[1]["aux"] == pytest.approx((0.72 - D * st[0]["aux"]) / D1, abs=1e-12)
+    assert abs(st[1]["dir"][2]) < 1.0
+    turns = [e["E"] for e in st if e["code"] == "T"]
+    assert len(turns) > 10
+    assert np.array(turns[1:]) / np.array(turns[:-1]) == pytest.approx(0.88, abs=1e-12)
     for a, b in zip(st[:-1], st[1:]):
         Dk = 1.52 + 0.25 / a["E"] + 0.078 * a["E"]
         assert a["E"] - b["E"] == pytest.approx(Dk * b["aux"], abs=1e-12)
-        assert b["aux"] <= 0.12 * a["E"] / Dk + 1e-12
         assert np.linalg.norm(b["pos"] - a["pos"]) == pytest.approx(b["aux"], abs=1e-12)
+        assert b["pos"] - a["pos"] == pytest.approx(b["aux"] * a["dir"], abs=1e-12)      # moves along the pre-step direction
+        if b["code"] == "S":
+            assert np.array_equal(a["dir"], b["dir"])                                  # sub-steps inside a condensed step do not deflect
+
+
+def test_multiple_scattering_accumulates_over_the_condensed_step(orc):
+    """theta0 uses rho*s/X0 summed over the sub-steps of the condensed step, in every material crossed."""
+    from test_oracle_physics import slab
+    ph = slab(orc, [(0.25, 1.0, 0), (0.25, 0.26, 1), (3.0, 1.85, 2)])
+    T0 = 6.0
+    ths = []
+    for h in range(4000):
+        ev = orc.trace(ph, 1, [0, 0, 0.1, 0, 0, 1, T0, 0], h, 3, max_events=8)
+        subs = []
+        for e in ev:
+            subs.append(e)
+            if e["code"] == "T":
+                break
+        assert [e["code"] for e in subs] == ["S", "S", "T"]
+        t = subs[0]["aux"] * 1.0 / 36.08 + subs[1]["aux"] * 0.26 / 36.08 + subs[2]["aux"] * 1.85 / 27.2
+        d = subs[-1]["dir"]
+        ths.append(math.atan2(math.hypot(d[0], d[1]), d[2]) ** 2 / t)
+    pbeta = T0 * (T0 + 2 * ME) / (T0 + ME)
+    assert np.mean(ths) == pytest.approx(2 * (13.6 / pbeta) ** 2, rel=5 / math.sqrt(4000))
 
 
 def test_multiple_scattering_moments(orc):
@@ -149,7 +182,7 @@ def test_multiple_scattering_moments(orc):
     th, phi = np.empty(n), np.empty(n)
     for h in range(n):
         ev = orc.trace(ph, 1, [0, 0, 0, 0, 0, 1, T0, 0], h, 12, max_events=2)
-        assert ev[0]["code"] == "S" and ev[0]["aux"] == pytest.approx(s)
+        assert ev[0]["code"] == "T" and ev[0]["aux"] == pytest.approx(s)
         d = ev[0]["dir"]
         th[h] = math.atan2(math.hypot(d[0], d[1]), d[2])
         phi[h] = math.atan2(d[1], d[0]) % (2 * math.pi)
