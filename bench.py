@@ -36,7 +36,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C1")
-    ap.add_argument("--batch", type=int, default=1 << 20)
+    ap.add_argument("--batch", type=int, default=1 << 22)
     ap.add_argument("--histories", type=int, default=0, help="override histories per GPU (default: the config's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--order", default="sorted", choices=["sorted", "mixed"])

@@ -63,6 +63,47 @@ struct Philox {
     return i == 0 ? w0 : (i == 1 ? w1 : (i == 2 ? w2 : w3));
   }
 };
+// The same stream, consumed through ONE generation site per event: window<K>() returns draws
+// n..n+3 of the track's stream without consuming them (the caller may consume up to K <= 4 of
+// them), generating at most one Philox block; consume(k, ...) advances.  c0..c3 cache the block that
+// holds draw n whenever n & 3 != 0.  Draw numbering is exactly DESIGN.md R1 (draw n = word n & 3 of
+// block n >> 2): only where the blocks are generated differs from Philox::next().
+struct RngWin {
+  uint32_t track, hlo, hhi, n;
+  uint32_t c0, c1, c2, c3;
+  __device__ __forceinline__ void init(uint64_t h, uint32_t trk, uint32_t ndraw) {
+    hlo = (uint32_t)h; hhi = (uint32_t)(h >> 32); track = trk; n = ndraw; c0 = c1 = c2 = c3 = 0u;   // ndraw & 3 == 0
+  }
+  __device__ __forceinline__ void gen(uint32_t k0, uint32_t k1, uint32_t j, uint32_t &g0, uint32_t &g1, uint32_t &g2, uint32_t &g3) const {
+    uint32_t x0 = j, x1 = track, x2 = hlo, x3 = hhi, a = k0, b = k1;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+      const uint32_t h0 = __umulhi(0xD2511F53u, x0), l0 = 0xD2511F53u * x0;
+      const uint32_t h1 = __umulhi(0xCD9E8D57u, x2), l1 = 0xCD9E8D57u * x2;
+      x0 = h1 ^ x1 ^ a; x1 = l1; x2 = h0 ^ x3 ^ b; x3 = l0;
+      a += 0x9E3779B9u; b += 0xBB67AE85u;
+    }
+    g0 = x0; g1 = x1; g2 = x2; g3 = x3;
+  }
+  template <int K>
+  __device__ __forceinline__ void window(uint32_t k0, uint32_t k1, uint32_t &d0, uint32_t &d1, uint32_t &d2, uint32_t &d3,
+                                         uint32_t &g0, uint32_t &g1, uint32_t &g2, uint32_t &g3) {
+    const uint32_t s = n & 3u;
+    g0 = g1 = g2 = g3 = 0u;
+    if (s == 0u || s + K > 4u) gen(k0, k1, (n + 3u) >> 2, g0, g1, g2, g3);
+    if (s == 0u) { c0 = g0; c1 = g1; c2 = g2; c3 = g3; }
+    d0 = s == 0u ? c0 : (s == 1u ? c1 : (s == 2u ? c2 : c3));
+    d1 = s == 0u ? c1 : (s == 1u ? c2 : (s == 2u ? c3 : g0));
+    d2 = s == 0u ? c2 : (s == 1u ? c3 : (s == 2u ? g0 : g1));
+    d3 = s == 0u ? c3 : (s == 1u ? g0 : (s == 2u ? g1 : g2));
+  }
+  __device__ __forceinline__ void consume(uint32_t k, uint32_t g0, uint32_t g1, uint32_t g2, uint32_t g3) {
+    const uint32_t m = n + k;
+    if ((m >> 2) != (n >> 2)) { c0 = g0; c1 = g1; c2 = g2; c3 = g3; }
+    n = m;
+  }
+};
+
 __device__ __forceinline__ float u_co(uint32_t x) { return (float)(x >> 8) * (1.0f / 16777216.0f); }          // [0,1)
 __device__ __forceinline__ float u_oc(uint32_t x) { return (float)((x >> 8) + 1u) * (1.0f / 16777216.0f); }   // (0,1]
 
@@ -140,6 +181,21 @@ struct PhotonXs {
     mu_max = m;
   }
 };
+
+// Photon cross-section table (built per mc_dose call on the device, in double, by k_build_xs): node i
+// holds (sigma_KN, ln^2(E/1.022), mu_max, 0) at log2(E) = x0 + i*h; k_photon keeps it in shared memory
+// and interpolates linearly in log2(E) (relative error ~1e-7 at n = 4096: DESIGN.md §6).
+struct XsTable { const float4 *nodes; float x0, inv_h; int n; };      // n intervals, n + 1 nodes
+
+__device__ __forceinline__ void xs_lookup(const float4 *tab, float x0, float inv_h, int n, float E,
+                                          float &skn, float &lp2, float &mu_max) {
+  float t = (__log2f(E) - x0) * inv_h;
+  t = fminf(fmaxf(t, 0.0f), (float)n);
+  int i = min((int)t, n - 1);
+  const float f = t - (float)i;
+  const float4 A = tab[i], B = tab[i + 1];
+  skn = __fmaf_rn(f, B.x - A.x, A.x); lp2 = __fmaf_rn(f, B.y - A.y, A.y); mu_max = __fmaf_rn(f, B.z - A.z, A.z);
+}
 
 // Rotate unit vector d by polar angle (ct, st) and azimuth phi = 2*pi*uphi.
 __device__ __forceinline__ void rotate(float &u, float &v, float &w, float ct, float st, float uphi) {

@@ -5,6 +5,7 @@
 #include "pslmc_transport.cuh"
 
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 
@@ -44,14 +45,14 @@ static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 // (2 planes), the electron queue (capacity 4B) and the photon queue (capacity B), each 3 planes,
 // then (optionally) the int64 dose grid.
 struct Layout {
-  size_t ctl, off, p0, p1, eq[3], pq[3], acc, total;
+  size_t ctl, off, xs, p0, p1, eq[3], pq[3], acc, total;
   unsigned eq_cap, pq_cap;
 };
 static Layout make_layout(uint64_t batch, size_t nvox, bool with_acc) {
   Layout L; size_t o = 0;
   auto take = [&](size_t b) { size_t at = o; o += align_up(b); return at; };
   L.eq_cap = (unsigned)std::min<uint64_t>(4 * batch, 0x7fffffffu); L.pq_cap = (unsigned)batch;
-  L.ctl = take(sizeof(Control)); L.off = take(sizeof(uint64_t) * 160);
+  L.ctl = take(sizeof(Control)); L.off = take(sizeof(uint64_t) * 160); L.xs = take(sizeof(float4) * (kXsIntervals + 1));
   L.p0 = take(16 * batch); L.p1 = take(16 * batch);
   for (int k = 0; k < 3; ++k) L.eq[k] = take((size_t)16 * L.eq_cap);
   for (int k = 0; k < 3; ++k) L.pq[k] = take((size_t)16 * L.pq_cap);
@@ -126,11 +127,11 @@ static bool phantom_ok(const phantom_t *ph) {
 
 // Persistent-grid size: every SM filled to the kernel's occupancy.
 template <typename K>
-static int persistent_blocks(K kernel) {
+static int persistent_blocks(K kernel, size_t smem = 0) {
   int dev = 0, sms = 0, per = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kernel, kThreads, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kernel, kThreads, smem);
   return std::max(1, sms * std::max(1, per));
 }
 
@@ -169,11 +170,21 @@ struct Run {
     a.fp = fp; a.fp_base = fp_base;
     a.electrons_local = (flags & MC_FLAG_ELECTRONS_LOCAL) ? 1 : 0;
     a.static_lanes = (flags & MC_FLAG_STATIC_LANES) ? 1 : 0;
+    a.xs = xs;
     return a;
+  }
+  XsTable xs{};
+  static constexpr size_t kXsSmem = sizeof(float4) * (kXsIntervals + 1);
+  // Builds the cross-section table of this call (after k_rhomax) for photon energies up to e_max.
+  void build_xs(double e_max) {
+    const double x0 = std::log2(0.045), x1 = std::log2(e_max * 1.001), hh = (x1 - x0) / kXsIntervals;
+    float4 *nodes = (float4 *)(ws + L.xs);
+    k_build_xs<<<(kXsIntervals + 256) / 256, 256, 0, st>>>(ctl, nodes, x0, hh, kXsIntervals);
+    xs.nodes = nodes; xs.x0 = (float)x0; xs.inv_h = (float)(1.0 / hh); xs.n = kXsIntervals;
   }
   void photon(const TransportArgs &a) {
     tm.begin(MC_K_PHOTON);
-    if (dbg) k_photon<true><<<blocks_photon[1], kThreads, 0, st>>>(a); else k_photon<false><<<blocks_photon[0], kThreads, 0, st>>>(a);
+    if (dbg) k_photon<true><<<blocks_photon[1], kThreads, kXsSmem, st>>>(a); else k_photon<false><<<blocks_photon[0], kThreads, kXsSmem, st>>>(a);
     tm.end(MC_K_PHOTON); ++launches[MC_K_PHOTON];
   }
   void electron(const TransportArgs &a) {
@@ -182,7 +193,9 @@ struct Run {
     tm.end(MC_K_ELECTRON); ++launches[MC_K_ELECTRON];
   }
   void init_blocks() {
-    blocks_photon[0] = persistent_blocks(k_photon<false>); blocks_photon[1] = persistent_blocks(k_photon<true>);
+    cudaFuncSetAttribute(k_photon<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXsSmem);
+    cudaFuncSetAttribute(k_photon<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXsSmem);
+    blocks_photon[0] = persistent_blocks(k_photon<false>, kXsSmem); blocks_photon[1] = persistent_blocks(k_photon<true>, kXsSmem);
     blocks_electron[0] = persistent_blocks(k_electron<false>); blocks_electron[1] = persistent_blocks(k_electron<true>);
   }
   // photons of the particle buffer, then annihilation photons, then every queued electron
@@ -284,6 +297,7 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
   if (!opts->dose_acc) CUDA_TRY(cudaMemsetAsync(acc, 0, 8 * nvox, r.st));
   r.tm.begin(MC_K_AUX);
   k_rhomax<<<296, 256, 0, r.st>>>(ph->density, ph->material, nvox, r.ctl);
+  r.build_xs(P->psr.e_min + P->psr.e_bin_width * P->n_ebin); ++r.launches[MC_K_AUX];
   r.tm.end(MC_K_AUX); ++r.launches[MC_K_AUX];
 
   SampleArgs sa{};
@@ -431,6 +445,7 @@ extern "C" int mc_transport_debug(const phantom_t *ph, int32_t particle_type, co
   CUDA_TRY(cudaEventRecord(ev0, r.st));
   CUDA_TRY(cudaMemsetAsync(r.ctl, 0, sizeof(Control), r.st));
   k_rhomax<<<296, 256, 0, r.st>>>(ph->density, ph->material, nvox, r.ctl);
+  r.build_xs(64.0);                              // debug entry: energies up to 64 MeV
   // the caller's planes stand in for the particle buffer; n_pb = count
   const unsigned cnt = (unsigned)count;
   CUDA_TRY(cudaMemcpyAsync(&r.ctl->n_pb, &cnt, sizeof cnt, cudaMemcpyHostToDevice, r.st));

@@ -191,6 +191,21 @@ __global__ void k_rhomax(const float *density, const uint8_t *material, size_t n
   }
 }
 
+// Photon cross-section table for this call (needs rhomax): node i at log2(E) = x0 + i*h, in double.
+constexpr int kXsIntervals = 4096;
+__global__ void k_build_xs(const Control *c, float4 *nodes, double x0, double h, int n) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i > n) return;
+  const double E = exp2(x0 + h * (double)i);
+  const double al = E / kMeD, L = log1p(2.0 * al), t = 1.0 + 2.0 * al;
+  const double skn = kTwoPiRe2 * ((1.0 + al) / (al * al) * (2.0 * (1.0 + al) / t - L / al) + L / (2.0 * al) - (1.0 + 3.0 * al) / (t * t));
+  const double l = E > 1.022 ? log(E / 1.022) : 0.0, lp2 = l * l, ie3 = 1.0 / (E * E * E);
+  double m = 0.0;
+  for (int k = 0; k < 3; ++k)
+    m = fmax(m, (double)c->rhomax[k] * ((double)c_mat.ne[k] * skn + (double)c_mat.cphoto[k] * ie3 + (double)c_mat.ppair[k] * lp2));
+  nodes[i] = make_float4((float)skn, (float)lp2, (float)m, 0.0f);
+}
+
 // dose[v] = acc[v] 2^-32 / (rho_v V N)
 __global__ void k_finalise(const long long *acc, const float *density, size_t n, double inv_vn, double *dose) {
   for (size_t v = blockIdx.x * (size_t)blockDim.x + threadIdx.x; v < n; v += (size_t)gridDim.x * blockDim.x) {

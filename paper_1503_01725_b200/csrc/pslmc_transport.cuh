@@ -36,6 +36,7 @@ struct TransportArgs {
   unsigned long long *fp; unsigned long long fp_base;
   int electrons_local, static_lanes;
   int want_type;                      // SRC_BUFFER, compact: take only entries of this particle type (bit 31 of p1.w)
+  XsTable xs;                         // k_photon: cross-section table (global; copied to shared memory per CTA)
 };
 
 struct Tally {                         // per-thread running sums, flushed once at kernel exit
@@ -131,117 +132,158 @@ __device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned i
   return t;
 }
 
+
 // ------------------------------------------------------------------ k_photon
+// One lane = one photon track at a time, as a small state machine.  Every loop iteration runs at most
+// two "events" per lane, each with ONE Philox generation site shared by all lanes of the warp:
+//   event 1 (state FLIGHT): cut-off test, Woodcock flight (draws a, b), voxel fetch, interaction choice;
+//   event 2 (state KAHN / PAIR): one Kahn trial (3 draws, + the azimuth draw when it is accepted, then the
+//            Compton kinematics) or the pair-production split (3 draws).
+// A lane whose Kahn trial is rejected retries in the next iteration while its neighbours fly, instead
+// of holding the warp in a rejection loop.  Cross-sections come from the shared-memory table.
+enum { PH_IDLE = 0, PH_FLIGHT = 1, PH_KAHN = 2, PH_PAIR = 3 };
+
 template <bool DBG>
-__global__ void __launch_bounds__(kThreads) k_photon(const __grid_constant__ TransportArgs a) {
+__global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ TransportArgs a) {
+  extern __shared__ float4 s_xs[];
+  for (int i = threadIdx.x; i <= a.xs.n; i += kThreads) s_xs[i] = a.xs.nodes[i];
+  __syncthreads();
   const Grid &g = a.g;
-  const float rhomax[3] = {a.ctl->rhomax[0], a.ctl->rhomax[1], a.ctl->rhomax[2]};
+  const uint32_t k0 = (uint32_t)a.seed, k1 = (uint32_t)(a.seed >> 32);
   const unsigned count = *a.src_count;
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
   Pending pend; pend.v = 0; pend.q = 0;
-  bool active = false, exhausted = false, collided = false;
+  int state = PH_IDLE; bool exhausted = false, collided = false;
   float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, E = 0;
-  int vi = 0, vj = 0, vk = 0;
+  int cvox = 0;                                          // voxel of the current position
   unsigned long long h = 0; uint32_t nchild = 0;
-  Philox rng; rng.n = 0; rng.track = 0; rng.k0 = rng.k1 = rng.hlo = rng.hhi = 0; rng.w0 = rng.w1 = rng.w2 = rng.w3 = 0;
-  PhotonXs xs; xs.skn = xs.inv_e3 = xs.lp2 = xs.mu_max = 0;
+  RngWin rng; rng.init(0ull, 0u, 0u);
   Fnv fnv; fnv.v = 0;
 
   for (;;) {
     // ---- refill idle lanes
-    const unsigned idx = refill_index(a, !active, count, exhausted);
+    const unsigned idx = refill_index(a, state == PH_IDLE, count, exhausted);
     if (idx != 0xffffffffu) {
       const TrackIn t = load_track(a, idx);
       if (t.ok) {
         x = t.x; y = t.y; z = t.z; u = t.u; v = t.v; w = t.w; E = t.E; h = t.h; nchild = 0; collided = false;
-        rng.init(a.seed, h, t.track, t.ndraw);
+        rng.init(h, t.track, t.ndraw);
         if (DBG) fnv.init(t.track);
         if (a.src_kind == SRC_BUFFER && a.buffer_is_debug) tl.inc += (unsigned long long)quanta(E);
-        active = true;
+        int vi, vj, vk;
         if (!locate(g, x, y, z, vi, vj, vk) && !enter(g, x, y, z, u, v, w, vi, vj, vk)) {
           tl.esc += (unsigned long long)quanta(E);
           if (DBG) { fnv.byte('M'); ++tl.st[ST_MISSED]; finish_track<DBG>(a, h, fnv); }
-          active = false;
-        } else xs.set(E, rhomax);
+        } else { cvox = vox_index(g, vi, vj, vk); state = PH_FLIGHT; }
       }
     }
-    if (!__any_sync(kFull, active)) { if (exhausted) break; else continue; }
+    if (!__any_sync(kFull, state != PH_IDLE)) { if (exhausted) break; else continue; }
 
-    // ---- one Woodcock flight (+ interaction) per active lane
-    bool push_e = false; float ex = 0, ey = 0, ez = 0, eT = 0; uint32_t etrack = 0;
-    if (active) {
+    // ---- event 1: one Woodcock flight and the choice of interaction
+    if (state == PH_FLIGHT) {
       bool done = false;
+      float skn = 0.f, lp2 = 0.f, mu_max = 0.f;
+      if (E >= kPcut) xs_lookup(s_xs, a.xs.x0, a.xs.inv_h, a.xs.n, E, skn, lp2, mu_max);
       if (E < kPcut) {                                   // below cut-off: absorbed on the spot
-        const long long q = quanta(E); pend.add(g, vox_index(g, vi, vj, vk), q); tl.dep += (unsigned long long)q;
+        const long long q = quanta(E); pend.add(g, cvox, q); tl.dep += (unsigned long long)q;
         if (DBG) { fnv.byte('A'); ++tl.st[ST_PCUT]; ++tl.st[ST_DEPOSITS]; }
         done = true;
-      } else if (!(xs.mu_max > 0.0f)) {
+      } else if (!(mu_max > 0.0f)) {
         tl.esc += (unsigned long long)quanta(E);
         if (DBG) { fnv.byte('E'); ++tl.st[ST_PESC]; if (!collided && rng.track == 0u) ++tl.st[ST_UNCOLLIDED]; }
         done = true;
       } else {
-        const float s = -logf(u_oc(rng.next())) / xs.mu_max;
-        x += s * u; y += s * v; z += s * w;
+        uint32_t d0, d1, d2, d3, g0, g1, g2, g3;
+        rng.window<2>(k0, k1, d0, d1, d2, d3, g0, g1, g2, g3);
+        rng.consume(2u, g0, g1, g2, g3);
+        const float s = -logf(u_oc(d0)) / mu_max;
+        x = __fmaf_rn(s, u, x); y = __fmaf_rn(s, v, y); z = __fmaf_rn(s, w, z);
         if (DBG) ++tl.st[ST_FLIGHTS];
+        int vi, vj, vk;
         if (!locate(g, x, y, z, vi, vj, vk)) {
           tl.esc += (unsigned long long)quanta(E);
           if (DBG) { fnv.byte('E'); ++tl.st[ST_PESC]; if (!collided && rng.track == 0u) ++tl.st[ST_UNCOLLIDED]; }
           done = true;
         } else {
-          const int vox = vox_index(g, vi, vj, vk);
-          const float rho = __ldg(g.density + vox); const int mt = __ldg(g.material + vox);
-          const float muC = rho * (c_mat.ne[mt] * xs.skn), muT = rho * (c_mat.cphoto[mt] * xs.inv_e3), muK = rho * (c_mat.ppair[mt] * xs.lp2);
-          const float tt = u_co(rng.next()) * xs.mu_max;
-          if (tt < muC) {                                // Compton
-            collided = true;
+          cvox = vox_index(g, vi, vj, vk);
+          const float rho = __ldg(g.density + cvox); const int mt = __ldg(g.material + cvox);
+          const float inv_e3 = 1.0f / (E * E * E);
+          const float muC = rho * (c_mat.ne[mt] * skn), muT = rho * (c_mat.cphoto[mt] * inv_e3), muK = rho * (c_mat.ppair[mt] * lp2);
+          const float tt = u_co(d1) * mu_max;
+          if (tt < muC) {                                // Compton: Kahn trials are event 2
+            collided = true; state = PH_KAHN;
             if (DBG) { fnv.byte('C'); ++tl.st[ST_COMPTON]; }
-            const float alpha = E / kMe, eta = kahn(alpha, rng);
-            const float k = (eta - 1.0f) / alpha, ct = 1.0f - k, sn = sqrtf(fmaxf(0.0f, k * (2.0f - k)));
-            const float uphi = u_co(rng.next());
-            const float Ep = E / eta, T = E - Ep, u0 = u, v0 = v, w0 = w;
-            rotate(u, v, w, ct, sn, uphi);
-            if (T >= kEcut && !a.electrons_local) {
-              float dxe = E * u0 - Ep * u, dye = E * v0 - Ep * v, dze = E * w0 - Ep * w;
-              const float n2 = dxe * dxe + dye * dye + dze * dze;
-              if (n2 > 0.0f) { const float inv = rsqrtf(n2); ex = dxe * inv; ey = dye * inv; ez = dze * inv; }
-              else { ex = u0; ey = v0; ez = w0; }
-              eT = T; etrack = child_track(rng.track, nchild, 0u); push_e = true;
-              if (DBG) ++tl.st[ST_SEC_E];
-            } else {
-              const long long q = quanta(T); pend.add(g, vox, q); tl.dep += (unsigned long long)q;
-              if (DBG) ++tl.st[ST_DEPOSITS];
-            }
-            ++nchild; E = Ep; xs.set(E, rhomax);
           } else if (tt < muC + muT) {                   // photo-electric: local absorption
-            const long long q = quanta(E); pend.add(g, vox, q); tl.dep += (unsigned long long)q;
+            const long long q = quanta(E); pend.add(g, cvox, q); tl.dep += (unsigned long long)q;
             if (DBG) { fnv.byte('P'); ++tl.st[ST_PHOTO]; ++tl.st[ST_DEPOSITS]; }
             done = true;
-          } else if (tt < muC + muT + muK) {             // pair production (rare: plain per-lane pushes)
+          } else if (tt < muC + muT + muK) {             // pair production: event 2
+            state = PH_PAIR;
             if (DBG) { fnv.byte('X'); ++tl.st[ST_PAIR]; }
-            const float Tsum = E - kEPair, Tm = u_co(rng.next()) * Tsum, Tp = Tsum - Tm;
-            const float Tc[2] = {Tm, Tp};
-#pragma unroll
-            for (int sl = 0; sl < 2; ++sl) {
-              if (Tc[sl] >= kEcut && !a.electrons_local) {
-                queue_push1(a.eq, a.ctl, x, y, z, Tc[sl], u, v, w, h, child_track(rng.track, nchild, sl));
-                if (DBG) ++tl.st[ST_SEC_E];
-              } else {
-                const long long q = quanta(Tc[sl]); pend.add(g, vox, q); tl.dep += (unsigned long long)q;
-                if (DBG) ++tl.st[ST_DEPOSITS];
-              }
-            }
-            const float cz = 2.0f * u_co(rng.next()) - 1.0f, sz = sqrtf(fmaxf(0.0f, 1.0f - cz * cz));
-            float sa, ca; sincospif(2.0f * u_co(rng.next()), &sa, &ca);
-            const float nx = sz * ca, ny = sz * sa;
-            queue_push1(a.pq, a.ctl, x, y, z, kEAnnih, nx, ny, cz, h, child_track(rng.track, nchild, 2u));
-            queue_push1(a.pq, a.ctl, x, y, z, kEAnnih, -nx, -ny, -cz, h, child_track(rng.track, nchild, 3u));
-            if (DBG) tl.st[ST_SEC_P] += 2;
-            done = true;
           } else if (DBG) { fnv.byte('V'); ++tl.st[ST_VIRTUAL]; }
         }
       }
-      if (done) { if (DBG) finish_track<DBG>(a, h, fnv); active = false; }
+      if (done) { if (DBG) finish_track<DBG>(a, h, fnv); state = PH_IDLE; }
+    }
+
+    // ---- event 2: one Kahn trial (+ Compton kinematics when accepted) or the pair split
+    bool push_e = false; float ex = 0, ey = 0, ez = 0, eT = 0; uint32_t etrack = 0;
+    if (state >= PH_KAHN) {
+      uint32_t d0, d1, d2, d3, g0, g1, g2, g3;
+      rng.window<4>(k0, k1, d0, d1, d2, d3, g0, g1, g2, g3);
+      if (state == PH_KAHN) {
+        // Kahn's rejection (P5).  With dn = 1 + 2 alpha r2:  branch A: eta = dn, branch B:
+        // eta = (2 alpha + 1)/dn.  k = (eta - 1)/alpha is 2 r2 (A) or 2 (1 - r2)/dn (B) in exact
+        // arithmetic; these forms have no cancellation in fp32.
+        const float alpha = E / kMe, ta = 2.0f * alpha, tp1 = ta + 1.0f;
+        const float r1 = u_co(d0), r2 = u_co(d1), r3 = u_co(d2);
+        const float dn = __fmaf_rn(ta, r2, 1.0f), idn = 1.0f / dn;
+        const bool brA = r1 <= tp1 / (ta + 9.0f);
+        const float ie = brA ? idn : dn / tp1;                          // 1/eta
+        const float k = brA ? 2.0f * r2 : 2.0f * (1.0f - r2) * idn;     // 1 - cos(theta)
+        const float ct = 1.0f - k;
+        const bool accept = brA ? (r3 <= 4.0f * (ie - ie * ie)) : (r3 <= 0.5f * (ct * ct + ie));
+        if (accept) {
+          rng.consume(4u, g0, g1, g2, g3);
+          const float sn = sqrtf(fmaxf(0.0f, k * (2.0f - k)));
+          const float Ep = E * ie, T = E - Ep, u0 = u, v0 = v, w0 = w;
+          rotate(u, v, w, ct, sn, u_co(d3));
+          if (T >= kEcut && !a.electrons_local) {
+            const float dxe = E * u0 - Ep * u, dye = E * v0 - Ep * v, dze = E * w0 - Ep * w;
+            const float n2 = dxe * dxe + dye * dye + dze * dze;
+            if (n2 > 0.0f) { const float inv = rsqrtf(n2); ex = dxe * inv; ey = dye * inv; ez = dze * inv; }
+            else { ex = u0; ey = v0; ez = w0; }
+            eT = T; etrack = child_track(rng.track, nchild, 0u); push_e = true;
+            if (DBG) ++tl.st[ST_SEC_E];
+          } else {
+            const long long q = quanta(T); pend.add(g, cvox, q); tl.dep += (unsigned long long)q;
+            if (DBG) ++tl.st[ST_DEPOSITS];
+          }
+          ++nchild; E = Ep; state = PH_FLIGHT;
+        } else rng.consume(3u, g0, g1, g2, g3);
+      } else {                                           // pair production (rare: plain per-lane pushes)
+        rng.consume(3u, g0, g1, g2, g3);
+        const float Tsum = E - kEPair, Tm = u_co(d0) * Tsum, Tp = Tsum - Tm;
+        const float Tc[2] = {Tm, Tp};
+#pragma unroll
+        for (int sl = 0; sl < 2; ++sl) {
+          if (Tc[sl] >= kEcut && !a.electrons_local) {
+            queue_push1(a.eq, a.ctl, x, y, z, Tc[sl], u, v, w, h, child_track(rng.track, nchild, sl));
+            if (DBG) ++tl.st[ST_SEC_E];
+          } else {
+            const long long q = quanta(Tc[sl]); pend.add(g, cvox, q); tl.dep += (unsigned long long)q;
+            if (DBG) ++tl.st[ST_DEPOSITS];
+          }
+        }
+        const float cz = 2.0f * u_co(d1) - 1.0f, sz = sqrtf(fmaxf(0.0f, 1.0f - cz * cz));
+        float sa, ca; sincospif(2.0f * u_co(d2), &sa, &ca);
+        const float nx = sz * ca, ny = sz * sa;
+        queue_push1(a.pq, a.ctl, x, y, z, kEAnnih, nx, ny, cz, h, child_track(rng.track, nchild, 2u));
+        queue_push1(a.pq, a.ctl, x, y, z, kEAnnih, -nx, -ny, -cz, h, child_track(rng.track, nchild, 3u));
+        if (DBG) { tl.st[ST_SEC_P] += 2; finish_track<DBG>(a, h, fnv); }
+        state = PH_IDLE;
+      }
     }
     // ---- Compton electrons: warp ballot + prefix sum, one tail atomic per warp
     unsigned slot;
@@ -258,21 +300,24 @@ __global__ void __launch_bounds__(kThreads) k_photon(const __grid_constant__ Tra
 // Electrons carry (voxel index, offset inside the voxel) instead of global coordinates: fp32 then
 // resolves positions to ~3e-8 cm relative to the voxel faces that decide every step, instead of the
 // ~1e-6 cm of a global coordinate.  In exact arithmetic this is the
-// same walk as floor((pos - o)/d) on global coordinates.
+// same walk as floor((pos - o)/d) on global coordinates.  One loop iteration = one sub-step; the two
+// draws of a condensed step come from one Philox site (draw numbers are always even here).
 template <bool DBG>
-__global__ void __launch_bounds__(kThreads) k_electron(const __grid_constant__ TransportArgs a) {
+__global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant__ TransportArgs a) {
   const Grid &g = a.g;
+  const uint32_t k0 = (uint32_t)a.seed, k1 = (uint32_t)(a.seed >> 32);
   const unsigned count = *a.src_count;
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
   Pending pend; pend.v = 0; pend.q = 0;
   bool active = false, exhausted = false;
   float lx = 0, ly = 0, lz = 0, u = 0, v = 0, w = 1, T = 0;      // offset inside voxel (vi,vj,vk), direction, energy
+  float iu = 0, iv = 0, iw = 1;                                   // reciprocal direction cosines (refreshed when the direction changes)
   int vi = 0, vj = 0, vk = 0;
   unsigned long long h = 0; uint32_t steps = 0;
   // condensed step (P7): energy still to lose in it, rho*s/X0 accumulated, energy at its start
   float budget = 0, tacc = 0, Tms = 0; bool fresh = true;
-  Philox rng; rng.n = 0; rng.track = 0; rng.k0 = rng.k1 = rng.hlo = rng.hhi = 0; rng.w0 = rng.w1 = rng.w2 = rng.w3 = 0;
+  RngWin rng; rng.init(0ull, 0u, 0u);
   Fnv fnv; fnv.v = 0;
 
   for (;;) {
@@ -282,7 +327,7 @@ __global__ void __launch_bounds__(kThreads) k_electron(const __grid_constant__ T
       if (t.ok) {
         float x = t.x, y = t.y, z = t.z;
         u = t.u; v = t.v; w = t.w; T = t.E; h = t.h; steps = 0; fresh = true;
-        rng.init(a.seed, h, t.track, t.ndraw);
+        rng.init(h, t.track, t.ndraw);
         if (DBG) { fnv.init(t.track); ++tl.st[ST_ETRACKS]; }
         if (a.src_kind == SRC_BUFFER && a.buffer_is_debug) tl.inc += (unsigned long long)quanta(T);
         active = true;
@@ -292,21 +337,21 @@ __global__ void __launch_bounds__(kThreads) k_electron(const __grid_constant__ T
           active = false;
         } else {
           lx = (x - g.ox) - (float)vi * g.dx; ly = (y - g.oy) - (float)vj * g.dy; lz = (z - g.oz) - (float)vk * g.dz;
+          iu = 1.0f / u; iv = 1.0f / v; iw = 1.0f / w;
         }
       }
     }
     if (!__any_sync(kFull, active)) { if (exhausted) break; else continue; }
 
-    if (active) {                                        // one condensed-history step
+    if (active) {                                        // one sub-step
       const int vox = vox_index(g, vi, vj, vk);
       const float rho = __ldg(g.density + vox); const int mt = __ldg(g.material + vox);
       if (fresh) { budget = kFe * T; Tms = T; tacc = 0.0f; fresh = false; }
       const float D = c_mat.sscale[mt] * (1.52f + 0.25f / T + 0.078f * T) * rho;
       const float sE = D > 0.0f ? budget / D : INFINITY;
-      float sv = INFINITY;
-      if (u > 0.0f) sv = fminf(sv, (g.dx - lx) / u); else if (u < 0.0f) sv = fminf(sv, -lx / u);
-      if (v > 0.0f) sv = fminf(sv, (g.dy - ly) / v); else if (v < 0.0f) sv = fminf(sv, -ly / v);
-      if (w > 0.0f) sv = fminf(sv, (g.dz - lz) / w); else if (w < 0.0f) sv = fminf(sv, -lz / w);
+      // distance to the exit face of this voxel (a zero direction component never limits)
+      const float sx = (u > 0.0f ? g.dx - lx : -lx) * iu, sy = (v > 0.0f ? g.dy - ly : -ly) * iv, sz = (w > 0.0f ? g.dz - lz : -lz) * iw;
+      float sv = fminf(fminf(u != 0.0f ? sx : INFINITY, v != 0.0f ? sy : INFINITY), w != 0.0f ? sz : INFINITY);
       sv = fmaxf(sv, 0.0f);
       const bool turn = sE <= sv + kEpsB;              // this sub-step ends the condensed step
       const float s = turn ? sE : sv + kEpsB, dT = turn ? budget : D * s;
@@ -319,7 +364,8 @@ __global__ void __launch_bounds__(kThreads) k_electron(const __grid_constant__ T
         done = true;
       } else {
         const long long q = quanta(dT); pend.add(g, vox, q); tl.dep += (unsigned long long)q;
-        lx += s * u; ly += s * v; lz += s * w; T -= dT; budget -= dT; tacc += rho * s * c_mat.inv_x0[mt];
+        lx = __fmaf_rn(s, u, lx); ly = __fmaf_rn(s, v, ly); lz = __fmaf_rn(s, w, lz);
+        T -= dT; budget -= dT; tacc += rho * s * c_mat.inv_x0[mt];
         // re-home: a step ends at most eps beyond the face it was limited by
         if (lx >= g.dx) { lx -= g.dx; ++vi; } else if (lx < 0.0f) { lx += g.dx; --vi; }
         if (ly >= g.dy) { ly -= g.dy; ++vj; } else if (ly < 0.0f) { ly += g.dy; --vj; }
@@ -329,12 +375,15 @@ __global__ void __launch_bounds__(kThreads) k_electron(const __grid_constant__ T
           if (DBG) { fnv.u32(steps); fnv.byte('E'); ++tl.st[ST_EESC]; }
           done = true;
         } else if (turn) {
+          uint32_t d0, d1, d2, d3, g0, g1, g2, g3;
+          rng.window<2>(k0, k1, d0, d1, d2, d3, g0, g1, g2, g3);
+          rng.consume(2u, g0, g1, g2, g3);
           const float pbeta = Tms * (Tms + 2.0f * kMe) / (Tms + kMe);
           const float th0 = 13.6f / pbeta * sqrtf(tacc);
-          const float a1 = u_oc(rng.next()), b1 = u_co(rng.next());
-          const float th = fminf(kPi, th0 * sqrtf(-2.0f * logf(a1)));
+          const float th = fminf(kPi, th0 * sqrtf(-2.0f * logf(u_oc(d0))));
           float st, ct; sincosf(th, &st, &ct);
-          rotate(u, v, w, ct, st, b1);
+          rotate(u, v, w, ct, st, u_co(d1));
+          iu = 1.0f / u; iv = 1.0f / v; iw = 1.0f / w;
           fresh = true;
         }
       }
