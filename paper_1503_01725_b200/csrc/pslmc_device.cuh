@@ -74,23 +74,24 @@ struct RngWin {
   __device__ __forceinline__ void init(uint64_t h, uint32_t trk, uint32_t ndraw) {
     hlo = (uint32_t)h; hhi = (uint32_t)(h >> 32); track = trk; n = ndraw; c0 = c1 = c2 = c3 = 0u;   // ndraw & 3 == 0
   }
-  __device__ __forceinline__ void gen(uint32_t k0, uint32_t k1, uint32_t j, uint32_t &g0, uint32_t &g1, uint32_t &g2, uint32_t &g3) const {
-    uint32_t x0 = j, x1 = track, x2 = hlo, x3 = hhi, a = k0, b = k1;
+  // ks = the 10 round keys (k0 + r*0x9E3779B9, k1 + r*0xBB67AE85), host-computed kernel parameters:
+  // the XORs then take them straight from the constant bank.
+  __device__ __forceinline__ void gen(const uint32_t (&ks)[20], uint32_t j, uint32_t &g0, uint32_t &g1, uint32_t &g2, uint32_t &g3) const {
+    uint32_t x0 = j, x1 = track, x2 = hlo, x3 = hhi;
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
       const uint32_t h0 = __umulhi(0xD2511F53u, x0), l0 = 0xD2511F53u * x0;
       const uint32_t h1 = __umulhi(0xCD9E8D57u, x2), l1 = 0xCD9E8D57u * x2;
-      x0 = h1 ^ x1 ^ a; x1 = l1; x2 = h0 ^ x3 ^ b; x3 = l0;
-      a += 0x9E3779B9u; b += 0xBB67AE85u;
+      x0 = h1 ^ x1 ^ ks[2 * r]; x1 = l1; x2 = h0 ^ x3 ^ ks[2 * r + 1]; x3 = l0;
     }
     g0 = x0; g1 = x1; g2 = x2; g3 = x3;
   }
   template <int K>
-  __device__ __forceinline__ void window(uint32_t k0, uint32_t k1, uint32_t &d0, uint32_t &d1, uint32_t &d2, uint32_t &d3,
+  __device__ __forceinline__ void window(const uint32_t (&ks)[20], uint32_t &d0, uint32_t &d1, uint32_t &d2, uint32_t &d3,
                                          uint32_t &g0, uint32_t &g1, uint32_t &g2, uint32_t &g3) {
     const uint32_t s = n & 3u;
     g0 = g1 = g2 = g3 = 0u;
-    if (s == 0u || s + K > 4u) gen(k0, k1, (n + 3u) >> 2, g0, g1, g2, g3);
+    if (s == 0u || s + K > 4u) gen(ks, (n + 3u) >> 2, g0, g1, g2, g3);
     if (s == 0u) { c0 = g0; c1 = g1; c2 = g2; c3 = g3; }
     d0 = s == 0u ? c0 : (s == 1u ? c1 : (s == 2u ? c2 : c3));
     d1 = s == 0u ? c1 : (s == 1u ? c2 : (s == 2u ? c3 : g0));
@@ -183,35 +184,41 @@ struct PhotonXs {
 };
 
 // Photon cross-section table (built per mc_dose call on the device, in double, by k_build_xs): node i
-// holds (sigma_KN, ln^2(E/1.022), mu_max, 0) at log2(E) = x0 + i*h; k_photon keeps it in shared memory
-// and interpolates linearly in log2(E) (relative error ~1e-7 at n = 4096: DESIGN.md §6).
-struct XsTable { const float4 *nodes; float x0, inv_h; int n; };      // n intervals, n + 1 nodes
+// holds (sigma_KN, mu_max) at log2(E) = x0 + i*h; k_photon keeps it in shared memory and interpolates
+// linearly in log2(E) (relative error ~1e-7 at n = 4096: DESIGN.md §6).  ln(E/1.022) of the pair term
+// comes from the same log2(E).
+struct XsTable { const float2 *nodes; float x0, inv_h; int n; };      // n intervals, n + 1 nodes
 
-__device__ __forceinline__ void xs_lookup(const float4 *tab, float x0, float inv_h, int n, float E,
+__device__ __forceinline__ void xs_lookup(const float2 *tab, float x0, float inv_h, int n, float E,
                                           float &skn, float &lp2, float &mu_max) {
-  float t = (__log2f(E) - x0) * inv_h;
+  const float lg = __log2f(E);
+  float t = (lg - x0) * inv_h;
   t = fminf(fmaxf(t, 0.0f), (float)n);
-  int i = min((int)t, n - 1);
+  const int i = min((int)t, n - 1);
   const float f = t - (float)i;
-  const float4 A = tab[i], B = tab[i + 1];
-  skn = __fmaf_rn(f, B.x - A.x, A.x); lp2 = __fmaf_rn(f, B.y - A.y, A.y); mu_max = __fmaf_rn(f, B.z - A.z, A.z);
+  const float2 A = tab[i], B = tab[i + 1];
+  skn = __fmaf_rn(f, B.x - A.x, A.x); mu_max = __fmaf_rn(f, B.y - A.y, A.y);
+  const float l = E > kEPair ? (lg - 0.03139551f) * 0.69314718f : 0.0f;      // log2(1.022) = 0.0313955
+  lp2 = l * l;
 }
 
-// Rotate unit vector d by polar angle (ct, st) and azimuth phi = 2*pi*uphi.
+__device__ __forceinline__ float sqrt_fast(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
 __device__ __forceinline__ void rotate(float &u, float &v, float &w, float ct, float st, float uphi) {
   float sp, cp;
   sincospif(2.0f * uphi, &sp, &cp);
   float nx, ny, nz;
-  const float s2 = u * u + v * v;                         // = 1 - w^2 for a unit vector, without the cancellation
+  const float s2 = __fmaf_rn(u, u, v * v);                // = 1 - w^2 for a unit vector, without the cancellation
   if (s2 > 1e-20f) {
-    float s = sqrtf(s2), is = 1.0f / s;
-    nx = u * ct + st * (u * w * cp - v * sp) * is;
-    ny = v * ct + st * (v * w * cp + u * sp) * is;
-    nz = w * ct - s * st * cp;
+    const float is = rsqrtf(s2), s = s2 * is, a = st * is;
+    nx = __fmaf_rn(u, ct, a * __fmaf_rn(u * w, cp, -(v * sp)));
+    ny = __fmaf_rn(v, ct, a * __fmaf_rn(v * w, cp, u * sp));
+    nz = __fmaf_rn(w, ct, -(s * st) * cp);
   } else {
     nx = st * cp; ny = st * sp; nz = w > 0.0f ? ct : -ct;
   }
-  float inv = rsqrtf(nx * nx + ny * ny + nz * nz);
+  const float inv = rsqrtf(__fmaf_rn(nx, nx, __fmaf_rn(ny, ny, nz * nz)));
   u = nx * inv; v = ny * inv; w = nz * inv;
 }
 

@@ -52,7 +52,7 @@ static Layout make_layout(uint64_t batch, size_t nvox, bool with_acc) {
   Layout L; size_t o = 0;
   auto take = [&](size_t b) { size_t at = o; o += align_up(b); return at; };
   L.eq_cap = (unsigned)std::min<uint64_t>(4 * batch, 0x7fffffffu); L.pq_cap = (unsigned)batch;
-  L.ctl = take(sizeof(Control)); L.off = take(sizeof(uint64_t) * 160); L.xs = take(sizeof(float4) * (kXsIntervals + 1));
+  L.ctl = take(sizeof(Control)); L.off = take(sizeof(uint64_t) * 160); L.xs = take(kXsBytes);
   L.p0 = take(16 * batch); L.p1 = take(16 * batch);
   for (int k = 0; k < 3; ++k) L.eq[k] = take((size_t)16 * L.eq_cap);
   for (int k = 0; k < 3; ++k) L.pq[k] = take((size_t)16 * L.pq_cap);
@@ -165,6 +165,7 @@ struct Run {
   TransportArgs base_args() const {
     TransportArgs a{};
     a.g = g; a.ctl = ctl; a.seed = seed; a.n_total = n_total; a.perm_a = perm_a;
+    for (int r = 0; r < 10; ++r) { a.ks[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; a.ks[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u; }
     a.p0 = (const float4 *)(ws + L.p0); a.p1 = (const float4 *)(ws + L.p1);
     a.eq = queue(L.eq, &ctl->n_eq, L.eq_cap); a.pq = queue(L.pq, &ctl->n_pq, L.pq_cap);
     a.fp = fp; a.fp_base = fp_base;
@@ -174,17 +175,20 @@ struct Run {
     return a;
   }
   XsTable xs{};
-  static constexpr size_t kXsSmem = sizeof(float4) * (kXsIntervals + 1);
+  static constexpr size_t kXsSmem = kXsBytes + sizeof(StageRing) * (kThreads / 32);   // k_photon dynamic shared memory
   // Builds the cross-section table of this call (after k_rhomax) for photon energies up to e_max.
   void build_xs(double e_max) {
     const double x0 = std::log2(0.045), x1 = std::log2(e_max * 1.001), hh = (x1 - x0) / kXsIntervals;
-    float4 *nodes = (float4 *)(ws + L.xs);
+    float2 *nodes = (float2 *)(ws + L.xs);
     k_build_xs<<<(kXsIntervals + 256) / 256, 256, 0, st>>>(ctl, nodes, x0, hh, kXsIntervals);
     xs.nodes = nodes; xs.x0 = (float)x0; xs.inv_h = (float)(1.0 / hh); xs.n = kXsIntervals;
   }
+  uint64_t batch = 0;                           // upper bound of the entries a photon launch can see
+  int photon_blocks(int persistent) const { return (int)std::max<uint64_t>(1, std::min<uint64_t>({(uint64_t)persistent, (batch + kThreads - 1) / kThreads, 4096 / (kThreads / 32)})); }
   void photon(const TransportArgs &a) {
     tm.begin(MC_K_PHOTON);
-    if (dbg) k_photon<true><<<blocks_photon[1], kThreads, kXsSmem, st>>>(a); else k_photon<false><<<blocks_photon[0], kThreads, kXsSmem, st>>>(a);
+    if (dbg) k_photon<true><<<photon_blocks(blocks_photon[1]), kThreads, kXsSmem, st>>>(a);
+    else k_photon<false><<<photon_blocks(blocks_photon[0]), kThreads, kXsSmem, st>>>(a);
     tm.end(MC_K_PHOTON); ++launches[MC_K_PHOTON];
   }
   void electron(const TransportArgs &a) {
@@ -279,7 +283,7 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
   r.st = (cudaStream_t)opts->cuda_stream; r.ws = (char *)ws; r.L = L; r.ctl = (Control *)(r.ws + L.ctl);
   long long *acc = opts->dose_acc ? (long long *)opts->dose_acc : (long long *)(r.ws + L.acc);
   r.g = make_grid(*ph, acc);
-  r.seed = seed; r.n_total = N; r.perm_a = mixed ? mixed_multiplier(N) : 0; r.flags = opts->flags;
+  r.seed = seed; r.n_total = N; r.perm_a = mixed ? mixed_multiplier(N) : 0; r.flags = opts->flags; r.batch = batch;
   r.fp = (unsigned long long *)opts->fingerprints; r.fp_base = hb;
   r.dbg = (opts->flags & MC_FLAG_STATS) || opts->fingerprints;
   r.tm.on = (opts->flags & MC_FLAG_TIMING) != 0; r.tm.st = r.st;
@@ -437,7 +441,7 @@ extern "C" int mc_transport_debug(const phantom_t *ph, int32_t particle_type, co
   Run r{};
   r.st = (cudaStream_t)opts->cuda_stream; r.ws = (char *)ws; r.L = L; r.ctl = (Control *)(r.ws + L.ctl);
   r.g = make_grid(*ph, (long long *)opts->dose_acc);
-  r.seed = seed; r.n_total = first_history + count; r.perm_a = 0; r.flags = opts->flags;
+  r.seed = seed; r.n_total = first_history + count; r.perm_a = 0; r.flags = opts->flags; r.batch = count;
   r.fp = (unsigned long long *)opts->fingerprints; r.fp_base = first_history;
   r.dbg = true; r.tm.on = false; r.init_blocks();
   cudaEvent_t ev0, ev1;

@@ -192,8 +192,7 @@ __global__ void k_rhomax(const float *density, const uint8_t *material, size_t n
 }
 
 // Photon cross-section table for this call (needs rhomax): node i at log2(E) = x0 + i*h, in double.
-constexpr int kXsIntervals = 4096;
-__global__ void k_build_xs(const Control *c, float4 *nodes, double x0, double h, int n) {
+__global__ void k_build_xs(const Control *c, float2 *nodes, double x0, double h, int n) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i > n) return;
   const double E = exp2(x0 + h * (double)i);
@@ -203,7 +202,7 @@ __global__ void k_build_xs(const Control *c, float4 *nodes, double x0, double h,
   double m = 0.0;
   for (int k = 0; k < 3; ++k)
     m = fmax(m, (double)c->rhomax[k] * ((double)c_mat.ne[k] * skn + (double)c_mat.cphoto[k] * ie3 + (double)c_mat.ppair[k] * lp2));
-  nodes[i] = make_float4((float)skn, (float)lp2, (float)m, 0.0f);
+  nodes[i] = make_float2((float)skn, (float)m);
 }
 
 // dose[v] = acc[v] 2^-32 / (rho_v V N)

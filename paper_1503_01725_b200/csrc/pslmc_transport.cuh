@@ -17,11 +17,22 @@ struct Queue {
 };
 
 enum { SRC_BUFFER = 0, SRC_QUEUE = 1 };
+#ifndef ELECTRON_CHUNK
+#define ELECTRON_CHUNK 32
+#endif
+#ifndef ELECTRON_REFILL_MIN
+#define ELECTRON_REFILL_MIN 8
+#endif
+constexpr int kElectronRefillMin = ELECTRON_REFILL_MIN;
+constexpr unsigned kElectronChunk = ELECTRON_CHUNK;
+constexpr int kXsIntervals = 4096;
+constexpr size_t kXsBytes = sizeof(float2) * (kXsIntervals + 2);     // padded to 16 bytes
 
 struct TransportArgs {
   Grid g;
   Control *ctl;
   unsigned long long seed;
+  uint32_t ks[20];                    // Philox round keys of `seed` (host-computed)
   // source
   int src_kind;                       // SRC_BUFFER: p0/p1 planes from k_sample;  SRC_QUEUE: src queue
   int buffer_is_debug;                // SRC_BUFFER only: 1 = indexed by history, p1.w = status (skip < 0)
@@ -75,17 +86,37 @@ __device__ __forceinline__ void finish_track(const TransportArgs &a, unsigned lo
   if (DBG && a.fp) atomicAdd(a.fp + (h - a.fp_base), f.v);
 }
 
-// Warp-aggregated push: lanes with `want` get consecutive slots behind one atomic.  Convergent call.
-__device__ __forceinline__ bool queue_reserve(const Queue &q, Control *ctl, bool want, unsigned &slot) {
-  const unsigned m = __ballot_sync(kFull, want);
-  if (!m) return false;
+// Warp-aggregated push through a per-warp shared-memory ring of 64 entries: lanes with `want` append
+// at consecutive ring positions (ballot + prefix sum); whenever the ring holds >= 32 entries the warp
+// takes 32 consecutive queue slots with ONE tail atomic and writes them as three coalesced 512-byte
+// rows.  No atomic and no global store in the common iteration; no holes in the queue.  Convergent calls.
+struct StageRing { float4 a[64], b[64]; uint4 c[64]; };           // 3 KiB per warp
+struct StageCursor { unsigned head, n; };
+__device__ __forceinline__ void stage_flush(const Queue &q, Control *ctl, StageRing &r, StageCursor &sc, unsigned n_out) {
   const unsigned lane = threadIdx.x & 31u;
+  __syncwarp();
   unsigned base = 0;
-  if (lane == (unsigned)(__ffs(m) - 1)) base = atomicAdd(q.count, __popc(m));
-  base = __shfl_sync(kFull, base, __ffs(m) - 1);
-  slot = base + __popc(m & ((1u << lane) - 1u));
-  if (want && slot >= q.cap) { ctl->overflow = 1u; return false; }
-  return want;
+  if (lane == 0) base = atomicAdd(q.count, n_out);
+  base = __shfl_sync(kFull, base, 0);
+  if (base + n_out > q.cap) ctl->overflow = 1u;
+  else if (lane < n_out) {
+    const unsigned p = (sc.head + lane) & 63u;
+    q.a[base + lane] = r.a[p]; q.b[base + lane] = r.b[p]; q.c[base + lane] = r.c[p];
+  }
+  sc.head = (sc.head + n_out) & 63u; sc.n -= n_out;
+  __syncwarp();
+}
+__device__ __forceinline__ void stage_push(const Queue &q, Control *ctl, StageRing &r, StageCursor &sc, bool want,
+                                           float4 A, float4 B, uint4 C) {
+  const unsigned m = __ballot_sync(kFull, want);
+  if (!m) return;
+  const unsigned lane = threadIdx.x & 31u;
+  if (want) {
+    const unsigned p = (sc.head + sc.n + __popc(m & ((1u << lane) - 1u))) & 63u;
+    r.a[p] = A; r.b[p] = B; r.c[p] = C;
+  }
+  sc.n += __popc(m);
+  if (sc.n >= 32u) stage_flush(q, ctl, r, sc, 32u);
 }
 // Divergent-context push of one track (rare paths: pair production).
 __device__ __forceinline__ void queue_push1(const Queue &q, Control *ctl, float x, float y, float z, float E,
@@ -96,20 +127,38 @@ __device__ __forceinline__ void queue_push1(const Queue &q, Control *ctl, float 
   q.c[slot] = make_uint4((uint32_t)h, (uint32_t)(h >> 32), track, 0u);
 }
 
-// Refill protocol shared by both kernels: lanes without a track take the next source indices.
-// Returns the source index for this lane or 0xffffffff.  `exhausted` becomes true (warp-uniform)
-// once the cursor passed the end.
-__device__ __forceinline__ unsigned refill_index(const TransportArgs &a, bool idle, unsigned count, bool &exhausted) {
+// Refill protocol shared by both kernels: lanes without a track take the next source indices.  A warp
+// takes `chunk` consecutive indices from the source cursor with ONE atomic and hands them out over
+// the next refills (warp-uniform cursor in `sc`).  Returns the source index for this lane or
+// 0xffffffff.  `exhausted` becomes true (warp-uniform) once the cursor passed the end.
+struct SrcCursor { unsigned next, end; };
+// Guided self-scheduling: the chunk shrinks with what was left at the warp's previous grab, so the
+// last chunks are small and the warps finish together.
+template <unsigned MAX_CHUNK>
+__device__ __forceinline__ unsigned source_chunk(const TransportArgs &a, unsigned count, unsigned seen_end, unsigned need) {
+  if (a.static_lanes) return 32u;
+  const unsigned warps = gridDim.x * (kThreads / 32), left = count - min(count, seen_end);
+  return min(MAX_CHUNK, max(need, (left / (warps * 2u)) & ~31u));     // near the end: exactly what the idle lanes need
+}
+template <int MIN_IDLE, unsigned MAX_CHUNK>
+__device__ __forceinline__ unsigned refill_index(const TransportArgs &a, bool idle, unsigned count, SrcCursor &sc, bool &exhausted) {
   const unsigned need = __ballot_sync(kFull, idle);
   if (!need || exhausted) return 0xffffffffu;
+  if (MIN_IDLE > 1 && need != kFull && __popc(need) < MIN_IDLE) return 0xffffffffu;   // refill in groups: the refill code then runs with more lanes
   if (a.static_lanes && need != kFull) return 0xffffffffu;       // ablation: a warp refills only when all lanes are done
-  const unsigned lane = threadIdx.x & 31u, leader = __ffs(need) - 1;
-  unsigned base = 0;
-  if (lane == leader) base = atomicAdd(a.src_head, __popc(need));
-  base = __shfl_sync(kFull, base, leader);
-  if (base + __popc(need) >= count) exhausted = true;
-  const unsigned idx = base + __popc(need & ((1u << lane) - 1u));
-  return (idle && idx < count) ? idx : 0xffffffffu;
+  const unsigned lane = threadIdx.x & 31u;
+  if (sc.next >= sc.end) {
+    const unsigned chunk = source_chunk<MAX_CHUNK>(a, count, sc.end, __popc(need));
+    unsigned base = 0;
+    if (lane == 0) base = atomicAdd(a.src_head, chunk);
+    base = __shfl_sync(kFull, base, 0);
+    if (base >= count) { exhausted = true; return 0xffffffffu; }
+    sc.next = base; sc.end = min(base + chunk, count);
+  }
+  const unsigned rank = __popc(need & ((1u << lane) - 1u)), avail = sc.end - sc.next;
+  const unsigned idx = sc.next + rank;
+  sc.next += min((unsigned)__popc(need), avail);
+  return (idle && rank < avail) ? idx : 0xffffffffu;
 }
 
 struct TrackIn { float x, y, z, u, v, w, E; unsigned long long h; uint32_t track, ndraw; bool ok; };
@@ -145,12 +194,15 @@ enum { PH_IDLE = 0, PH_FLIGHT = 1, PH_KAHN = 2, PH_PAIR = 3 };
 
 template <bool DBG>
 __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ TransportArgs a) {
-  extern __shared__ float4 s_xs[];
+  extern __shared__ __align__(16) unsigned char s_raw[];           // [xs table | one StageRing per warp]
+  float2 *s_xs = reinterpret_cast<float2 *>(s_raw);
   for (int i = threadIdx.x; i <= a.xs.n; i += kThreads) s_xs[i] = a.xs.nodes[i];
   __syncthreads();
   const Grid &g = a.g;
-  const uint32_t k0 = (uint32_t)a.seed, k1 = (uint32_t)(a.seed >> 32);
-  const unsigned count = *a.src_count;
+  const unsigned count = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
+  SrcCursor sc; sc.next = sc.end = 0u;
+  StageRing &ring = *reinterpret_cast<StageRing *>(s_raw + kXsBytes + sizeof(StageRing) * (threadIdx.x >> 5));
+  StageCursor stg; stg.head = stg.n = 0u;
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
   Pending pend; pend.v = 0; pend.q = 0;
@@ -163,7 +215,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
 
   for (;;) {
     // ---- refill idle lanes
-    const unsigned idx = refill_index(a, state == PH_IDLE, count, exhausted);
+    const unsigned idx = refill_index<1, 128u>(a, state == PH_IDLE, count, sc, exhausted);
     if (idx != 0xffffffffu) {
       const TrackIn t = load_track(a, idx);
       if (t.ok) {
@@ -195,7 +247,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
         done = true;
       } else {
         uint32_t d0, d1, d2, d3, g0, g1, g2, g3;
-        rng.window<2>(k0, k1, d0, d1, d2, d3, g0, g1, g2, g3);
+        rng.window<2>(a.ks, d0, d1, d2, d3, g0, g1, g2, g3);
         rng.consume(2u, g0, g1, g2, g3);
         const float s = -logf(u_oc(d0)) / mu_max;
         x = __fmaf_rn(s, u, x); y = __fmaf_rn(s, v, y); z = __fmaf_rn(s, w, z);
@@ -231,7 +283,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
     bool push_e = false; float ex = 0, ey = 0, ez = 0, eT = 0; uint32_t etrack = 0;
     if (state >= PH_KAHN) {
       uint32_t d0, d1, d2, d3, g0, g1, g2, g3;
-      rng.window<4>(k0, k1, d0, d1, d2, d3, g0, g1, g2, g3);
+      rng.window<4>(a.ks, d0, d1, d2, d3, g0, g1, g2, g3);
       if (state == PH_KAHN) {
         // Kahn's rejection (P5).  With dn = 1 + 2 alpha r2:  branch A: eta = dn, branch B:
         // eta = (2 alpha + 1)/dn.  k = (eta - 1)/alpha is 2 r2 (A) or 2 (1 - r2)/dn (B) in exact
@@ -286,12 +338,10 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
       }
     }
     // ---- Compton electrons: warp ballot + prefix sum, one tail atomic per warp
-    unsigned slot;
-    if (queue_reserve(a.eq, a.ctl, push_e, slot)) {
-      a.eq.a[slot] = make_float4(x, y, z, eT); a.eq.b[slot] = make_float4(ex, ey, ez, 0.f);
-      a.eq.c[slot] = make_uint4((uint32_t)h, (uint32_t)(h >> 32), etrack, 0u);
-    }
+    stage_push(a.eq, a.ctl, ring, stg, push_e, make_float4(x, y, z, eT), make_float4(ex, ey, ez, 0.f),
+               make_uint4((uint32_t)h, (uint32_t)(h >> 32), etrack, 0u));
   }
+  if (stg.n) stage_flush(a.eq, a.ctl, ring, stg, stg.n);
   pend.flush(g);
   tally_flush<DBG>(a, tl);
 }
@@ -305,8 +355,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
 template <bool DBG>
 __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant__ TransportArgs a) {
   const Grid &g = a.g;
-  const uint32_t k0 = (uint32_t)a.seed, k1 = (uint32_t)(a.seed >> 32);
-  const unsigned count = *a.src_count;
+  const unsigned count = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
+  SrcCursor sc; sc.next = sc.end = 0u;
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
   Pending pend; pend.v = 0; pend.q = 0;
@@ -321,7 +371,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
   Fnv fnv; fnv.v = 0;
 
   for (;;) {
-    const unsigned idx = refill_index(a, !active, count, exhausted);
+    const unsigned idx = refill_index<kElectronRefillMin, kElectronChunk>(a, !active, count, sc, exhausted);
     if (idx != 0xffffffffu) {
       const TrackIn t = load_track(a, idx);
       if (t.ok) {
@@ -337,7 +387,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
           active = false;
         } else {
           lx = (x - g.ox) - (float)vi * g.dx; ly = (y - g.oy) - (float)vj * g.dy; lz = (z - g.oz) - (float)vk * g.dz;
-          iu = 1.0f / u; iv = 1.0f / v; iw = 1.0f / w;
+          iu = rcp_fast(u); iv = rcp_fast(v); iw = rcp_fast(w);
         }
       }
     }
@@ -347,8 +397,8 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
       const int vox = vox_index(g, vi, vj, vk);
       const float rho = __ldg(g.density + vox); const int mt = __ldg(g.material + vox);
       if (fresh) { budget = kFe * T; Tms = T; tacc = 0.0f; fresh = false; }
-      const float D = c_mat.sscale[mt] * (1.52f + 0.25f / T + 0.078f * T) * rho;
-      const float sE = D > 0.0f ? budget / D : INFINITY;
+      const float D = (c_mat.sscale[mt] * rho) * __fmaf_rn(0.078f, T, __fmaf_rn(0.25f, rcp_fast(T), 1.52f));
+      const float sE = D > 0.0f ? __fdividef(budget, D) : INFINITY;
       // distance to the exit face of this voxel (a zero direction component never limits)
       const float sx = (u > 0.0f ? g.dx - lx : -lx) * iu, sy = (v > 0.0f ? g.dy - ly : -ly) * iv, sz = (w > 0.0f ? g.dz - lz : -lz) * iw;
       float sv = fminf(fminf(u != 0.0f ? sx : INFINITY, v != 0.0f ? sy : INFINITY), w != 0.0f ? sz : INFINITY);
@@ -365,7 +415,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
       } else {
         const long long q = quanta(dT); pend.add(g, vox, q); tl.dep += (unsigned long long)q;
         lx = __fmaf_rn(s, u, lx); ly = __fmaf_rn(s, v, ly); lz = __fmaf_rn(s, w, lz);
-        T -= dT; budget -= dT; tacc += rho * s * c_mat.inv_x0[mt];
+        T -= dT; budget -= dT; tacc = __fmaf_rn(rho * s, c_mat.inv_x0[mt], tacc);
         // re-home: a step ends at most eps beyond the face it was limited by
         if (lx >= g.dx) { lx -= g.dx; ++vi; } else if (lx < 0.0f) { lx += g.dx; --vi; }
         if (ly >= g.dy) { ly -= g.dy; ++vj; } else if (ly < 0.0f) { ly += g.dy; --vj; }
@@ -376,14 +426,14 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
           done = true;
         } else if (turn) {
           uint32_t d0, d1, d2, d3, g0, g1, g2, g3;
-          rng.window<2>(k0, k1, d0, d1, d2, d3, g0, g1, g2, g3);
+          rng.window<2>(a.ks, d0, d1, d2, d3, g0, g1, g2, g3);
           rng.consume(2u, g0, g1, g2, g3);
-          const float pbeta = Tms * (Tms + 2.0f * kMe) / (Tms + kMe);
-          const float th0 = 13.6f / pbeta * sqrtf(tacc);
-          const float th = fminf(kPi, th0 * sqrtf(-2.0f * logf(u_oc(d0))));
+          // theta = (13.6 / p beta) sqrt(tacc) sqrt(-2 ln a), p beta = Tms (Tms + 2 me)/(Tms + me): one division, one root
+          const float c = __fdividef(13.6f * (Tms + kMe), Tms * (Tms + 2.0f * kMe));
+          const float th = fminf(kPi, c * sqrt_fast(tacc * (-2.0f * logf(u_oc(d0)))));
           float st, ct; sincosf(th, &st, &ct);
           rotate(u, v, w, ct, st, u_co(d1));
-          iu = 1.0f / u; iv = 1.0f / v; iw = 1.0f / w;
+          iu = rcp_fast(u); iv = rcp_fast(v); iw = rcp_fast(w);
           fresh = true;
         }
       }
