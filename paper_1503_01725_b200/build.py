@@ -28,7 +28,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tmp = LIB + ".tmp%d" % os.getpid()
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
+        cmd = [nvcc] + NVCC_FLAGS + os.environ.get("PSLMC_NVCC_EXTRA", "").split() + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)
     return LIB

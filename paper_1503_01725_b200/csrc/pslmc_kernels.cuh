@@ -25,7 +25,8 @@ struct Control {
   unsigned overflow;               // a queue was full: result invalid → MC_E_OVERFLOW
   unsigned hw_eq, hw_pq;           // queue high-water marks
   unsigned pad2;
-  unsigned long long n_accepted;   // primaries that passed the jaws
+  unsigned long long n_accepted;   // primaries that passed the jaws and entered the phantom
+  unsigned long long n_missed;     // primaries that passed the jaws but missed the phantom (k_sample, compact mode)
   unsigned long long ledger[kLedgerSlots][4][2];   // [slot][incident,deposited,escaped,jaw][lo,hi] quanta
   unsigned long long stat[ST_COUNT];
   float rhomax[4];                 // largest density per material (as float, written via atomicMax on bits)
@@ -64,6 +65,8 @@ struct SampleArgs {
   unsigned long long *fp;            // fingerprints or null
   unsigned long long fp_base;
   int compact;                       // 1: survivors packed, p1.w = local index bits; 0: indexed by t, p1.w = status
+  Grid g;                            // compact mode: survivors are moved to their phantom entry point here (P4),
+  int stats;                         //   with every lane of the warp busy, instead of in the transport kernels' refill
 };
 
 __device__ __forceinline__ unsigned long long history_of(unsigned long long t, unsigned long long perm_a, unsigned long long n_total) {
@@ -73,15 +76,16 @@ __device__ __forceinline__ unsigned long long history_of(unsigned long long t, u
 // ------------------------------------------------------------------ k_sample
 __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ SampleArgs a) {
   __shared__ unsigned long long s_off[160];
-  __shared__ unsigned long long s_led[kThreads / 32][2];
+  __shared__ unsigned long long s_led[kThreads / 32][3];
+  __shared__ unsigned s_miss[kThreads / 32];
   const SourceModel &m = a.m;
   for (int i = threadIdx.x; i <= m.n_groups; i += kThreads) s_off[i] = a.off_g[i];
   __syncthreads();
   const unsigned t = blockIdx.x * kThreads + threadIdx.x;
   const unsigned lane = threadIdx.x & 31u;
   const bool live = t < a.count;
-  unsigned long long q_inc = 0, q_jaw = 0;
-  bool pass = false;
+  unsigned long long q_inc = 0, q_jaw = 0, q_esc = 0;
+  bool pass = false, missed = false;
   float4 o0 = make_float4(0.f, 0.f, 0.f, 0.f), o1 = o0;
   int g = 0;
   if (live) {
@@ -136,6 +140,18 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
         Fnv f; f.init(0u); f.byte('J');
         atomicAdd(a.fp + (h - a.fp_base), f.v);
       }
+    } else if (a.compact) {
+      // P4 entry: a particle that starts outside the grid is moved to its entry point (+ eps); a miss ends here
+      int vi, vj, vk;
+      if (!locate(a.g, o0.x, o0.y, o0.z, vi, vj, vk) && !enter(a.g, o0.x, o0.y, o0.z, o1.x, o1.y, o1.z, vi, vj, vk)) {
+        missed = true; pass = false; q_esc = q_inc;
+        if (a.fp) {
+          Fnv f; f.init(0u);
+          if (m.particle_type[stype]) f.u32(0u);           // an electron track records its (zero) step count first
+          f.byte('M');
+          atomicAdd(a.fp + (h - a.fp_base), f.v);
+        }
+      }
     }
   }
   if (a.compact) {
@@ -155,14 +171,16 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
   }
   // ledgers: incident and jaw-rejected energy, block-reduced, spread over slots
   if (a.ctl) {
-    q_inc = warp_sum_u64(q_inc); q_jaw = warp_sum_u64(q_jaw);
-    if (lane == 0) { s_led[threadIdx.x >> 5][0] = q_inc; s_led[threadIdx.x >> 5][1] = q_jaw; }
+    q_inc = warp_sum_u64(q_inc); q_jaw = warp_sum_u64(q_jaw); q_esc = warp_sum_u64(q_esc);
+    const unsigned nmiss = __popc(__ballot_sync(kFull, missed));
+    if (lane == 0) { s_led[threadIdx.x >> 5][0] = q_inc; s_led[threadIdx.x >> 5][1] = q_jaw; s_led[threadIdx.x >> 5][2] = q_esc; s_miss[threadIdx.x >> 5] = nmiss; }
     __syncthreads();
     if (threadIdx.x == 0) {
-      unsigned long long si = 0, sj = 0;
-      for (int w = 0; w < kThreads / 32; ++w) { si += s_led[w][0]; sj += s_led[w][1]; }
+      unsigned long long si = 0, sj = 0, se = 0; unsigned nm = 0;
+      for (int w = 0; w < kThreads / 32; ++w) { si += s_led[w][0]; sj += s_led[w][1]; se += s_led[w][2]; nm += s_miss[w]; }
       unsigned long long (*L)[2] = a.ctl->ledger[blockIdx.x % kLedgerSlots];
-      add128(L[0], si); add128(L[3], sj);
+      add128(L[0], si); add128(L[3], sj); add128(L[2], se);
+      if (nm) { atomicAdd(&a.ctl->n_missed, (unsigned long long)nm); if (a.stats) atomicAdd(&a.ctl->stat[ST_MISSED], (unsigned long long)nm); }
     }
   }
 }

@@ -224,7 +224,11 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
         if (DBG) fnv.init(t.track);
         if (a.src_kind == SRC_BUFFER && a.buffer_is_debug) tl.inc += (unsigned long long)quanta(E);
         int vi, vj, vk;
-        if (!locate(g, x, y, z, vi, vj, vk) && !enter(g, x, y, z, u, v, w, vi, vj, vk)) {
+        // only the debug buffer holds tracks outside the grid: k_sample already moved the primaries to
+        // their entry points, and queued secondaries are born inside
+        bool in = locate(g, x, y, z, vi, vj, vk);
+        if (!in && a.buffer_is_debug) in = enter(g, x, y, z, u, v, w, vi, vj, vk);
+        if (!in) {
           tl.esc += (unsigned long long)quanta(E);
           if (DBG) { fnv.byte('M'); ++tl.st[ST_MISSED]; finish_track<DBG>(a, h, fnv); }
         } else { cvox = vox_index(g, vi, vj, vk); state = PH_FLIGHT; }
@@ -260,7 +264,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
         } else {
           cvox = vox_index(g, vi, vj, vk);
           const float rho = __ldg(g.density + cvox); const int mt = __ldg(g.material + cvox);
-          const float inv_e3 = 1.0f / (E * E * E);
+          const float inv_e3 = rcp_fast(E * E * E);
           const float muC = rho * (c_mat.ne[mt] * skn), muT = rho * (c_mat.cphoto[mt] * inv_e3), muK = rho * (c_mat.ppair[mt] * lp2);
           const float tt = u_co(d1) * mu_max;
           if (tt < muC) {                                // Compton: Kahn trials are event 2
@@ -288,17 +292,17 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
         // Kahn's rejection (P5).  With dn = 1 + 2 alpha r2:  branch A: eta = dn, branch B:
         // eta = (2 alpha + 1)/dn.  k = (eta - 1)/alpha is 2 r2 (A) or 2 (1 - r2)/dn (B) in exact
         // arithmetic; these forms have no cancellation in fp32.
-        const float alpha = E / kMe, ta = 2.0f * alpha, tp1 = ta + 1.0f;
+        const float ta = E * (2.0f / kMe), tp1 = ta + 1.0f;           // 2 alpha
         const float r1 = u_co(d0), r2 = u_co(d1), r3 = u_co(d2);
-        const float dn = __fmaf_rn(ta, r2, 1.0f), idn = 1.0f / dn;
-        const bool brA = r1 <= tp1 / (ta + 9.0f);
-        const float ie = brA ? idn : dn / tp1;                          // 1/eta
+        const float dn = __fmaf_rn(ta, r2, 1.0f), idn = rcp_fast(dn);
+        const bool brA = r1 <= __fdividef(tp1, ta + 9.0f);
+        const float ie = brA ? idn : __fdividef(dn, tp1);               // 1/eta
         const float k = brA ? 2.0f * r2 : 2.0f * (1.0f - r2) * idn;     // 1 - cos(theta)
         const float ct = 1.0f - k;
         const bool accept = brA ? (r3 <= 4.0f * (ie - ie * ie)) : (r3 <= 0.5f * (ct * ct + ie));
         if (accept) {
           rng.consume(4u, g0, g1, g2, g3);
-          const float sn = sqrtf(fmaxf(0.0f, k * (2.0f - k)));
+          const float sn = sqrt_fast(fmaxf(0.0f, k * (2.0f - k)));
           const float Ep = E * ie, T = E - Ep, u0 = u, v0 = v, w0 = w;
           rotate(u, v, w, ct, sn, u_co(d3));
           if (T >= kEcut && !a.electrons_local) {
@@ -381,7 +385,9 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
         if (DBG) { fnv.init(t.track); ++tl.st[ST_ETRACKS]; }
         if (a.src_kind == SRC_BUFFER && a.buffer_is_debug) tl.inc += (unsigned long long)quanta(T);
         active = true;
-        if (!locate(g, x, y, z, vi, vj, vk) && !enter(g, x, y, z, u, v, w, vi, vj, vk)) {
+        bool in = locate(g, x, y, z, vi, vj, vk);
+        if (!in && a.buffer_is_debug) in = enter(g, x, y, z, u, v, w, vi, vj, vk);
+        if (!in) {
           tl.esc += (unsigned long long)quanta(T);
           if (DBG) { fnv.u32(0u); fnv.byte('M'); ++tl.st[ST_MISSED]; finish_track<DBG>(a, h, fnv); }
           active = false;
@@ -430,8 +436,8 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
           rng.consume(2u, g0, g1, g2, g3);
           // theta = (13.6 / p beta) sqrt(tacc) sqrt(-2 ln a), p beta = Tms (Tms + 2 me)/(Tms + me): one division, one root
           const float c = __fdividef(13.6f * (Tms + kMe), Tms * (Tms + 2.0f * kMe));
-          const float th = fminf(kPi, c * sqrt_fast(tacc * (-2.0f * logf(u_oc(d0)))));
-          float st, ct; sincosf(th, &st, &ct);
+          const float th = fminf(kPi, c * sqrt_fast(tacc * (-2.0f * __logf(u_oc(d0)))));
+          float st, ct; __sincosf(th, &st, &ct);               // th in [0, pi]: SFU path, abs error ~4e-7
           rotate(u, v, w, ct, st, u_co(d1));
           iu = rcp_fast(u); iv = rcp_fast(v); iw = rcp_fast(w);
           fresh = true;
