@@ -149,7 +149,7 @@ __device__ __forceinline__ bool enter(const Grid &g, float &x, float &y, float &
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     if (d[a] == 0.0f) { if (p[a] < lo[a] || p[a] >= hi[a]) return false; continue; }
-    float t1 = (lo[a] - p[a]) / d[a], t2 = (hi[a] - p[a]) / d[a];
+    float t1 = (lo[a] - p[a]) / d[a], t2 = (hi[a] - p[a]) / d[a];      // IEEE division: the entry point seeds every later voxel decision
     tmin = fmaxf(tmin, fminf(t1, t2)); tmax = fminf(tmax, fmaxf(t1, t2));
   }
   if (tmin > tmax || tmax <= 0.0f) return false;
@@ -245,6 +245,13 @@ __device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v)
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return v;
+}
+// Warp sum of energy quanta known to be < 2^44 each (E < 4096 MeV): two hardware integer reductions
+// on the low 22 and the high 22 bits (exact).
+__device__ __forceinline__ unsigned long long warp_sum_q(unsigned long long v) {
+  const unsigned lo = __reduce_add_sync(0xffffffffu, (unsigned)v & 0x3fffffu);
+  const unsigned hi = __reduce_add_sync(0xffffffffu, (unsigned)(v >> 22));
+  return ((unsigned long long)hi << 22) + lo;
 }
 // 128-bit unsigned accumulate into (lo, hi) words in global memory.
 __device__ __forceinline__ void add128(unsigned long long *lohi, unsigned long long q) {

@@ -85,6 +85,10 @@ int upload_tables(psl *P) {
   return MC_OK;
 }
 
+static void round_keys(uint64_t seed, uint32_t ks[20]) {
+  for (int r = 0; r < 10; ++r) { ks[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; ks[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u; }
+}
+
 static SourceModel source_model(const psl &P) {
   SourceModel m{};
   m.table = (const AliasEntry *)P.d_table; m.let_off = P.d_let_off; m.n_let = P.d_n_let;
@@ -165,7 +169,7 @@ struct Run {
   TransportArgs base_args() const {
     TransportArgs a{};
     a.g = g; a.ctl = ctl; a.seed = seed; a.n_total = n_total; a.perm_a = perm_a;
-    for (int r = 0; r < 10; ++r) { a.ks[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; a.ks[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u; }
+    round_keys(seed, a.ks);
     a.p0 = (const float4 *)(ws + L.p0); a.p1 = (const float4 *)(ws + L.p1);
     a.eq = queue(L.eq, &ctl->n_eq, L.eq_cap); a.pq = queue(L.pq, &ctl->n_pq, L.pq_cap);
     a.fp = fp; a.fp_base = fp_base;
@@ -305,7 +309,7 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
   r.tm.end(MC_K_AUX); ++r.launches[MC_K_AUX];
 
   SampleArgs sa{};
-  sa.m = source_model(*P); sa.beam = beam_xf(*beam); sa.off_g = d_off; sa.seed = seed; sa.n_total = N; sa.perm_a = r.perm_a;
+  sa.m = source_model(*P); sa.beam = beam_xf(*beam); sa.off_g = d_off; sa.seed = seed; round_keys(seed, sa.ks); sa.n_total = N; sa.perm_a = r.perm_a;
   sa.p0 = (float4 *)(r.ws + L.p0); sa.p1 = (float4 *)(r.ws + L.p1); sa.ctl = r.ctl; sa.fp = r.fp; sa.fp_base = hb; sa.compact = 1; sa.g = r.g; sa.stats = r.dbg ? 1 : 0;
 
   memset(&g_stats, 0, sizeof g_stats);
@@ -418,7 +422,7 @@ extern "C" int mc_sample_debug(const psl_t *P, const beam_geom_t *beam, uint64_t
   CUDA_TRY(cudaMemcpyAsync(d_off, off.data(), sizeof(uint64_t) * off.size(), cudaMemcpyHostToDevice, st));
   SampleArgs sa{};
   sa.m = source_model(*P); sa.beam = beam_xf(*beam); sa.off_g = (const unsigned long long *)d_off;
-  sa.seed = seed; sa.first = first_history; sa.n_total = n_histories; sa.perm_a = 0; sa.count = (unsigned)count;
+  sa.seed = seed; round_keys(seed, sa.ks); sa.first = first_history; sa.n_total = n_histories; sa.perm_a = 0; sa.count = (unsigned)count;
   sa.p0 = (float4 *)soa_out; sa.p1 = (float4 *)soa_out + count; sa.ctl = nullptr; sa.fp = nullptr; sa.compact = 0;
   k_sample<<<(unsigned)((count + kThreads - 1) / kThreads), kThreads, 0, st>>>(sa);
   CUDA_TRY(cudaGetLastError());

@@ -58,6 +58,7 @@ struct SampleArgs {
   SourceModel m;
   BeamXf beam;
   const unsigned long long *off_g;   // [G+1] device
+  uint32_t ks[20];                   // Philox round keys of `seed` (host-computed)
   unsigned long long seed, first, n_total, perm_a;   // perm_a != 0 → mixed order: h = (perm_a * t) mod n_total
   unsigned count;
   float4 *p0, *p1;                   // outputs (two float4 planes)
@@ -79,7 +80,17 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
   __shared__ unsigned long long s_led[kThreads / 32][3];
   __shared__ unsigned s_miss[kThreads / 32];
   const SourceModel &m = a.m;
+  __shared__ int s_g0;
   for (int i = threadIdx.x; i <= m.n_groups; i += kThreads) s_off[i] = a.off_g[i];
+  // group of h: last g with off[g] <= h (empty groups have off[g] == off[g+1] and are skipped by "last").
+  // Sorted order: history ids of a block are consecutive, so one thread searches for the block's first
+  // history and the others walk forward from there (usually zero steps).
+  if (threadIdx.x == kThreads - 1 && a.perm_a == 0) {            // (reads the global copy: no barrier before this)
+    const unsigned long long hb = a.first + (unsigned long long)blockIdx.x * kThreads;
+    int lo = 0, hi = m.n_groups;
+    while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (a.off_g[mid] <= hb) lo = mid; else hi = mid; }
+    s_g0 = lo;
+  }
   __syncthreads();
   const unsigned t = blockIdx.x * kThreads + threadIdx.x;
   const unsigned lane = threadIdx.x & 31u;
@@ -87,17 +98,23 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
   unsigned long long q_inc = 0, q_jaw = 0, q_esc = 0;
   bool pass = false, missed = false;
   float4 o0 = make_float4(0.f, 0.f, 0.f, 0.f), o1 = o0;
-  int g = 0;
+  int g = 0, ptype = 0;
   if (live) {
     const unsigned long long h = history_of(a.first + t, a.perm_a, a.n_total);
-    // group of h: last g with off[g] <= h (empty groups have off[g] == off[g+1] and are skipped by "last")
-    int lo = 0, hi = m.n_groups;           // invariant: off[lo] <= h < off[hi]
-    while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (s_off[mid] <= h) lo = mid; else hi = mid; }
-    g = lo;
-    const int stype = g / m.n_ebin, ebin = g - stype * m.n_ebin;
-    Philox rng; rng.init(a.seed, h, 0u, 0u);
-    const uint32_t x0 = rng.next(), x1 = rng.next(), x2 = rng.next(), x3 = rng.next();
-    const uint32_t y0 = rng.next(), y1 = rng.next();
+    if (a.perm_a == 0) {
+      g = s_g0;
+      while (g + 1 < m.n_groups && s_off[g + 1] <= h) ++g;
+    } else {
+      int lo = 0, hi = m.n_groups;         // invariant: off[lo] <= h < off[hi]
+      while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (s_off[mid] <= h) lo = mid; else hi = mid; }
+      g = lo;
+    }
+    const int stype = (g >= m.n_ebin) + (g >= 2 * m.n_ebin), ebin = g - stype * m.n_ebin;     // three sub-sources
+    ptype = m.particle_type[stype];
+    RngWin rng; rng.init(h, 0u, 0u);
+    uint32_t x0, x1, x2, x3, y0, y1, y2, y3;
+    rng.gen(a.ks, 0u, x0, x1, x2, x3);
+    rng.gen(a.ks, 1u, y0, y1, y2, y3);
     // 1. let through the alias table
     const unsigned long long mm = (unsigned long long)x0 * m.n_let[g];
     const uint32_t col = (uint32_t)(mm >> 32), frac = (uint32_t)mm;
@@ -113,8 +130,10 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
     // 3. energy uniform in the bin
     const float E = (m.e_min + (float)ebin * m.e_bin_width) + u_oc(x3) * m.e_bin_width;
     // 4. source point on the sub-source's Gaussian (Eq. 4)
-    const float rho = m.sigma_src[stype] * sqrtf(-2.0f * logf(u_oc(y0)));
-    sincospif(2.0f * u_co(y1), &sn, &cs);
+    // (SFU log / root / trig here: the source point only tilts the direction by rho / (z_p - z_s))
+    const float rho = m.sigma_src[stype] * sqrt_fast(-2.0f * __logf(u_oc(y0)));
+    __sincosf(__fmaf_rn(6.283185307f, u_co(y1), -3.141592654f), &sn, &cs); sn = -sn; cs = -cs;
+    (void)y2; (void)y3;
     const float qx = rho * cs, qy = rho * sn, qz = m.z_src[stype];
     // 5. direction (Eq. 5)
     float dx = px - qx, dy = py - qy, dz = pz - qz;
@@ -126,13 +145,13 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
     // 7. beam set-up
     const float *R = a.beam.R;
     const float bz = pz - a.beam.sad;
-    o0.x = a.beam.iso[0] + R[0] * px + R[1] * py + R[2] * bz;
-    o0.y = a.beam.iso[1] + R[3] * px + R[4] * py + R[5] * bz;
-    o0.z = a.beam.iso[2] + R[6] * px + R[7] * py + R[8] * bz;
+    o0.x = __fmaf_rn(R[0], px, __fmaf_rn(R[1], py, __fmaf_rn(R[2], bz, a.beam.iso[0])));
+    o0.y = __fmaf_rn(R[3], px, __fmaf_rn(R[4], py, __fmaf_rn(R[5], bz, a.beam.iso[1])));
+    o0.z = __fmaf_rn(R[6], px, __fmaf_rn(R[7], py, __fmaf_rn(R[8], bz, a.beam.iso[2])));
     o0.w = E;
-    o1.x = R[0] * dx + R[1] * dy + R[2] * dz;
-    o1.y = R[3] * dx + R[4] * dy + R[5] * dz;
-    o1.z = R[6] * dx + R[7] * dy + R[8] * dz;
+    o1.x = __fmaf_rn(R[0], dx, __fmaf_rn(R[1], dy, R[2] * dz));
+    o1.y = __fmaf_rn(R[3], dx, __fmaf_rn(R[4], dy, R[5] * dz));
+    o1.z = __fmaf_rn(R[6], dx, __fmaf_rn(R[7], dy, R[8] * dz));
     q_inc = (unsigned long long)quanta(E);
     if (!pass) {
       q_jaw = q_inc;
@@ -147,7 +166,7 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
         missed = true; pass = false; q_esc = q_inc;
         if (a.fp) {
           Fnv f; f.init(0u);
-          if (m.particle_type[stype]) f.u32(0u);           // an electron track records its (zero) step count first
+          if (ptype) f.u32(0u);           // an electron track records its (zero) step count first
           f.byte('M');
           atomicAdd(a.fp + (h - a.fp_base), f.v);
         }
@@ -162,7 +181,7 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
     base = __shfl_sync(kFull, base, 0);
     if (live && pass) {
       const unsigned dst = base + __popc(keep & ((1u << lane) - 1u));
-      o1.w = __uint_as_float(t | ((unsigned)m.particle_type[g / m.n_ebin] << 31));
+      o1.w = __uint_as_float(t | ((unsigned)ptype << 31));
       a.p0[dst] = o0; a.p1[dst] = o1;
     }
   } else if (live) {
@@ -171,7 +190,7 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
   }
   // ledgers: incident and jaw-rejected energy, block-reduced, spread over slots
   if (a.ctl) {
-    q_inc = warp_sum_u64(q_inc); q_jaw = warp_sum_u64(q_jaw); q_esc = warp_sum_u64(q_esc);
+    q_inc = warp_sum_q(q_inc); q_jaw = warp_sum_q(q_jaw); q_esc = warp_sum_q(q_esc);
     const unsigned nmiss = __popc(__ballot_sync(kFull, missed));
     if (lane == 0) { s_led[threadIdx.x >> 5][0] = q_inc; s_led[threadIdx.x >> 5][1] = q_jaw; s_led[threadIdx.x >> 5][2] = q_esc; s_miss[threadIdx.x >> 5] = nmiss; }
     __syncthreads();
