@@ -45,7 +45,7 @@ static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 // (2 planes), the electron queue (capacity 4B) and the photon queue (capacity B), each 3 planes,
 // then (optionally) the int64 dose grid.
 struct Layout {
-  size_t ctl, off, xs, p0, p1, eq[3], pq[3], acc, total;
+  size_t ctl, off, xs, p0, p1, eq[3], pq[2][3], acc, total;
   unsigned eq_cap, pq_cap;
 };
 static Layout make_layout(uint64_t batch, size_t nvox, bool with_acc) {
@@ -55,7 +55,7 @@ static Layout make_layout(uint64_t batch, size_t nvox, bool with_acc) {
   L.ctl = take(sizeof(Control)); L.off = take(sizeof(uint64_t) * 160); L.xs = take(kXsBytes);
   L.p0 = take(16 * batch); L.p1 = take(16 * batch);
   for (int k = 0; k < 3; ++k) L.eq[k] = take((size_t)16 * L.eq_cap);
-  for (int k = 0; k < 3; ++k) L.pq[k] = take((size_t)16 * L.pq_cap);
+  for (int b = 0; b < 2; ++b) for (int k = 0; k < 3; ++k) L.pq[b][k] = take((size_t)16 * L.pq_cap);
   L.acc = take(with_acc ? 8 * nvox : 0);
   L.total = o;
   return L;
@@ -171,7 +171,7 @@ struct Run {
     a.g = g; a.ctl = ctl; a.seed = seed; a.n_total = n_total; a.perm_a = perm_a;
     round_keys(seed, a.ks);
     a.p0 = (const float4 *)(ws + L.p0); a.p1 = (const float4 *)(ws + L.p1);
-    a.eq = queue(L.eq, &ctl->n_eq, L.eq_cap); a.pq = queue(L.pq, &ctl->n_pq, L.pq_cap);
+    a.eq = queue(L.eq, &ctl->n_eq, L.eq_cap); a.pq = queue(L.pq[pq_fill], &ctl->n_pq, L.pq_cap);
     a.fp = fp; a.fp_base = fp_base;
     a.electrons_local = (flags & MC_FLAG_ELECTRONS_LOCAL) ? 1 : 0;
     a.static_lanes = (flags & MC_FLAG_STATIC_LANES) ? 1 : 0;
@@ -206,17 +206,46 @@ struct Run {
     blocks_photon[0] = persistent_blocks(k_photon<false>, kXsSmem); blocks_photon[1] = persistent_blocks(k_photon<true>, kXsSmem);
     blocks_electron[0] = persistent_blocks(k_electron<false>); blocks_electron[1] = persistent_blocks(k_electron<true>);
   }
-  // photons of the particle buffer, then annihilation photons, then every queued electron
-  void transport_photon_batch(uint64_t first, bool debug_buffer, const unsigned *count_ptr) {
+  // Folds the finished batch's counters, resets them, and swaps the photon queues (n_pq -> n_pq_prev).
+  void next_batch() {
+    tm.begin(MC_K_AUX); k_next_batch<<<1, 1, 0, st>>>(ctl); tm.end(MC_K_AUX); ++launches[MC_K_AUX];
+    pq_fill ^= 1;
+  }
+  const float4 *dbg_p0 = nullptr, *dbg_p1 = nullptr;
+  int pq_fill = 0; bool pq_pending = false;     // photon queues ping-pong: batch i fills pq[i & 1] and consumes pq[(i - 1) & 1]
+  // mc_transport_debug: photons of the caller's buffer, then their annihilation photons, then every queued electron
+  void transport_photon_debug(uint64_t first, const unsigned *count_ptr) {
     TransportArgs a = base_args();
-    a.src_kind = SRC_BUFFER; a.buffer_is_debug = debug_buffer; a.first = first; a.want_type = 0;
-    a.src_count = count_ptr; a.src_head = &ctl->head_pb;
+    a.src_kind = SRC_BUFFER; a.buffer_is_debug = 1; a.first = first; a.want_type = 0;
+    a.src_count = count_ptr; a.src_head = &ctl->head_pb; a.p0 = dbg_p0; a.p1 = dbg_p1;
     photon(a);
     TransportArgs b = base_args();
     b.src_kind = SRC_QUEUE; b.src = b.pq; b.src_count = &ctl->n_pq; b.src_head = &ctl->head_pq;
     b.pq.cap = 0;                              // 0.511 MeV photons cannot pair-produce; a push would flag overflow
     photon(b);
     drain_electrons();
+  }
+  // mc_dose: call right after k_next_batch + k_sample.  The photons of the particle buffer and the
+  // annihilation photons the PREVIOUS batch left in the other photon queue go through one launch
+  // (a launch over a few hundred 0.511 MeV photons alone costs the latency of its longest history).
+  void transport_photon_batch(uint64_t first) {
+    TransportArgs a = base_args();
+    a.src_kind = SRC_BUFFER; a.buffer_is_debug = 0; a.first = first; a.want_type = 0;
+    a.src_count = &ctl->n_pb; a.src_head = &ctl->head_pb;
+    a.src = queue(L.pq[pq_fill ^ 1], &ctl->n_pq_prev, L.pq_cap); a.src2_count = &ctl->n_pq_prev;
+    photon(a);
+    pq_pending = true;
+    drain_electrons();
+  }
+  // Annihilation photons still queued after the last photon batch (call after a k_next_batch).
+  void drain_photon_queue() {
+    if (!pq_pending) return;
+    TransportArgs b = base_args();
+    b.src_kind = SRC_QUEUE; b.src = queue(L.pq[pq_fill ^ 1], &ctl->n_pq_prev, L.pq_cap); b.src_count = &ctl->n_pq_prev; b.src_head = &ctl->head_pq;
+    b.pq.cap = 0;
+    photon(b);
+    drain_electrons();
+    pq_pending = false;
   }
   void drain_electrons() {
     TransportArgs c = base_args();
@@ -314,7 +343,7 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
 
   memset(&g_stats, 0, sizeof g_stats);
   auto sample_batch = [&](uint64_t first, uint64_t count) {
-    r.tm.begin(MC_K_AUX); k_next_batch<<<1, 1, 0, r.st>>>(r.ctl); r.tm.end(MC_K_AUX); ++r.launches[MC_K_AUX];
+    r.next_batch();
     sa.first = first; sa.count = (unsigned)count;
     r.tm.begin(MC_K_SAMPLE);
     k_sample<<<(unsigned)((count + kThreads - 1) / kThreads), kThreads, 0, r.st>>>(sa);
@@ -327,9 +356,10 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
       const uint64_t lo = std::max(hb, off[(size_t)s * ne]), hi = std::min(he, off[(size_t)(s + 1) * ne]);
       if (lo >= hi) continue;
       g_stats.n_hist[s] = hi - lo;
+      if (P->psr.particle_type[s] != 0 && r.pq_pending) { r.next_batch(); r.drain_photon_queue(); }   // no photon launch ahead to carry them
       for (uint64_t first = lo; first < hi; first += batch) {
         sample_batch(first, std::min(batch, hi - first));
-        if (P->psr.particle_type[s] == 0) r.transport_photon_batch(first, false, &r.ctl->n_pb);
+        if (P->psr.particle_type[s] == 0) r.transport_photon_batch(first);
         else r.transport_electron_buffer(first, false, &r.ctl->n_pb, &r.ctl->head_pb);
       }
     }
@@ -338,11 +368,12 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
     for (uint64_t first = hb; first < he; first += batch) {
       sample_batch(first, std::min(batch, he - first));
       r.transport_electron_buffer(first, false, &r.ctl->n_pb, &r.ctl->pad0);
-      r.transport_photon_batch(first, false, &r.ctl->n_pb);
+      r.transport_photon_batch(first);
     }
     if (hb == 0 && he == N) for (int s = 0; s < 3; ++s) g_stats.n_hist[s] = off[(size_t)(s + 1) * ne] - off[(size_t)s * ne];
   }
-  k_next_batch<<<1, 1, 0, r.st>>>(r.ctl); ++r.launches[MC_K_AUX];
+  r.next_batch();
+  if (r.pq_pending) { r.drain_photon_queue(); r.next_batch(); }
   if (dose_out) {
     r.tm.begin(MC_K_FINALISE);
     const double inv_vn = 1.0 / (ph->dx * ph->dy * ph->dz * (double)N);
@@ -462,11 +493,8 @@ extern "C" int mc_transport_debug(const phantom_t *ph, int32_t particle_type, co
   a.src_kind = SRC_BUFFER; a.buffer_is_debug = 1; a.first = first_history; a.want_type = particle_type;
   a.src_count = &r.ctl->n_pb; a.src_head = &r.ctl->head_pb;
   if (particle_type == 0) {
-    r.photon(a);
-    TransportArgs b = r.base_args();
-    b.src_kind = SRC_QUEUE; b.src = b.pq; b.src_count = &r.ctl->n_pq; b.src_head = &r.ctl->head_pq; b.pq.cap = 0;
-    r.photon(b);
-    r.drain_electrons();
+    r.dbg_p0 = (const float4 *)soa_in; r.dbg_p1 = (const float4 *)soa_in + count;
+    r.transport_photon_debug(first_history, &r.ctl->n_pb);
   } else {
     r.electron(a);
   }

@@ -20,7 +20,8 @@ struct Control {
   unsigned n_pb, head_pb;          // particle buffer: entries written by k_sample, consume cursor
   unsigned n_eq, head_eq;          // electron queue
   unsigned n_pq, head_pq;          // photon queue (annihilation photons)
-  unsigned pad0, pad1;
+  unsigned pad0;                   // (mixed order: consume cursor of the electron pass over the particle buffer)
+  unsigned n_pq_prev;              // annihilation photons of the PREVIOUS batch, consumed by this batch's photon launch
   // per call
   unsigned overflow;               // a queue was full: result invalid → MC_E_OVERFLOW
   unsigned hw_eq, hw_pq;           // queue high-water marks
@@ -209,7 +210,8 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
 __global__ void k_next_batch(Control *c) {
   c->n_accepted += c->n_pb;
   c->hw_eq = max(c->hw_eq, c->n_eq); c->hw_pq = max(c->hw_pq, c->n_pq);
-  c->n_pb = c->head_pb = c->n_eq = c->head_eq = c->n_pq = c->head_pq = c->pad0 = c->pad1 = 0;
+  c->n_pq_prev = c->n_pq;           // the photon queues ping-pong: last batch's annihilation photons ride with the next photon launch
+  c->n_pb = c->head_pb = c->n_eq = c->head_eq = c->n_pq = c->head_pq = c->pad0 = 0;
 }
 
 // Largest density per material (Woodcock majorant input).  Densities are >= 0, so float order = uint order.

@@ -39,6 +39,7 @@ struct TransportArgs {
   const float4 *p0, *p1;
   Queue src;
   const unsigned *src_count;          // entries available (device)
+  const unsigned *src2_count;         // SRC_BUFFER only, or null: `src` holds this many extra tracks, consumed after the buffer
   unsigned *src_head;                 // consume cursor (device)
   unsigned long long first, n_total, perm_a;
   // sinks
@@ -163,9 +164,9 @@ __device__ __forceinline__ unsigned refill_index(const TransportArgs &a, bool id
 
 struct TrackIn { float x, y, z, u, v, w, E; unsigned long long h; uint32_t track, ndraw; bool ok; };
 
-__device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned idx) {
+__device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned idx, unsigned n1) {
   TrackIn t;
-  if (a.src_kind == SRC_BUFFER) {
+  if (a.src_kind == SRC_BUFFER && idx < n1) {
     const float4 A = a.p0[idx], B = a.p1[idx];
     t.x = A.x; t.y = A.y; t.z = A.z; t.E = A.w; t.u = B.x; t.v = B.y; t.w = B.z;
     unsigned long long tt;
@@ -174,6 +175,7 @@ __device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned i
     t.h = history_of(a.first + tt, a.perm_a, a.n_total);
     t.track = 0u; t.ndraw = 8u;
   } else {
+    if (a.src_kind == SRC_BUFFER) idx -= n1;
     const float4 A = a.src.a[idx], B = a.src.b[idx]; const uint4 C = a.src.c[idx];
     t.x = A.x; t.y = A.y; t.z = A.z; t.E = A.w; t.u = B.x; t.v = B.y; t.w = B.z;
     t.h = ((unsigned long long)C.y << 32) | C.x; t.track = C.z; t.ndraw = 0u; t.ok = true;
@@ -199,7 +201,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
   for (int i = threadIdx.x; i <= a.xs.n; i += kThreads) s_xs[i] = a.xs.nodes[i];
   __syncthreads();
   const Grid &g = a.g;
-  const unsigned count = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
+  const unsigned n1 = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
+  const unsigned count = n1 + ((a.src_kind == SRC_BUFFER && a.src2_count) ? min(*a.src2_count, a.src.cap) : 0u);
   SrcCursor sc; sc.next = sc.end = 0u;
   StageRing &ring = *reinterpret_cast<StageRing *>(s_raw + kXsBytes + sizeof(StageRing) * (threadIdx.x >> 5));
   StageCursor stg; stg.head = stg.n = 0u;
@@ -217,12 +220,12 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
     // ---- refill idle lanes
     const unsigned idx = refill_index<1, 128u>(a, state == PH_IDLE, count, sc, exhausted);
     if (idx != 0xffffffffu) {
-      const TrackIn t = load_track(a, idx);
+      const TrackIn t = load_track(a, idx, n1);
       if (t.ok) {
         x = t.x; y = t.y; z = t.z; u = t.u; v = t.v; w = t.w; E = t.E; h = t.h; nchild = 0; collided = false;
         rng.init(h, t.track, t.ndraw);
         if (DBG) fnv.init(t.track);
-        if (a.src_kind == SRC_BUFFER && a.buffer_is_debug) tl.inc += (unsigned long long)quanta(E);
+        if (a.buffer_is_debug) tl.inc += (unsigned long long)quanta(E);
         int vi, vj, vk;
         // only the debug buffer holds tracks outside the grid: k_sample already moved the primaries to
         // their entry points, and queued secondaries are born inside
@@ -359,7 +362,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
 template <bool DBG>
 __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant__ TransportArgs a) {
   const Grid &g = a.g;
-  const unsigned count = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
+  const unsigned n1 = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
+  const unsigned count = n1 + ((a.src_kind == SRC_BUFFER && a.src2_count) ? min(*a.src2_count, a.src.cap) : 0u);
   SrcCursor sc; sc.next = sc.end = 0u;
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
@@ -377,13 +381,13 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
   for (;;) {
     const unsigned idx = refill_index<kElectronRefillMin, kElectronChunk>(a, !active, count, sc, exhausted);
     if (idx != 0xffffffffu) {
-      const TrackIn t = load_track(a, idx);
+      const TrackIn t = load_track(a, idx, n1);
       if (t.ok) {
         float x = t.x, y = t.y, z = t.z;
         u = t.u; v = t.v; w = t.w; T = t.E; h = t.h; steps = 0; fresh = true;
         rng.init(h, t.track, t.ndraw);
         if (DBG) { fnv.init(t.track); ++tl.st[ST_ETRACKS]; }
-        if (a.src_kind == SRC_BUFFER && a.buffer_is_debug) tl.inc += (unsigned long long)quanta(T);
+        if (a.buffer_is_debug) tl.inc += (unsigned long long)quanta(T);
         active = true;
         bool in = locate(g, x, y, z, vi, vj, vk);
         if (!in && a.buffer_is_debug) in = enter(g, x, y, z, u, v, w, vi, vj, vk);
