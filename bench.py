@@ -75,7 +75,7 @@ def run_reference(args):
     oracle.build()
     cfg = workloads.make_config(args.config)
     n_total = args.histories or cfg["n_histories"]
-    n_sample = min(n_total, 2_000_000)
+    n_sample = min(n_total, 4_000_000)
     for _ in range(args.warmup):
         time_oracle(cfg, n_total, min(n_sample, 100_000))
     rates, ms = [], []
@@ -137,7 +137,10 @@ class ClockSampler:
 # Algorithmic work per history of the bench workload, stated in DESIGN.md §Roofline and measured once
 # with ncu (profiles/): SASS thread-instructions the transport kernels retire per C1 primary history,
 # and the bytes k_sample must write per history (32 B per particle that passes the jaws).
-ALG_THREAD_INST_PER_HISTORY = {"C1": {"photon": 1150.0, "electron": 1300.0}}
+ALG_THREAD_INST_PER_HISTORY = {"C1": {"photon": 646.0, "electron": 898.0, "sample": 486.0}}      # profiles/r1b_launches.md
+# DRAM bytes (read + write) per step of each kernel class, from the ncu --set full captures of profiles/r1b_top_kernels.md
+# (the two primary-batch launches; the path's working set is L2-resident, so this is far below any HBM bound)
+NCU_DRAM_BYTES_PER_STEP = {"C1": {"photon": 2.21e8, "electron": 1.42e8, "sample": 4.5e7}}
 SAMPLE_BYTES_PER_PARTICLE = 32.0
 
 
@@ -253,8 +256,11 @@ def run_ours(args):
         peak = ALU_LANES * f_clk / 1e12                  # T thread-instr/s at the SM clock seen under load
         achieved = alg[dom] * hist_rank / (ms_class[dom] * 1e-3) / 1e12
         roof = {"bound": "alu", "kernel": "k_" + dom, "achieved": achieved, "peak": peak, "unit": "Tinst/s (thread)",
-                "frac": achieved / peak, "traffic": None,
+                "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_STEP.get(args.config, {}).get(dom),
                 "peak_source": "148 SM x 128 lanes x SM clock under load (DESIGN.md)", "alg_thread_inst_per_history": alg[dom]}
+    # the three hot kernels together: useful thread-instructions of a step over the lane-issue slots of the whole step
+    f_clk_all = (ck["sm_mhz"] or sm_max) * 1e6 if ck else sm_max * 1e6
+    whole = sum(alg.values()) * hist_rank / (total_ms * 1e-3) / (ALU_LANES * f_clk_all)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -268,13 +274,14 @@ def run_ours(args):
                 "ms_per_step": sum(e2e_ms) / len(e2e_ms)},
         "gpu_launches": launches,
         "roofline": roof,
+        "whole_path_lane_issue_frac": whole,
         "kernel_ms_per_step": {k: v / args.steps for k, v in ms_class.items()},
         "k_sample": {"achieved_GBps": sample_gbs, "frac_of_hbm": sample_gbs / hbm_peak,
                      "histories_per_s": hist_rank / (ms_class["sample"] * 1e-3) if ms_class["sample"] > 0 else None},
         "paper_context": "Table 1 (unstated GPU, OpenCL): 1e9 histories 10x10 water in 69.15 s = 1.45e7 histories/s",
     }
     if not args.no_cpu_baseline and world == 1:
-        v, done, dt = time_oracle(cfg, n_total, min(n_total, 6_000_000))
+        v, done, dt = time_oracle(cfg, n_total, min(n_total, 20_000_000))
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                                "sample": "%d of %d histories in 64 equally spaced id ranges, %.1f s" % (done, n_total, dt)}
     print(json.dumps(out))
