@@ -124,8 +124,10 @@ struct Fnv {
 struct Grid {
   int nx, ny, nz;
   float ox, oy, oz, dx, dy, dz, idx, idy, idz;      // origin, voxel size, reciprocal voxel size
-  const float   *density;
+  const float   *density;                            // caller's arrays (k_pack_phantom, k_finalise)
   const uint8_t *material;
+  const uint32_t *vox;                               // packed phantom, one gather per voxel: density bits rounded to a
+                                                     // 22-bit mantissa | material index in the two low bits
   unsigned long long *acc;                           // int64 fixed-point dose accumulator (2^-32 MeV)
 };
 
@@ -136,6 +138,10 @@ __device__ __forceinline__ bool locate(const Grid &g, float x, float y, float z,
   bool in = fi >= 0.0f && fi < (float)g.nx && fj >= 0.0f && fj < (float)g.ny && fk >= 0.0f && fk < (float)g.nz;
   i = (int)fi; j = (int)fj; k = (int)fk;
   return in;
+}
+__device__ __forceinline__ void fetch_voxel(const Grid &g, int v, float &rho, int &mt) {
+  const uint32_t p = __ldg(g.vox + v);
+  rho = __uint_as_float(p & ~3u); mt = (int)(p & 3u);
 }
 __device__ __forceinline__ int vox_index(const Grid &g, int i, int j, int k) { return (k * g.ny + j) * g.nx + i; }
 

@@ -214,11 +214,15 @@ __global__ void k_next_batch(Control *c) {
   c->n_pb = c->head_pb = c->n_eq = c->head_eq = c->n_pq = c->head_pq = c->pad0 = 0;
 }
 
-// Largest density per material (Woodcock majorant input).  Densities are >= 0, so float order = uint order.
-__global__ void k_rhomax(const float *density, const uint8_t *material, size_t n, Control *c) {
+// Packs the caller's phantom into one 32-bit word per voxel (density rounded to nearest on a 22-bit
+// mantissa, material in the two low bits) and finds the largest PACKED density per material (Woodcock
+// majorant input).  Densities are >= 0, so float order = uint order.
+__global__ void k_pack_phantom(const float *density, const uint8_t *material, size_t n, uint32_t *vox, Control *c) {
   float best[3] = {0.f, 0.f, 0.f};
   for (size_t v = blockIdx.x * (size_t)blockDim.x + threadIdx.x; v < n; v += (size_t)gridDim.x * blockDim.x) {
-    const float d = density[v]; const int mt = material[v];
+    const uint32_t bits = (__float_as_uint(density[v]) + 2u) & ~3u; const int mt = min((int)material[v], 2);
+    vox[v] = bits | (uint32_t)mt;
+    const float d = __uint_as_float(bits);
     if (mt == 0) best[0] = fmaxf(best[0], d); else if (mt == 1) best[1] = fmaxf(best[1], d); else best[2] = fmaxf(best[2], d);
   }
 #pragma unroll

@@ -266,7 +266,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
           done = true;
         } else {
           cvox = vox_index(g, vi, vj, vk);
-          const float rho = __ldg(g.density + cvox); const int mt = __ldg(g.material + cvox);
+          float rho; int mt; fetch_voxel(g, cvox, rho, mt);
           const float inv_e3 = rcp_fast(E * E * E);
           const float muC = rho * (c_mat.ne[mt] * skn), muT = rho * (c_mat.cphoto[mt] * inv_e3), muK = rho * (c_mat.ppair[mt] * lp2);
           const float tt = u_co(d1) * mu_max;
@@ -287,7 +287,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
     }
 
     // ---- event 2: one Kahn trial (+ Compton kinematics when accepted) or the pair split
-    bool push_e = false; float ex = 0, ey = 0, ez = 0, eT = 0; uint32_t etrack = 0;
+    bool push_e = false, push_p = false; float ex = 0, ey = 0, ez = 0, eT = 0; uint32_t etrack = 0;
+    float pairT[2] = {0.f, 0.f};
     if (state >= PH_KAHN) {
       uint32_t d0, d1, d2, d3, g0, g1, g2, g3;
       rng.window<4>(a.ks, d0, d1, d2, d3, g0, g1, g2, g3);
@@ -321,14 +322,14 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
           }
           ++nchild; E = Ep; state = PH_FLIGHT;
         } else rng.consume(3u, g0, g1, g2, g3);
-      } else {                                           // pair production (rare: plain per-lane pushes)
+      } else {                                           // pair production: the pushes happen below, convergently
         rng.consume(3u, g0, g1, g2, g3);
         const float Tsum = E - kEPair, Tm = u_co(d0) * Tsum, Tp = Tsum - Tm;
         const float Tc[2] = {Tm, Tp};
 #pragma unroll
         for (int sl = 0; sl < 2; ++sl) {
           if (Tc[sl] >= kEcut && !a.electrons_local) {
-            queue_push1(a.eq, a.ctl, x, y, z, Tc[sl], u, v, w, h, child_track(rng.track, nchild, sl));
+            pairT[sl] = Tc[sl];
             if (DBG) ++tl.st[ST_SEC_E];
           } else {
             const long long q = quanta(Tc[sl]); pend.add(g, cvox, q); tl.dep += (unsigned long long)q;
@@ -337,16 +338,38 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
         }
         const float cz = 2.0f * u_co(d1) - 1.0f, sz = sqrtf(fmaxf(0.0f, 1.0f - cz * cz));
         float sa, ca; sincospif(2.0f * u_co(d2), &sa, &ca);
-        const float nx = sz * ca, ny = sz * sa;
-        queue_push1(a.pq, a.ctl, x, y, z, kEAnnih, nx, ny, cz, h, child_track(rng.track, nchild, 2u));
-        queue_push1(a.pq, a.ctl, x, y, z, kEAnnih, -nx, -ny, -cz, h, child_track(rng.track, nchild, 3u));
+        ex = sz * ca; ey = sz * sa; ez = cz; push_p = true;
         if (DBG) { tl.st[ST_SEC_P] += 2; finish_track<DBG>(a, h, fnv); }
         state = PH_IDLE;
       }
     }
-    // ---- Compton electrons: warp ballot + prefix sum, one tail atomic per warp
+    // ---- secondaries, convergent: Compton electrons through the staging ring ...
     stage_push(a.eq, a.ctl, ring, stg, push_e, make_float4(x, y, z, eT), make_float4(ex, ey, ez, 0.f),
                make_uint4((uint32_t)h, (uint32_t)(h >> 32), etrack, 0u));
+    // ... and, in the rare iteration with a pair production in the warp, the e-/e+ through the same ring and
+    // the two annihilation photons behind ONE warp-aggregated tail atomic (the lane's x, y, z, u, v, w, h,
+    // nchild are still those of the converting photon: it only refills at the top of the next iteration)
+    const unsigned mp = __ballot_sync(kFull, push_p);
+    if (mp) {
+#pragma unroll
+      for (int sl = 0; sl < 2; ++sl)
+        stage_push(a.eq, a.ctl, ring, stg, pairT[sl] > 0.0f, make_float4(x, y, z, pairT[sl]), make_float4(u, v, w, 0.f),
+                   make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, (uint32_t)sl), 0u));
+      const unsigned lane = threadIdx.x & 31u, leader = __ffs(mp) - 1;
+      unsigned base = 0;
+      if (lane == leader) base = atomicAdd(a.pq.count, 2u * __popc(mp));
+      base = __shfl_sync(kFull, base, leader);
+      if (push_p) {
+        const unsigned slot = base + 2u * __popc(mp & ((1u << lane) - 1u));
+        if (slot + 2u > a.pq.cap) a.ctl->overflow = 1u;
+        else {
+          a.pq.a[slot] = a.pq.a[slot + 1] = make_float4(x, y, z, kEAnnih);
+          a.pq.b[slot] = make_float4(ex, ey, ez, 0.f); a.pq.b[slot + 1] = make_float4(-ex, -ey, -ez, 0.f);
+          a.pq.c[slot] = make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, 2u), 0u);
+          a.pq.c[slot + 1] = make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, 3u), 0u);
+        }
+      }
+    }
   }
   if (stg.n) stage_flush(a.eq, a.ctl, ring, stg, stg.n);
   pend.flush(g);
@@ -405,7 +428,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
 
     if (active) {                                        // one sub-step
       const int vox = vox_index(g, vi, vj, vk);
-      const float rho = __ldg(g.density + vox); const int mt = __ldg(g.material + vox);
+      float rho; int mt; fetch_voxel(g, vox, rho, mt);
       if (fresh) { budget = kFe * T; Tms = T; tacc = 0.0f; fresh = false; }
       const float D = (c_mat.sscale[mt] * rho) * __fmaf_rn(0.078f, T, __fmaf_rn(0.25f, rcp_fast(T), 1.52f));
       const float sE = D > 0.0f ? __fdividef(budget, D) : INFINITY;
