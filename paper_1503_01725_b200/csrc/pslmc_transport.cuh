@@ -92,23 +92,32 @@ __device__ __forceinline__ void finish_track(const TransportArgs &a, unsigned lo
 // takes 32 consecutive queue slots with ONE tail atomic and writes them as three coalesced 512-byte
 // rows.  No atomic and no global store in the common iteration; no holes in the queue.  Convergent calls.
 struct StageRing { float4 a[64], b[64]; uint4 c[64]; };           // 3 KiB per warp
-struct StageCursor { unsigned head, n; };
-__device__ __forceinline__ void stage_flush(const Queue &q, Control *ctl, StageRing &r, StageCursor &sc, unsigned n_out) {
+struct StageCursor { unsigned head, n, base_raw; bool pending; };
+// The flush is split in two so that the tail atomic's latency is not waited for: stage_reserve issues
+// the atomic for 32 slots (result left in lane 0's register), stage_complete - one loop iteration later,
+// or at kernel exit - broadcasts it and writes the 32 oldest ring entries.
+__device__ __forceinline__ void stage_reserve(const Queue &q, StageCursor &sc, unsigned n_out) {
+  if ((threadIdx.x & 31u) == 0) sc.base_raw = atomicAdd(q.count, n_out);
+  sc.pending = true;
+}
+__device__ __forceinline__ void stage_complete(const Queue &q, Control *ctl, StageRing &r, StageCursor &sc, unsigned n_out) {
   const unsigned lane = threadIdx.x & 31u;
   __syncwarp();
-  unsigned base = 0;
-  if (lane == 0) base = atomicAdd(q.count, n_out);
-  base = __shfl_sync(kFull, base, 0);
+  const unsigned base = __shfl_sync(kFull, sc.base_raw, 0);
   if (base + n_out > q.cap) ctl->overflow = 1u;
   else if (lane < n_out) {
     const unsigned p = (sc.head + lane) & 63u;
     q.a[base + lane] = r.a[p]; q.b[base + lane] = r.b[p]; q.c[base + lane] = r.c[p];
   }
-  sc.head = (sc.head + n_out) & 63u; sc.n -= n_out;
+  sc.head = (sc.head + n_out) & 63u; sc.n -= n_out; sc.pending = false;
   __syncwarp();
 }
+// One call per loop iteration (convergent): finishes the flush reserved in the previous iteration, appends
+// this iteration's entries, and reserves the next flush once 32 are staged.  The ring never holds more
+// than 31 + 32 entries.
 __device__ __forceinline__ void stage_push(const Queue &q, Control *ctl, StageRing &r, StageCursor &sc, bool want,
                                            float4 A, float4 B, uint4 C) {
+  if (sc.pending) stage_complete(q, ctl, r, sc, 32u);
   const unsigned m = __ballot_sync(kFull, want);
   if (!m) return;
   const unsigned lane = threadIdx.x & 31u;
@@ -117,17 +126,12 @@ __device__ __forceinline__ void stage_push(const Queue &q, Control *ctl, StageRi
     r.a[p] = A; r.b[p] = B; r.c[p] = C;
   }
   sc.n += __popc(m);
-  if (sc.n >= 32u) stage_flush(q, ctl, r, sc, 32u);
+  if (sc.n >= 32u) stage_reserve(q, sc, 32u);
 }
-// Divergent-context push of one track (rare paths: pair production).
-__device__ __forceinline__ void queue_push1(const Queue &q, Control *ctl, float x, float y, float z, float E,
-                                            float u, float v, float w, unsigned long long h, uint32_t track) {
-  const unsigned slot = atomicAdd(q.count, 1u);
-  if (slot >= q.cap) { ctl->overflow = 1u; return; }
-  q.a[slot] = make_float4(x, y, z, E); q.b[slot] = make_float4(u, v, w, 0.f);
-  q.c[slot] = make_uint4((uint32_t)h, (uint32_t)(h >> 32), track, 0u);
+__device__ __forceinline__ void stage_drain(const Queue &q, Control *ctl, StageRing &r, StageCursor &sc) {
+  if (sc.pending) stage_complete(q, ctl, r, sc, 32u);
+  if (sc.n) { const unsigned n = sc.n; stage_reserve(q, sc, n); stage_complete(q, ctl, r, sc, n); }
 }
-
 // Refill protocol shared by both kernels: lanes without a track take the next source indices.  A warp
 // takes `chunk` consecutive indices from the source cursor with ONE atomic and hands them out over
 // the next refills (warp-uniform cursor in `sc`).  Returns the source index for this lane or
@@ -141,8 +145,19 @@ __device__ __forceinline__ unsigned source_chunk(const TransportArgs &a, unsigne
   const unsigned warps = gridDim.x * (kThreads / 32), left = count - min(count, seen_end);
   return min(MAX_CHUNK, max(need, (left / (warps * 2u)) & ~31u));     // near the end: exactly what the idle lanes need
 }
+// L2 prefetch of the source entries [first, end) a warp has just reserved (<= 128 entries = 16 lines per
+// 16-byte plane): the loads of the following refills then find them on chip.
+__device__ __forceinline__ void prefetch_chunk(const TransportArgs &a, unsigned n1, unsigned first, unsigned end) {
+  const unsigned lane = threadIdx.x & 31u, e = first + (lane & 15u) * 8u;       // 8 entries per 128-byte line
+  if (e >= end) return;
+  const void *p0, *p1, *p2 = nullptr;
+  if (a.src_kind == SRC_BUFFER && e < n1) { p0 = a.p0 + e; p1 = a.p1 + e; }
+  else { const unsigned q = a.src_kind == SRC_BUFFER ? e - n1 : e; p0 = a.src.a + q; p1 = a.src.b + q; p2 = a.src.c + q; }
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(lane < 16u ? p0 : p1));
+  if (p2 && lane < 16u) asm volatile("prefetch.global.L2 [%0];" ::"l"(p2));
+}
 template <int MIN_IDLE, unsigned MAX_CHUNK>
-__device__ __forceinline__ unsigned refill_index(const TransportArgs &a, bool idle, unsigned count, SrcCursor &sc, bool &exhausted) {
+__device__ __forceinline__ unsigned refill_index(const TransportArgs &a, bool idle, unsigned n1, unsigned count, SrcCursor &sc, bool &exhausted) {
   const unsigned need = __ballot_sync(kFull, idle);
   if (!need || exhausted) return 0xffffffffu;
   if (MIN_IDLE > 1 && need != kFull && __popc(need) < MIN_IDLE) return 0xffffffffu;   // refill in groups: the refill code then runs with more lanes
@@ -155,6 +170,7 @@ __device__ __forceinline__ unsigned refill_index(const TransportArgs &a, bool id
     base = __shfl_sync(kFull, base, 0);
     if (base >= count) { exhausted = true; return 0xffffffffu; }
     sc.next = base; sc.end = min(base + chunk, count);
+    prefetch_chunk(a, n1, sc.next, sc.end);
   }
   const unsigned rank = __popc(need & ((1u << lane) - 1u)), avail = sc.end - sc.next;
   const unsigned idx = sc.next + rank;
@@ -205,7 +221,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
   const unsigned count = n1 + ((a.src_kind == SRC_BUFFER && a.src2_count) ? min(*a.src2_count, a.src.cap) : 0u);
   SrcCursor sc; sc.next = sc.end = 0u;
   StageRing &ring = *reinterpret_cast<StageRing *>(s_raw + kXsBytes + sizeof(StageRing) * (threadIdx.x >> 5));
-  StageCursor stg; stg.head = stg.n = 0u;
+  StageCursor stg; stg.head = stg.n = stg.base_raw = 0u; stg.pending = false;
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
   Pending pend; pend.v = 0; pend.q = 0;
@@ -218,7 +234,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
 
   for (;;) {
     // ---- refill idle lanes
-    const unsigned idx = refill_index<1, 128u>(a, state == PH_IDLE, count, sc, exhausted);
+    const unsigned idx = refill_index<1, 128u>(a, state == PH_IDLE, n1, count, sc, exhausted);
     if (idx != 0xffffffffu) {
       const TrackIn t = load_track(a, idx, n1);
       if (t.ok) {
@@ -371,7 +387,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
       }
     }
   }
-  if (stg.n) stage_flush(a.eq, a.ctl, ring, stg, stg.n);
+  stage_drain(a.eq, a.ctl, ring, stg);
   pend.flush(g);
   tally_flush<DBG>(a, tl);
 }
@@ -402,7 +418,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
   Fnv fnv; fnv.v = 0;
 
   for (;;) {
-    const unsigned idx = refill_index<kElectronRefillMin, kElectronChunk>(a, !active, count, sc, exhausted);
+    const unsigned idx = refill_index<kElectronRefillMin, kElectronChunk>(a, !active, n1, count, sc, exhausted);
     if (idx != 0xffffffffu) {
       const TrackIn t = load_track(a, idx, n1);
       if (t.ok) {
