@@ -76,6 +76,8 @@ typedef struct psl psl_t;          /* opaque: active lets, alias tables, group w
 #define MC_FLAG_STATS           2  /* fill the event counters of mc_stats_t (ledgers are always) */
 #define MC_FLAG_TIMING          4  /* CUDA-event time per kernel class into mc_stats_t           */
 #define MC_FLAG_STATIC_LANES    8  /* ablation: one particle per thread, no lane refill          */
+#define MC_FLAG_STAGE_SCORING  16  /* stage the scoring atomics of hot voxels in shared memory    */
+                                   /* (per-CTA table, added to the grid at kernel exit; same bits)  */
 
 typedef struct {
   void     *workspace;             /* DEVICE scratch or NULL (library-managed, cached in psl_t)  */

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpslmc.so")
 
 MC_ORDER_SORTED, MC_ORDER_MIXED = 0, 1
-MC_FLAG_ELECTRONS_LOCAL, MC_FLAG_STATS, MC_FLAG_TIMING, MC_FLAG_STATIC_LANES = 1, 2, 4, 8
+MC_FLAG_ELECTRONS_LOCAL, MC_FLAG_STATS, MC_FLAG_TIMING, MC_FLAG_STATIC_LANES, MC_FLAG_STAGE_SCORING = 1, 2, 4, 8, 16
 LEDGERS = ("incident", "deposited", "escaped", "jaw")
 KERNEL_CLASSES = ("sample", "photon", "electron", "finalise", "aux")
 EXPORTS = ("psl_build", "psl_free", "psl_export", "psl_allocate", "mc_workspace_bytes", "mc_dose", "mc_dose_host",

@@ -210,6 +210,7 @@ struct Run {
     a.fp = fp; a.fp_base = fp_base;
     a.electrons_local = (flags & MC_FLAG_ELECTRONS_LOCAL) ? 1 : 0;
     a.static_lanes = (flags & MC_FLAG_STATIC_LANES) ? 1 : 0;
+    a.stage_scoring = (flags & MC_FLAG_STAGE_SCORING) ? 1 : 0;
     a.xs = xs;
     return a;
   }
@@ -226,20 +227,37 @@ struct Run {
   int photon_blocks(int persistent) const { return (int)std::max<uint64_t>(1, std::min<uint64_t>({(uint64_t)persistent, (batch + kThreads - 1) / kThreads, 4096 / (kThreads / 32)})); }
   void photon(const TransportArgs &a) {
     tm.begin(MC_K_PHOTON);
-    if (dbg) k_photon<true><<<photon_blocks(blocks_photon[1]), kThreads, kXsSmem, st>>>(a);
-    else k_photon<false><<<photon_blocks(blocks_photon[0]), kThreads, kXsSmem, st>>>(a);
+    const int nb = photon_blocks(blocks_photon[dbg]);
+    if (a.stage_scoring) {
+      if (dbg) k_photon<true, true><<<nb, kThreads, kXsSmem + kScoreBytes, st>>>(a); else k_photon<false, true><<<nb, kThreads, kXsSmem + kScoreBytes, st>>>(a);
+    } else {
+      if (dbg) k_photon<true, false><<<nb, kThreads, kXsSmem, st>>>(a); else k_photon<false, false><<<nb, kThreads, kXsSmem, st>>>(a);
+    }
     tm.end(MC_K_PHOTON); ++launches[MC_K_PHOTON];
   }
   void electron(const TransportArgs &a) {
     tm.begin(MC_K_ELECTRON);
-    if (dbg) k_electron<true><<<blocks_electron[1], kThreads, 0, st>>>(a); else k_electron<false><<<blocks_electron[0], kThreads, 0, st>>>(a);
+    const int nb = blocks_electron[dbg];
+    if (a.stage_scoring) {
+      if (dbg) k_electron<true, true><<<nb, kThreads, kScoreBytes, st>>>(a); else k_electron<false, true><<<nb, kThreads, kScoreBytes, st>>>(a);
+    } else {
+      if (dbg) k_electron<true, false><<<nb, kThreads, 0, st>>>(a); else k_electron<false, false><<<nb, kThreads, 0, st>>>(a);
+    }
     tm.end(MC_K_ELECTRON); ++launches[MC_K_ELECTRON];
   }
   void init_blocks() {
-    cudaFuncSetAttribute(k_photon<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXsSmem);
-    cudaFuncSetAttribute(k_photon<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXsSmem);
-    blocks_photon[0] = persistent_blocks(k_photon<false>, kXsSmem); blocks_photon[1] = persistent_blocks(k_photon<true>, kXsSmem);
-    blocks_electron[0] = persistent_blocks(k_electron<false>); blocks_electron[1] = persistent_blocks(k_electron<true>);
+    const bool stage = (flags & MC_FLAG_STAGE_SCORING) != 0;
+    if (stage) {
+      cudaFuncSetAttribute(k_photon<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kXsSmem + kScoreBytes));
+      cudaFuncSetAttribute(k_photon<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kXsSmem + kScoreBytes));
+      blocks_photon[0] = persistent_blocks(k_photon<false, true>, kXsSmem + kScoreBytes); blocks_photon[1] = persistent_blocks(k_photon<true, true>, kXsSmem + kScoreBytes);
+      blocks_electron[0] = persistent_blocks(k_electron<false, true>, kScoreBytes); blocks_electron[1] = persistent_blocks(k_electron<true, true>, kScoreBytes);
+    } else {
+      cudaFuncSetAttribute(k_photon<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXsSmem);
+      cudaFuncSetAttribute(k_photon<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXsSmem);
+      blocks_photon[0] = persistent_blocks(k_photon<false, false>, kXsSmem); blocks_photon[1] = persistent_blocks(k_photon<true, false>, kXsSmem);
+      blocks_electron[0] = persistent_blocks(k_electron<false, false>); blocks_electron[1] = persistent_blocks(k_electron<true, false>);
+    }
   }
   // Folds the finished batch's counters, resets them, and swaps the photon queues (n_pq -> n_pq_prev).
   void next_batch() {

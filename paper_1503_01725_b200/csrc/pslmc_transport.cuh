@@ -46,7 +46,7 @@ struct TransportArgs {
   Queue eq, pq;
   // options
   unsigned long long *fp; unsigned long long fp_base;
-  int electrons_local, static_lanes;
+  int electrons_local, static_lanes, stage_scoring;
   int want_type;                      // SRC_BUFFER, compact: take only entries of this particle type (bit 31 of p1.w)
   XsTable xs;                         // k_photon: cross-section table (global; copied to shared memory per CTA)
 };
@@ -73,11 +73,47 @@ __device__ __forceinline__ void tally_flush(const TransportArgs &a, Tally &t) {
 }
 
 // Pending deposit: consecutive deposits into one voxel are merged before the atomic (integers: exact).
+// Optional shared-memory staging of the scoring atomics (north_star (4), MC_FLAG_STAGE_SCORING): a per-CTA
+// direct-mapped table of kScoreSlots voxel accumulators.  A voxel claims a free slot on first touch and keeps it
+// for the whole launch (no eviction: integer sums make the result independent of who claimed what); deposits to
+// a voxel that owns a slot are shared-memory atomics, all others go to the global grid as before; the table is
+// added to the grid once at kernel exit.  Helps only where a launch concentrates its deposits on <~ 1e3 voxels
+// per CTA (narrow beams); DESIGN.md §5 has the measured ablation.
+constexpr int kScoreSlots = 1024;
+constexpr size_t kScoreBytes = (size_t)kScoreSlots * (sizeof(unsigned long long) + sizeof(int));
+template <bool ON>
+struct ScoreStage {
+  unsigned long long *sum; int *tag;                 // shared memory (unused when !ON)
+  __device__ __forceinline__ void init(unsigned char *smem) {
+    sum = nullptr; tag = nullptr;
+    if (!ON) return;
+    sum = reinterpret_cast<unsigned long long *>(smem); tag = reinterpret_cast<int *>(smem + sizeof(unsigned long long) * kScoreSlots);
+    for (int i = threadIdx.x; i < kScoreSlots; i += kThreads) { sum[i] = 0ull; tag[i] = -1; }
+    __syncthreads();
+  }
+  __device__ __forceinline__ void add(const Grid &g, int v, unsigned long long q) const {
+    if (ON) {
+      const unsigned s = ((unsigned)v * 2654435761u) >> 22;                       // 10 bits
+      int t = tag[s];
+      if (t == -1) { t = atomicCAS(tag + s, -1, v); if (t == -1) t = v; }
+      if (t == v) { atomicAdd(sum + s, q); return; }
+    }
+    atomicAdd(g.acc + v, q);
+  }
+  __device__ __forceinline__ void drain(const Grid &g) const {                    // every thread of the CTA calls this
+    if (!ON) return;
+    __syncthreads();
+    for (int i = threadIdx.x; i < kScoreSlots; i += kThreads)
+      if (tag[i] >= 0 && sum[i]) atomicAdd(g.acc + tag[i], sum[i]);
+  }
+};
+
+// Pending deposit: consecutive deposits into one voxel are merged before the atomic (integers: exact).
 struct Pending {
   int v; long long q;
-  __device__ __forceinline__ void flush(const Grid &g) { if (q) atomicAdd(g.acc + v, (unsigned long long)q); q = 0; }
-  __device__ __forceinline__ void add(const Grid &g, int vox, long long dq) {
-    if (vox != v) { flush(g); v = vox; }
+  template <bool ON> __device__ __forceinline__ void flush(const Grid &g, const ScoreStage<ON> &st) { if (q) st.add(g, v, (unsigned long long)q); q = 0; }
+  template <bool ON> __device__ __forceinline__ void add(const Grid &g, const ScoreStage<ON> &st, int vox, long long dq) {
+    if (vox != v) { flush(g, st); v = vox; }
     q += dq;
   }
 };
@@ -210,12 +246,13 @@ __device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned i
 // of holding the warp in a rejection loop.  Cross-sections come from the shared-memory table.
 enum { PH_IDLE = 0, PH_FLIGHT = 1, PH_KAHN = 2, PH_PAIR = 3 };
 
-template <bool DBG>
+template <bool DBG, bool STAGE>
 __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ TransportArgs a) {
   extern __shared__ __align__(16) unsigned char s_raw[];           // [xs table | one StageRing per warp]
   float2 *s_xs = reinterpret_cast<float2 *>(s_raw);
   for (int i = threadIdx.x; i <= a.xs.n; i += kThreads) s_xs[i] = a.xs.nodes[i];
   __syncthreads();
+  ScoreStage<STAGE> stage; stage.init(s_raw + kXsBytes + sizeof(StageRing) * (kThreads / 32));
   const Grid &g = a.g;
   const unsigned n1 = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
   const unsigned count = n1 + ((a.src_kind == SRC_BUFFER && a.src2_count) ? min(*a.src2_count, a.src.cap) : 0u);
@@ -261,7 +298,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
       float skn = 0.f, lp2 = 0.f, mu_max = 0.f;
       if (E >= kPcut) xs_lookup(s_xs, a.xs.x0, a.xs.inv_h, a.xs.n, E, skn, lp2, mu_max);
       if (E < kPcut) {                                   // below cut-off: absorbed on the spot
-        const long long q = quanta(E); pend.add(g, cvox, q); tl.dep += (unsigned long long)q;
+        const long long q = quanta(E); pend.add(g, stage, cvox, q); tl.dep += (unsigned long long)q;
         if (DBG) { fnv.byte('A'); ++tl.st[ST_PCUT]; ++tl.st[ST_DEPOSITS]; }
         done = true;
       } else if (!(mu_max > 0.0f)) {
@@ -290,7 +327,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
             collided = true; state = PH_KAHN;
             if (DBG) { fnv.byte('C'); ++tl.st[ST_COMPTON]; }
           } else if (tt < muC + muT) {                   // photo-electric: local absorption
-            const long long q = quanta(E); pend.add(g, cvox, q); tl.dep += (unsigned long long)q;
+            const long long q = quanta(E); pend.add(g, stage, cvox, q); tl.dep += (unsigned long long)q;
             if (DBG) { fnv.byte('P'); ++tl.st[ST_PHOTO]; ++tl.st[ST_DEPOSITS]; }
             done = true;
           } else if (tt < muC + muT + muK) {             // pair production: event 2
@@ -333,7 +370,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
             eT = T; etrack = child_track(rng.track, nchild, 0u); push_e = true;
             if (DBG) ++tl.st[ST_SEC_E];
           } else {
-            const long long q = quanta(T); pend.add(g, cvox, q); tl.dep += (unsigned long long)q;
+            const long long q = quanta(T); pend.add(g, stage, cvox, q); tl.dep += (unsigned long long)q;
             if (DBG) ++tl.st[ST_DEPOSITS];
           }
           ++nchild; E = Ep; state = PH_FLIGHT;
@@ -348,7 +385,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
             pairT[sl] = Tc[sl];
             if (DBG) ++tl.st[ST_SEC_E];
           } else {
-            const long long q = quanta(Tc[sl]); pend.add(g, cvox, q); tl.dep += (unsigned long long)q;
+            const long long q = quanta(Tc[sl]); pend.add(g, stage, cvox, q); tl.dep += (unsigned long long)q;
             if (DBG) ++tl.st[ST_DEPOSITS];
           }
         }
@@ -388,7 +425,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
     }
   }
   stage_drain(a.eq, a.ctl, ring, stg);
-  pend.flush(g);
+  pend.flush(g, stage);
+  stage.drain(g);
   tally_flush<DBG>(a, tl);
 }
 
@@ -398,9 +436,11 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
 // ~1e-6 cm of a global coordinate.  In exact arithmetic this is the
 // same walk as floor((pos - o)/d) on global coordinates.  One loop iteration = one sub-step; the two
 // draws of a condensed step come from one Philox site (draw numbers are always even here).
-template <bool DBG>
+template <bool DBG, bool STAGE>
 __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant__ TransportArgs a) {
+  extern __shared__ __align__(16) unsigned char s_raw[];           // [score staging table] when enabled
   const Grid &g = a.g;
+  ScoreStage<STAGE> stage; stage.init(s_raw);
   const unsigned n1 = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
   const unsigned count = n1 + ((a.src_kind == SRC_BUFFER && a.src2_count) ? min(*a.src2_count, a.src.cap) : 0u);
   SrcCursor sc; sc.next = sc.end = 0u;
@@ -458,11 +498,11 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
       if (DBG) { ++tl.st[ST_ESTEPS]; ++tl.st[ST_DEPOSITS]; }
       bool done = false;
       if (T - dT <= kEcut) {
-        const long long q = quanta(T); pend.add(g, vox, q); tl.dep += (unsigned long long)q;
+        const long long q = quanta(T); pend.add(g, stage, vox, q); tl.dep += (unsigned long long)q;
         if (DBG) { fnv.u32(steps); fnv.byte('A'); }
         done = true;
       } else {
-        const long long q = quanta(dT); pend.add(g, vox, q); tl.dep += (unsigned long long)q;
+        const long long q = quanta(dT); pend.add(g, stage, vox, q); tl.dep += (unsigned long long)q;
         lx = __fmaf_rn(s, u, lx); ly = __fmaf_rn(s, v, ly); lz = __fmaf_rn(s, w, lz);
         T -= dT; budget -= dT; tacc = __fmaf_rn(rho * s, c_mat.inv_x0[mt], tacc);
         // re-home: a step ends at most eps beyond the face it was limited by
@@ -489,7 +529,8 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
       if (done) { if (DBG) finish_track<DBG>(a, h, fnv); active = false; }
     }
   }
-  pend.flush(g);
+  pend.flush(g, stage);
+  stage.drain(g);
   tally_flush<DBG>(a, tl);
 }
 
