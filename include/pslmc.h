@@ -173,6 +173,13 @@ int  mc_transport_debug(const phantom_t *ph, int32_t particle_type, const float 
                         uint64_t first_history, uint64_t count, uint64_t seed,
                         const mc_opts_t *opts);
 
+/* The photon cross-section lookup of k_photon (per-call table in log2 E, linear interpolation) for a
+ * list of energies: builds the table for the given largest density per material (rhomax[3]: water,
+ * lung, bone) and top energy e_max (MeV, > 0.05), then evaluates it ON THE DEVICE.
+ * E_host: HOST float[n] (0.05 <= E <= e_max); out_host: HOST float[3n] = (sigma_KN cm^2 per electron,
+ * ln^2(E/1.022) or 0 below threshold, mu_max cm^-1) per energy.                                  */
+int  mc_xs_debug(const float rhomax[3], double e_max, const float *E_host, uint64_t n, float *out_host);
+
 /* One Philox4x32-10 block computed ON THE DEVICE: key = seed, counter = (block, track, h_lo, h_hi).
  * out: HOST u32[4].                                                                             */
 int  mc_philox_debug(uint64_t seed, uint64_t history, uint32_t track, uint32_t block,

@@ -19,7 +19,7 @@ MC_FLAG_ELECTRONS_LOCAL, MC_FLAG_STATS, MC_FLAG_TIMING, MC_FLAG_STATIC_LANES, MC
 LEDGERS = ("incident", "deposited", "escaped", "jaw")
 KERNEL_CLASSES = ("sample", "photon", "electron", "finalise", "aux")
 EXPORTS = ("psl_build", "psl_free", "psl_export", "psl_allocate", "mc_workspace_bytes", "mc_dose", "mc_dose_host",
-           "mc_stats", "mc_last_error", "mc_sample_debug", "mc_transport_debug", "mc_philox_debug")
+           "mc_stats", "mc_last_error", "mc_sample_debug", "mc_transport_debug", "mc_philox_debug", "mc_xs_debug")
 
 
 class PslmcError(RuntimeError):
@@ -93,6 +93,7 @@ def lib():
         L.mc_transport_debug.argtypes = [C.POINTER(phantom_t), C.c_int32, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64,
                                          C.POINTER(mc_opts_t)]
         L.mc_philox_debug.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
+        L.mc_xs_debug.argtypes = [C.c_void_p, C.c_double, C.c_void_p, C.c_uint64, C.c_void_p]
         _lib = L
     return _lib
 
@@ -248,6 +249,15 @@ def transport_debug(phantom: DevicePhantom, ptype: int, soa, first: int, seed: i
 def philox_debug(seed: int, history: int, track: int, block: int) -> np.ndarray:
     out = np.empty(4, np.uint32)
     _check(lib().mc_philox_debug(seed, history, track, block, out.ctypes.data_as(C.c_void_p)))
+    return out
+
+
+def xs_debug(rhomax, e_max: float, energies) -> np.ndarray:
+    """k_photon's cross-section lookup for `energies` (MeV): rows of (sigma_KN, ln^2(E/1.022), mu_max)."""
+    rm = np.ascontiguousarray(rhomax, np.float32)
+    e = np.ascontiguousarray(energies, np.float32)
+    out = np.empty((e.size, 3), np.float32)
+    _check(lib().mc_xs_debug(rm.ctypes.data_as(C.c_void_p), float(e_max), e.ctypes.data_as(C.c_void_p), e.size, out.ctypes.data_as(C.c_void_p)))
     return out
 
 

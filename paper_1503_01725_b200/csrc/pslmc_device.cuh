@@ -189,27 +189,37 @@ struct PhotonXs {
   }
 };
 
-// Photon cross-section table (built per mc_dose call on the device, in double, by k_build_xs): node i
-// holds (sigma_KN, mu_max) at log2(E) = x0 + i*h; k_photon keeps it in shared memory and interpolates
-// linearly in log2(E) (relative error ~1e-7 at n = 4096: DESIGN.md §6).  ln(E/1.022) of the pair term
-// comes from the same log2(E).
-struct XsTable { const float2 *nodes; float x0, inv_h; int n; };      // n intervals, n + 1 nodes
+__device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 
-__device__ __forceinline__ void xs_lookup(const float2 *tab, float x0, float inv_h, int n, float E,
-                                          float &skn, float &lp2, float &mu_max) {
+// Photon cross-section data (built per mc_dose call on the device, in double, by k_build_xs), kept in shared
+// memory by k_photon:  floats [0,12) = per material m the Woodcock majorant coefficients
+// (rhomax_m ne_m, rhomax_m cphoto_m, rhomax_m ppair_m, 0);  floats [12, 12 + n + 1) = sigma_KN at
+// log2(E) = x0 + i*h, interpolated linearly (relative error ~1e-7 at n = 4096: DESIGN.md §6).  1/E^3 and
+// ln(E/1.022) are computed directly (the latter from the same log2 E), so
+// mu_max = max_m (A_m sigma_KN + B_m / E^3 + C_m ln^2) carries no interpolation error of its own.
+constexpr int kXsHead = 12;
+struct XsTable { const float *data; float x0, inv_h; int n; };      // n intervals, n + 1 nodes after the head
+
+__device__ __forceinline__ void xs_lookup(const float *tab, float x0, float inv_h, int n, float E,
+                                          float &skn, float &inv_e3, float &lp2, float &mu_max) {
   const float lg = __log2f(E);
   float t = (lg - x0) * inv_h;
   t = fminf(fmaxf(t, 0.0f), (float)n);
   const int i = min((int)t, n - 1);
   const float f = t - (float)i;
-  const float2 A = tab[i], B = tab[i + 1];
-  skn = __fmaf_rn(f, B.x - A.x, A.x); mu_max = __fmaf_rn(f, B.y - A.y, A.y);
+  const float a = tab[kXsHead + i], b = tab[kXsHead + i + 1];
+  skn = __fmaf_rn(f, b - a, a);
   const float l = E > kEPair ? (lg - 0.03139551f) * 0.69314718f : 0.0f;      // log2(1.022) = 0.0313955
   lp2 = l * l;
+  inv_e3 = rcp_fast(E * E * E);
+  const float4 *mj = reinterpret_cast<const float4 *>(tab);
+  float m = 0.0f;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) { const float4 c = mj[k]; m = fmaxf(m, __fmaf_rn(c.x, skn, __fmaf_rn(c.y, inv_e3, c.z * lp2))); }
+  mu_max = m;
 }
 
 __device__ __forceinline__ float sqrt_fast(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
-__device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 
 __device__ __forceinline__ void rotate(float &u, float &v, float &w, float ct, float st, float uphi) {
   float sp, cp;

@@ -219,9 +219,9 @@ struct Run {
   // Builds the cross-section table of this call (after k_rhomax) for photon energies up to e_max.
   void build_xs(double e_max) {
     const double x0 = std::log2(0.045), x1 = std::log2(e_max * 1.001), hh = (x1 - x0) / kXsIntervals;
-    float2 *nodes = (float2 *)(ws + L.xs);
+    float *nodes = (float *)(ws + L.xs);
     k_build_xs<<<(kXsIntervals + 256) / 256, 256, 0, st>>>(ctl, nodes, x0, hh, kXsIntervals);
-    xs.nodes = nodes; xs.x0 = (float)x0; xs.inv_h = (float)(1.0 / hh); xs.n = kXsIntervals;
+    xs.data = nodes; xs.x0 = (float)x0; xs.inv_h = (float)(1.0 / hh); xs.n = kXsIntervals;
   }
   uint64_t batch = 0;                           // upper bound of the entries a photon launch can see
   int photon_blocks(int persistent) const { return (int)std::max<uint64_t>(1, std::min<uint64_t>({(uint64_t)persistent, (batch + kThreads - 1) / kThreads, 4096 / (kThreads / 32)})); }
@@ -563,6 +563,25 @@ extern "C" int mc_transport_debug(const phantom_t *ph, int32_t particle_type, co
   cudaEventDestroy(ev0); cudaEventDestroy(ev1);
   fold_stats(hc, r, &g_stats);
   if (hc.overflow) return fail(MC_E_OVERFLOW, "mc_transport_debug: a secondary queue overflowed");
+  return MC_OK;
+}
+
+extern "C" int mc_xs_debug(const float rhomax[3], double e_max, const float *E_host, uint64_t n, float *out_host) {
+  if (!rhomax || !E_host || !out_host || !(e_max > 0.05) || n > (1ull << 28)) return fail(MC_E_INVALID_ARG, "mc_xs_debug: invalid argument");
+  if (n == 0) return MC_OK;
+  char *d = nullptr;
+  const size_t o_ctl = 0, o_xs = align_up(sizeof(Control)), o_e = o_xs + align_up(kXsBytes), o_out = o_e + align_up(4 * n), total = o_out + 12 * n;
+  CUDA_TRY(cudaMalloc((void **)&d, total));
+  Control hc; memset(&hc, 0, sizeof hc);
+  for (int k = 0; k < 3; ++k) hc.rhomax[k] = rhomax[k];
+  CUDA_TRY(cudaMemcpy(d + o_ctl, &hc, sizeof hc, cudaMemcpyHostToDevice));
+  CUDA_TRY(cudaMemcpy(d + o_e, E_host, 4 * n, cudaMemcpyHostToDevice));
+  Run r{}; r.st = nullptr; r.ws = d; r.L.xs = o_xs; r.ctl = (Control *)(d + o_ctl);
+  r.build_xs(e_max);
+  k_xs_debug<<<(unsigned)((n + 255) / 256), 256>>>(r.xs, (const float *)(d + o_e), n, (float *)(d + o_out));
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaMemcpy(out_host, d + o_out, 12 * n, cudaMemcpyDeviceToHost));
+  cudaFree(d);
   return MC_OK;
 }
 

@@ -234,18 +234,28 @@ __global__ void k_pack_phantom(const float *density, const uint8_t *material, si
   }
 }
 
-// Photon cross-section table for this call (needs rhomax): node i at log2(E) = x0 + i*h, in double.
-__global__ void k_build_xs(const Control *c, float2 *nodes, double x0, double h, int n) {
+// Photon cross-section data of this call (needs rhomax): layout in pslmc_device.cuh (XsTable), evaluated in double.
+__global__ void k_build_xs(const Control *c, float *data, double x0, double h, int n) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < 3) {
+    const double rm = (double)c->rhomax[i];
+    data[4 * i] = (float)(rm * (double)c_mat.ne[i]); data[4 * i + 1] = (float)(rm * (double)c_mat.cphoto[i]);
+    data[4 * i + 2] = (float)(rm * (double)c_mat.ppair[i]); data[4 * i + 3] = 0.0f;
+  }
   if (i > n) return;
   const double E = exp2(x0 + h * (double)i);
   const double al = E / kMeD, L = log1p(2.0 * al), t = 1.0 + 2.0 * al;
   const double skn = kTwoPiRe2 * ((1.0 + al) / (al * al) * (2.0 * (1.0 + al) / t - L / al) + L / (2.0 * al) - (1.0 + 3.0 * al) / (t * t));
-  const double l = E > 1.022 ? log(E / 1.022) : 0.0, lp2 = l * l, ie3 = 1.0 / (E * E * E);
-  double m = 0.0;
-  for (int k = 0; k < 3; ++k)
-    m = fmax(m, (double)c->rhomax[k] * ((double)c_mat.ne[k] * skn + (double)c_mat.cphoto[k] * ie3 + (double)c_mat.ppair[k] * lp2));
-  nodes[i] = make_float2((float)skn, (float)m);
+  data[kXsHead + i] = (float)skn;
+}
+
+// Parity probe: the table lookup k_photon does, for a list of energies.  out: (sigma_KN, ln^2(E/1.022), mu_max) per energy.
+__global__ void k_xs_debug(XsTable xs, const float *E, size_t n, float *out) {
+  const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  float skn, ie3, lp2, mu;
+  xs_lookup(xs.data, xs.x0, xs.inv_h, xs.n, E[i], skn, ie3, lp2, mu);
+  out[3 * i] = skn; out[3 * i + 1] = lp2; out[3 * i + 2] = mu;
 }
 
 // dose[v] = acc[v] 2^-32 / (rho_v V N)

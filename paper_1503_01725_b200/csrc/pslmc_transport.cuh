@@ -26,7 +26,7 @@ enum { SRC_BUFFER = 0, SRC_QUEUE = 1 };
 constexpr int kElectronRefillMin = ELECTRON_REFILL_MIN;
 constexpr unsigned kElectronChunk = ELECTRON_CHUNK;
 constexpr int kXsIntervals = 4096;
-constexpr size_t kXsBytes = sizeof(float2) * (kXsIntervals + 2);     // padded to 16 bytes
+constexpr size_t kXsBytes = sizeof(float) * (kXsHead + kXsIntervals + 4);     // head + n + 1 nodes, padded to 16 bytes
 
 struct TransportArgs {
   Grid g;
@@ -249,8 +249,8 @@ enum { PH_IDLE = 0, PH_FLIGHT = 1, PH_KAHN = 2, PH_PAIR = 3 };
 template <bool DBG, bool STAGE>
 __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ TransportArgs a) {
   extern __shared__ __align__(16) unsigned char s_raw[];           // [xs table | one StageRing per warp]
-  float2 *s_xs = reinterpret_cast<float2 *>(s_raw);
-  for (int i = threadIdx.x; i <= a.xs.n; i += kThreads) s_xs[i] = a.xs.nodes[i];
+  float *s_xs = reinterpret_cast<float *>(s_raw);
+  for (int i = threadIdx.x; i <= kXsHead + a.xs.n; i += kThreads) s_xs[i] = a.xs.data[i];
   __syncthreads();
   ScoreStage<STAGE> stage; stage.init(s_raw + kXsBytes + sizeof(StageRing) * (kThreads / 32));
   const Grid &g = a.g;
@@ -295,8 +295,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
     // ---- event 1: one Woodcock flight and the choice of interaction
     if (state == PH_FLIGHT) {
       bool done = false;
-      float skn = 0.f, lp2 = 0.f, mu_max = 0.f;
-      if (E >= kPcut) xs_lookup(s_xs, a.xs.x0, a.xs.inv_h, a.xs.n, E, skn, lp2, mu_max);
+      float skn = 0.f, inv_e3 = 0.f, lp2 = 0.f, mu_max = 0.f;
+      if (E >= kPcut) xs_lookup(s_xs, a.xs.x0, a.xs.inv_h, a.xs.n, E, skn, inv_e3, lp2, mu_max);
       if (E < kPcut) {                                   // below cut-off: absorbed on the spot
         const long long q = quanta(E); pend.add(g, stage, cvox, q); tl.dep += (unsigned long long)q;
         if (DBG) { fnv.byte('A'); ++tl.st[ST_PCUT]; ++tl.st[ST_DEPOSITS]; }
@@ -320,7 +320,6 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
         } else {
           cvox = vox_index(g, vi, vj, vk);
           float rho; int mt; fetch_voxel(g, cvox, rho, mt);
-          const float inv_e3 = rcp_fast(E * E * E);
           const float muC = rho * (c_mat.ne[mt] * skn), muT = rho * (c_mat.cphoto[mt] * inv_e3), muK = rho * (c_mat.ppair[mt] * lp2);
           const float tt = u_co(d1) * mu_max;
           if (tt < muC) {                                // Compton: Kahn trials are event 2

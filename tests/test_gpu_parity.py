@@ -60,6 +60,25 @@ def test_tables_and_allocation_bit_exact(name, B, gpsl, opsl, cfg):
         assert np.array_equal(gpsl(name).allocate(N), o.allocate(N))
 
 
+def test_cross_section_table_matches_closed_forms(B, orc):
+    """k_photon reads sigma_KN and mu_max from a per-call table (4096 intervals in log2 E, linear interpolation):
+    against the oracle's closed forms the relative error must stay below 5e-7."""
+    rng = np.random.default_rng(11)
+    E = np.concatenate([np.exp(rng.uniform(np.log(0.05), np.log(6.0), 200_000)), [0.05, 0.0500001, 1.0219, 1.0221, 5.999999, 6.0]]).astype(np.float32)
+    rhomax = np.array([1.02, 0.3, 1.9], np.float32)
+    got = B.xs_debug(rhomax, 6.0, E).astype(np.float64)
+    E64 = E.astype(np.float64)
+    skn = np.array([orc.sigma_kn(e) for e in E64])
+    assert np.max(np.abs(got[:, 0] / skn - 1)) < 5e-7
+    lp2 = np.where(E64 > 1.022, np.log(E64 / 1.022) ** 2, 0.0)
+    assert np.max(np.abs(got[:, 1] - lp2)) < 2e-6 * np.maximum(lp2, 1e-3).max()
+    mu = np.zeros_like(E64)
+    for m in range(3):
+        c = np.array([orc.mu_over_rho(m, e) for e in E64]).sum(axis=1)
+        mu = np.maximum(mu, float(rhomax[m]) * c)
+    assert np.max(np.abs(got[:, 2] / mu - 1)) < 5e-7
+
+
 # ---------------------------------------------------------------- k_sample
 def check_samples(B, g, o, beam, N, seed, first, count):
     got = soa_to_rows(g.sample_debug(beam, N, seed, first, count))
