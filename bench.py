@@ -137,7 +137,8 @@ class ClockSampler:
 # Algorithmic work per history of the bench workload, stated in DESIGN.md §Roofline and measured once
 # with ncu (profiles/): SASS thread-instructions the transport kernels retire per C1 primary history,
 # and the bytes k_sample must write per history (32 B per particle that passes the jaws).
-ALG_THREAD_INST_PER_HISTORY = {"C1": {"photon": 646.0, "electron": 898.0, "sample": 486.0}}      # profiles/r1b_launches.md
+ALG_THREAD_INST_PER_HISTORY = {"C1": {"photon": 646.0, "electron": 898.0, "sample": 486.0},      # profiles/r1b_launches.md
+                               "C4": {"photon": 2575.0, "electron": 2604.0, "sample": 600.0}}    # profiles/r1b_ablation_c4.md (batch 2^22, sorted)
 # DRAM bytes (read + write) per step of each kernel class, from the ncu --set full captures of profiles/r1b_top_kernels.md
 # (the two primary-batch launches; the path's working set is L2-resident, so this is far below any HBM bound)
 NCU_DRAM_BYTES_PER_STEP = {"C1": {"photon": 2.21e8, "electron": 1.42e8, "sample": 4.5e7}}
@@ -245,7 +246,9 @@ def run_ours(args):
     hbm_peak, sm_max, which = load_peaks()
     dom = max(("sample", "photon", "electron"), key=lambda k: ms_class[k])
     hist_rank = (he - hb) * args.steps
-    alg = ALG_THREAD_INST_PER_HISTORY.get(args.config, ALG_THREAD_INST_PER_HISTORY["C1"])
+    alg = ALG_THREAD_INST_PER_HISTORY.get(args.config)
+    if alg is None:                                      # no ncu count for this workload: report times only
+        alg = {"photon": float("nan"), "electron": float("nan"), "sample": float("nan")}
     n_acc = hist_rank - st["n_jaw_rejected"] * args.steps
     sample_gbs = SAMPLE_BYTES_PER_PARTICLE * n_acc / (ms_class["sample"] * 1e-3) / 1e9 if ms_class["sample"] > 0 else 0.0
     if dom == "sample":
