@@ -287,7 +287,13 @@ def run_ours(args):
         v, done, dt = time_oracle(cfg, n_total, min(n_total, 20_000_000))
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                                "sample": "%d of %d histories in 64 equally spaced id ranges, %.1f s" % (done, n_total, dt)}
-    print(json.dumps(out))
+    def clean(x):                                        # strict JSON: no NaN
+        if isinstance(x, dict):
+            return {k: clean(v) for k, v in x.items()}
+        if isinstance(x, float) and x != x:
+            return None
+        return x
+    print(json.dumps(clean(out)))
     if world > 1:
         dist.destroy_process_group()
 
