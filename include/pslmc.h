@@ -90,6 +90,12 @@ typedef struct {
   uint64_t *fingerprints;          /* DEVICE u64[history_end-history_begin] or NULL; ADDED to    */
   uint64_t  history_begin;         /* sub-range of history ids to run (sharding) ...             */
   uint64_t  history_end;           /* ... 0 means n_histories                                    */
+  int32_t   pipelines;             /* 0 = default (2): batches are dealt to this many independent  */
+                                   /* launch sequences on internal streams so that one kernel's    */
+                                   /* tail overlaps the next kernel; 1 = strictly serial launches  */
+                                   /* on cuda_stream (per-kernel times in mc_stats are then        */
+                                   /* disjoint).  Same bits either way.                            */
+  int32_t   reserved;              /* must be 0                                                    */
 } mc_opts_t;
 
 /* Ledger / kernel-class indices of mc_stats_t.                                                  */
@@ -111,7 +117,8 @@ typedef struct {
   uint64_t n_deposits;
   uint64_t queue_high_water[2];    /* electron queue, photon queue (entries)                     */
   uint64_t launches[5];            /* per MC_K_* class                                           */
-  float    ms[5];                  /* per MC_K_* class (MC_FLAG_TIMING)                          */
+  float    ms[5];                  /* per MC_K_* class (MC_FLAG_TIMING); with pipelines > 1 the    */
+                                   /* classes overlap in time and their sum exceeds ms_total       */
   float    ms_total;               /* whole mc_dose on its stream, CUDA events (always)          */
 } mc_stats_t;
 

@@ -51,7 +51,7 @@ class beam_geom_t(C.Structure):
 class mc_opts_t(C.Structure):
     _fields_ = [("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("cuda_stream", C.c_void_p),
                 ("dose_acc", C.c_void_p), ("order", C.c_int32), ("flags", C.c_int32), ("fingerprints", C.c_void_p),
-                ("history_begin", C.c_uint64), ("history_end", C.c_uint64)]
+                ("history_begin", C.c_uint64), ("history_end", C.c_uint64), ("pipelines", C.c_int32), ("reserved", C.c_int32)]
 
 
 class mc_stats_t(C.Structure):
@@ -147,7 +147,7 @@ def stats() -> dict:
 
 
 def _opts(stream=None, workspace=None, dose_acc=None, order=0, flags=0, fingerprints=None, history_begin=0,
-          history_end=0) -> mc_opts_t:
+          history_end=0, pipelines=0) -> mc_opts_t:
     o = mc_opts_t()
     if workspace is not None:
         o.workspace, o.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
@@ -156,6 +156,7 @@ def _opts(stream=None, workspace=None, dose_acc=None, order=0, flags=0, fingerpr
     o.order, o.flags = order, flags
     o.fingerprints = fingerprints.data_ptr() if fingerprints is not None else None
     o.history_begin, o.history_end = history_begin, history_end
+    o.pipelines = pipelines
     return o
 
 
@@ -214,7 +215,7 @@ class Psl:
                                      _stream_ptr(stream)))
         return out
 
-    def dose(self, phantom: DevicePhantom, beam: dict, n_histories: int, seed: int, batch: int = 1 << 20, dose_out=None,
+    def dose(self, phantom: DevicePhantom, beam: dict, n_histories: int, seed: int, batch: int = 1 << 22, dose_out=None,
              **opt):
         """mc_dose.  Returns dose_out (torch float64 on the device, MeV/g per history)."""
         import torch
@@ -225,7 +226,7 @@ class Psl:
                              dose_out.data_ptr() if dose_out is not None else None, C.byref(o)))
         return dose_out
 
-    def dose_host(self, ph: dict, beam: dict, n_histories: int, seed: int, batch: int = 1 << 20, dose_out: np.ndarray = None,
+    def dose_host(self, ph: dict, beam: dict, n_histories: int, seed: int, batch: int = 1 << 22, dose_out: np.ndarray = None,
                   density: np.ndarray = None, material: np.ndarray = None, **opt) -> np.ndarray:
         """mc_dose_host: host phantom arrays in, host dose out (copies inside the call)."""
         density = np.ascontiguousarray(ph["density"], np.float32) if density is None else density

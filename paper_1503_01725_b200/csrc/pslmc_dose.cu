@@ -42,24 +42,32 @@ static int scratch_get(Scratch &s, size_t bytes, void **out) {
 
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
-// Workspace layout for a batch of B primaries: control block, group offsets, the particle buffer
-// (2 planes), the electron queue (capacity 4B) and the photon queue (capacity B), each 3 planes,
-// then (optionally) the int64 dose grid.
+// Workspace layout for a batch of B primaries.  Shared by the whole call: group offsets, cross-section
+// data, packed phantom, (optionally) the int64 dose grid.  Per pipeline (kMaxPipes of them, see run_dose):
+// control block, the particle buffer (2 planes), the electron queue (capacity 4B) and the two photon
+// queues (capacity B each), 3 planes per queue.
+constexpr int kMaxPipes = 2;
 struct Layout {
   size_t ctl, off, xs, vox, p0, p1, eq[3], pq[2][3], acc, total;
   unsigned eq_cap, pq_cap;
 };
-static Layout make_layout(uint64_t batch, size_t nvox, bool with_acc) {
+static void make_layouts(uint64_t batch, size_t nvox, bool with_acc, Layout out[kMaxPipes]) {
   Layout L; size_t o = 0;
   auto take = [&](size_t b) { size_t at = o; o += align_up(b); return at; };
   L.eq_cap = (unsigned)std::min<uint64_t>(4 * batch, 0x7fffffffu); L.pq_cap = (unsigned)batch;
-  L.ctl = take(sizeof(Control)); L.off = take(sizeof(uint64_t) * 160); L.xs = take(kXsBytes); L.vox = take(4 * nvox);
-  L.p0 = take(16 * batch); L.p1 = take(16 * batch);
-  for (int k = 0; k < 3; ++k) L.eq[k] = take((size_t)16 * L.eq_cap);
-  for (int b = 0; b < 2; ++b) for (int k = 0; k < 3; ++k) L.pq[b][k] = take((size_t)16 * L.pq_cap);
+  L.off = take(sizeof(uint64_t) * 160); L.xs = take(kXsBytes); L.vox = take(4 * nvox);
   L.acc = take(with_acc ? 8 * nvox : 0);
-  L.total = o;
-  return L;
+  for (int p = 0; p < kMaxPipes; ++p) {
+    Layout &Q = out[p]; Q = L;
+    Q.ctl = take(sizeof(Control));
+    Q.p0 = take(16 * batch); Q.p1 = take(16 * batch);
+    for (int k = 0; k < 3; ++k) Q.eq[k] = take((size_t)16 * L.eq_cap);
+    for (int b = 0; b < 2; ++b) for (int k = 0; k < 3; ++k) Q.pq[b][k] = take((size_t)16 * L.pq_cap);
+  }
+  for (int p = 0; p < kMaxPipes; ++p) out[p].total = o;
+}
+static Layout make_layout(uint64_t batch, size_t nvox, bool with_acc) {
+  Layout Ls[kMaxPipes]; make_layouts(batch, nvox, with_acc, Ls); return Ls[0];
 }
 
 int upload_tables(psl *P) {
@@ -313,6 +321,19 @@ struct Run {
   }
 };
 
+// Adds the per-call part of `src` (ledgers, counters, totals) into `dst` (pipelines are folded on the host).
+static void merge_control(Control &dst, const Control &src) {
+  for (int sl = 0; sl < kLedgerSlots; ++sl)
+    for (int k = 0; k < 4; ++k) {
+      unsigned __int128 a = ((unsigned __int128)dst.ledger[sl][k][1] << 64) | dst.ledger[sl][k][0];
+      a += ((unsigned __int128)src.ledger[sl][k][1] << 64) | src.ledger[sl][k][0];
+      dst.ledger[sl][k][0] = (unsigned long long)a; dst.ledger[sl][k][1] = (unsigned long long)(a >> 64);
+    }
+  for (int k = 0; k < ST_COUNT; ++k) dst.stat[k] += src.stat[k];
+  dst.hw_eq = std::max(dst.hw_eq, src.hw_eq); dst.hw_pq = std::max(dst.hw_pq, src.hw_pq);
+  dst.n_accepted += src.n_accepted; dst.n_missed += src.n_missed; dst.overflow |= src.overflow;
+}
+
 static void fold_stats(const Control &c, const Run &r, mc_stats_t *s) {
   for (int k = 0; k < 4; ++k) {
     unsigned __int128 tot = 0;
@@ -344,6 +365,28 @@ static uint64_t mixed_multiplier(uint64_t N) {
   return a;
 }
 
+// Number of pipelines of a call (PSLMC_PIPELINES = 1 switches the overlap off) and their streams (created once).
+static int pipe_count(int requested) {
+  const char *e = getenv("PSLMC_PIPELINES");
+  const int n = requested > 0 ? requested : (e ? atoi(e) : kMaxPipes);
+  return std::max(1, std::min(n, kMaxPipes));
+}
+static const std::vector<cudaStream_t> *pipe_streams() {
+  static std::vector<cudaStream_t> st;
+  static int dev_of = -1;
+  int dev = 0; cudaGetDevice(&dev);
+  if (st.empty() || dev_of != dev) {
+    st.clear();
+    for (int p = 0; p < kMaxPipes; ++p) {
+      cudaStream_t s = nullptr;
+      if (cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); st.clear(); return nullptr; }
+      st.push_back(s);
+    }
+    dev_of = dev;
+  }
+  return &st;
+}
+
 // The driver proper.  All pointers inside `ph` are DEVICE pointers here.
 static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam, uint64_t N, uint64_t seed, uint64_t batch,
                     double *dose_out, const mc_opts_t *opts) {
@@ -360,92 +403,143 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
   if (dev != P->device) return fail(MC_E_INVALID_ARG, "mc_dose: psl_t was built on another device");
 
   const size_t nvox = (size_t)ph->nx * ph->ny * ph->nz;
-  const Layout L = make_layout(batch, nvox, opts->dose_acc == nullptr);
+  Layout Ls[kMaxPipes];
+  make_layouts(batch, nvox, opts->dose_acc == nullptr, Ls);
+  const Layout &L = Ls[0];
   void *ws = opts->workspace;
   if (ws) { if (opts->workspace_bytes < L.total) return fail(MC_E_WORKSPACE, "mc_dose: workspace too small (see mc_workspace_bytes)"); }
   else { int rc = scratch_get(g_scratch, L.total, &ws); if (rc) return rc; }
 
-  Run r{};
-  r.st = (cudaStream_t)opts->cuda_stream; r.ws = (char *)ws; r.L = L; r.ctl = (Control *)(r.ws + L.ctl);
-  long long *acc = opts->dose_acc ? (long long *)opts->dose_acc : (long long *)(r.ws + L.acc);
-  r.g = make_grid(*ph, acc); r.g.vox = (const uint32_t *)(r.ws + L.vox);
-  r.seed = seed; r.n_total = N; r.perm_a = mixed ? mixed_multiplier(N) : 0; r.flags = opts->flags; r.batch = batch;
-  r.fp = (unsigned long long *)opts->fingerprints; r.fp_base = hb;
-  r.dbg = (opts->flags & MC_FLAG_STATS) || opts->fingerprints;
-  r.tm.on = (opts->flags & MC_FLAG_TIMING) != 0; r.tm.st = r.st;
-  r.init_blocks();
+  // Pipelines: batches are dealt round-robin to npipe independent launch sequences, each with its own control
+  // block, particle buffer, queues and stream, all scoring into the one int64 grid.  Every transport kernel is
+  // a persistent grid that fills the GPU, so the CTAs of one pipeline's next kernel start as the other
+  // pipeline's kernel drains: the tails (lanes finishing their last, longest histories) overlap with useful
+  // work instead of leaving SMs idle.  Integer tallies keep the result bit-identical for any npipe.
+  const std::vector<cudaStream_t> *pstreams = nullptr;
+  int npipe = pipe_count(opts->pipelines);
+  if (npipe > 1 && !(pstreams = pipe_streams())) npipe = 1;
+  cudaStream_t us = (cudaStream_t)opts->cuda_stream;
+  long long *acc = opts->dose_acc ? (long long *)opts->dose_acc : (long long *)((char *)ws + L.acc);
+
+  Run pipes[kMaxPipes];
+  for (int p = 0; p < npipe; ++p) {
+    Run &r = pipes[p];
+    r.st = npipe > 1 ? (*pstreams)[p] : us; r.ws = (char *)ws; r.L = Ls[p]; r.ctl = (Control *)(r.ws + Ls[p].ctl);
+    r.g = make_grid(*ph, acc); r.g.vox = (const uint32_t *)(r.ws + L.vox);
+    r.seed = seed; r.n_total = N; r.perm_a = mixed ? mixed_multiplier(N) : 0; r.flags = opts->flags; r.batch = batch;
+    r.fp = (unsigned long long *)opts->fingerprints; r.fp_base = hb;
+    r.dbg = (opts->flags & MC_FLAG_STATS) || opts->fingerprints;
+    r.tm.on = (opts->flags & MC_FLAG_TIMING) != 0; r.tm.st = r.st;
+    if (p == 0) r.init_blocks();
+    else { for (int k = 0; k < 2; ++k) { r.blocks_photon[k] = pipes[0].blocks_photon[k]; r.blocks_electron[k] = pipes[0].blocks_electron[k]; } }
+  }
+  Run &r0 = pipes[0];
 
   std::vector<uint64_t> off(P->groups.size() + 1);
   allocate_host(*P, N, off.data());
-  unsigned long long *d_off = (unsigned long long *)(r.ws + L.off);
+  unsigned long long *d_off = (unsigned long long *)((char *)ws + L.off);
 
+  // ---- prologue on the caller's stream
   cudaEvent_t ev0, ev1;
   CUDA_TRY(cudaEventCreate(&ev0)); CUDA_TRY(cudaEventCreate(&ev1));
-  CUDA_TRY(cudaEventRecord(ev0, r.st));
-  CUDA_TRY(cudaMemsetAsync(r.ctl, 0, sizeof(Control), r.st));
-  CUDA_TRY(cudaMemcpyAsync(d_off, off.data(), sizeof(uint64_t) * off.size(), cudaMemcpyHostToDevice, r.st));
-  if (!opts->dose_acc) CUDA_TRY(cudaMemsetAsync(acc, 0, 8 * nvox, r.st));
-  r.tm.begin(MC_K_AUX);
-  k_pack_phantom<<<592, 256, 0, r.st>>>(ph->density, ph->material, nvox, (uint32_t *)(r.ws + r.L.vox), r.ctl);
-  r.build_xs(P->psr.e_min + P->psr.e_bin_width * P->n_ebin); ++r.launches[MC_K_AUX];
-  L2Window l2w; l2w.set(r.st, r.ws + L.vox, 4 * nvox);
-  r.tm.end(MC_K_AUX); ++r.launches[MC_K_AUX];
+  CUDA_TRY(cudaEventRecord(ev0, us));
+  for (int p = 0; p < npipe; ++p) CUDA_TRY(cudaMemsetAsync(pipes[p].ctl, 0, sizeof(Control), us));
+  CUDA_TRY(cudaMemcpyAsync(d_off, off.data(), sizeof(uint64_t) * off.size(), cudaMemcpyHostToDevice, us));
+  if (!opts->dose_acc) CUDA_TRY(cudaMemsetAsync(acc, 0, 8 * nvox, us));
+  Timer tm_us; tm_us.on = r0.tm.on; tm_us.st = us;
+  uint64_t launches_us[5] = {0, 0, 0, 0, 0};
+  tm_us.begin(MC_K_AUX);
+  k_pack_phantom<<<592, 256, 0, us>>>(ph->density, ph->material, nvox, (uint32_t *)((char *)ws + L.vox), r0.ctl);
+  { cudaStream_t keep = r0.st; r0.st = us; r0.build_xs(P->psr.e_min + P->psr.e_bin_width * P->n_ebin); r0.st = keep; }
+  tm_us.end(MC_K_AUX); launches_us[MC_K_AUX] += 2;
+  for (int p = 1; p < npipe; ++p) pipes[p].xs = r0.xs;
+  L2Window l2w; l2w.set(us, (char *)ws + L.vox, 4 * nvox);
+  cudaEvent_t ev_fork = nullptr, ev_join[kMaxPipes] = {nullptr, nullptr};
+  if (npipe > 1) {
+    CUDA_TRY(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
+    CUDA_TRY(cudaEventRecord(ev_fork, us));
+    for (int p = 0; p < npipe; ++p) CUDA_TRY(cudaStreamWaitEvent(pipes[p].st, ev_fork, 0));
+  }
 
-  SampleArgs sa{};
-  sa.m = source_model(*P); sa.beam = beam_xf(*beam); sa.off_g = d_off; sa.seed = seed; round_keys(seed, sa.ks); sa.n_total = N; sa.perm_a = r.perm_a;
-  sa.p0 = (float4 *)(r.ws + L.p0); sa.p1 = (float4 *)(r.ws + L.p1); sa.ctl = r.ctl; sa.fp = r.fp; sa.fp_base = hb; sa.compact = 1; sa.g = r.g; sa.stats = r.dbg ? 1 : 0;
+  SampleArgs sa[kMaxPipes];
+  for (int p = 0; p < npipe; ++p) {
+    Run &r = pipes[p]; SampleArgs &a = sa[p]; a = SampleArgs{};
+    a.m = source_model(*P); a.beam = beam_xf(*beam); a.off_g = d_off; a.seed = seed; round_keys(seed, a.ks); a.n_total = N; a.perm_a = r.perm_a;
+    a.p0 = (float4 *)(r.ws + r.L.p0); a.p1 = (float4 *)(r.ws + r.L.p1); a.ctl = r.ctl; a.fp = r.fp; a.fp_base = hb; a.compact = 1; a.g = r.g; a.stats = r.dbg ? 1 : 0;
+  }
 
   memset(&g_stats, 0, sizeof g_stats);
-  auto sample_batch = [&](uint64_t first, uint64_t count) {
+  auto sample_batch = [&](int p, uint64_t first, uint64_t count) {
+    Run &r = pipes[p];
     r.next_batch();
-    sa.first = first; sa.count = (unsigned)count;
+    sa[p].first = first; sa[p].count = (unsigned)count;
     r.tm.begin(MC_K_SAMPLE);
-    k_sample<<<(unsigned)((count + kThreads - 1) / kThreads), kThreads, 0, r.st>>>(sa);
+    k_sample<<<(unsigned)((count + kThreads - 1) / kThreads), kThreads, 0, r.st>>>(sa[p]);
     r.tm.end(MC_K_SAMPLE); ++r.launches[MC_K_SAMPLE];
   };
   const int ne = P->n_ebin;
+  uint64_t task = 0;
   if (!mixed) {
     // one sub-source type at a time, energy bins ascending, M histories per launch
     for (int s = 0; s < 3; ++s) {
       const uint64_t lo = std::max(hb, off[(size_t)s * ne]), hi = std::min(he, off[(size_t)(s + 1) * ne]);
       if (lo >= hi) continue;
       g_stats.n_hist[s] = hi - lo;
-      if (P->psr.particle_type[s] != 0 && r.pq_pending) { r.next_batch(); r.drain_photon_queue(); }   // no photon launch ahead to carry them
-      for (uint64_t first = lo; first < hi; first += batch) {
-        sample_batch(first, std::min(batch, hi - first));
+      for (uint64_t first = lo; first < hi; first += batch, ++task) {
+        const int p = (int)(task % npipe); Run &r = pipes[p];
+        if (P->psr.particle_type[s] != 0 && r.pq_pending) { r.next_batch(); r.drain_photon_queue(); }   // no photon launch ahead to carry them
+        sample_batch(p, first, std::min(batch, hi - first));
         if (P->psr.particle_type[s] == 0) r.transport_photon_batch(first);
         else r.transport_electron_buffer(first, false, &r.ctl->n_pb, &r.ctl->head_pb);
       }
     }
   } else {
     for (int s = 0; s < 3; ++s) g_stats.n_hist[s] = 0;     // mixed: per-type counts are not tracked per range
-    for (uint64_t first = hb; first < he; first += batch) {
-      sample_batch(first, std::min(batch, he - first));
+    for (uint64_t first = hb; first < he; first += batch, ++task) {
+      const int p = (int)(task % npipe); Run &r = pipes[p];
+      sample_batch(p, first, std::min(batch, he - first));
       r.transport_electron_buffer(first, false, &r.ctl->n_pb, &r.ctl->pad0);
       r.transport_photon_batch(first);
     }
     if (hb == 0 && he == N) for (int s = 0; s < 3; ++s) g_stats.n_hist[s] = off[(size_t)(s + 1) * ne] - off[(size_t)s * ne];
   }
-  r.next_batch();
-  if (r.pq_pending) { r.drain_photon_queue(); r.next_batch(); }
-  if (dose_out) {
-    r.tm.begin(MC_K_FINALISE);
-    const double inv_vn = 1.0 / (ph->dx * ph->dy * ph->dz * (double)N);
-    k_finalise<<<592, 256, 0, r.st>>>(acc, ph->density, nvox, inv_vn, dose_out);
-    r.tm.end(MC_K_FINALISE); ++r.launches[MC_K_FINALISE];
+  for (int p = 0; p < npipe; ++p) {
+    Run &r = pipes[p];
+    r.next_batch();
+    if (r.pq_pending) { r.drain_photon_queue(); r.next_batch(); }
+    if (npipe > 1) {
+      CUDA_TRY(cudaEventCreateWithFlags(&ev_join[p], cudaEventDisableTiming));
+      CUDA_TRY(cudaEventRecord(ev_join[p], r.st));
+      CUDA_TRY(cudaStreamWaitEvent(us, ev_join[p], 0));
+    }
   }
-  CUDA_TRY(cudaEventRecord(ev1, r.st));
+  if (dose_out) {
+    tm_us.begin(MC_K_FINALISE);
+    const double inv_vn = 1.0 / (ph->dx * ph->dy * ph->dz * (double)N);
+    k_finalise<<<592, 256, 0, us>>>(acc, ph->density, nvox, inv_vn, dose_out);
+    tm_us.end(MC_K_FINALISE); ++launches_us[MC_K_FINALISE];
+  }
+  CUDA_TRY(cudaEventRecord(ev1, us));
   CUDA_TRY(cudaGetLastError());
-  Control hc;
-  CUDA_TRY(cudaMemcpyAsync(&hc, r.ctl, sizeof(Control), cudaMemcpyDeviceToHost, r.st));
-  CUDA_TRY(cudaStreamSynchronize(r.st));
+  Control hc[kMaxPipes];
+  for (int p = 0; p < npipe; ++p) CUDA_TRY(cudaMemcpyAsync(&hc[p], pipes[p].ctl, sizeof(Control), cudaMemcpyDeviceToHost, us));
+  CUDA_TRY(cudaStreamSynchronize(us));
   l2w.clear();
   CUDA_TRY(cudaEventElapsedTime(&g_stats.ms_total, ev0, ev1));
   cudaEventDestroy(ev0); cudaEventDestroy(ev1);
-  r.tm.collect(g_stats.ms);
-  fold_stats(hc, r, &g_stats);
-  g_stats.n_jaw_rejected = (he - hb) - hc.n_accepted - hc.n_missed;
-  if (hc.overflow) return fail(MC_E_OVERFLOW, "mc_dose: a secondary queue overflowed; use a larger batch workspace");
+  if (ev_fork) cudaEventDestroy(ev_fork);
+  for (int p = 0; p < npipe; ++p) if (ev_join[p]) cudaEventDestroy(ev_join[p]);
+  // fold the pipelines: kernel-class times add up (they overlap in wall time), counters and ledgers sum exactly
+  tm_us.collect(g_stats.ms);
+  for (int p = 0; p < npipe; ++p) {
+    float ms[5]; pipes[p].tm.collect(ms);
+    for (int k = 0; k < 5; ++k) { g_stats.ms[k] += ms[k]; launches_us[k] += pipes[p].launches[k]; }
+    if (p > 0) merge_control(hc[0], hc[p]);
+  }
+  for (int k = 0; k < 5; ++k) r0.launches[k] = launches_us[k];
+  fold_stats(hc[0], r0, &g_stats);
+  g_stats.n_jaw_rejected = (he - hb) - hc[0].n_accepted - hc[0].n_missed;
+  if (hc[0].overflow) return fail(MC_E_OVERFLOW, "mc_dose: a secondary queue overflowed; use a larger batch workspace");
   return MC_OK;
 }
 

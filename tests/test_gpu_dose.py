@@ -82,6 +82,7 @@ def test_bitwise_identity_under_batch_order_partition(B, gpsl, cfg):
     ref_acc, ref_dose, ref_st, ref_fp = gpu_dose(B, g, dph, beam, N, seed, 1 << 16)
     for batch, opt in ((1000, {}), (33_333, {}), (1 << 20, {}), (1 << 13, dict(order=B.MC_ORDER_MIXED)),
                        (1 << 15, dict(flags=B.MC_FLAG_STATIC_LANES)), (1 << 15, dict(flags=B.MC_FLAG_STATS | B.MC_FLAG_TIMING)),
+                       (1 << 14, dict(pipelines=1)), (1 << 12, dict(pipelines=2, flags=B.MC_FLAG_TIMING)),
                        (1 << 16, dict(flags=B.MC_FLAG_STAGE_SCORING)), (1 << 12, dict(flags=B.MC_FLAG_STAGE_SCORING | B.MC_FLAG_STATS, order=B.MC_ORDER_MIXED))):
         acc, dose, st, fp = gpu_dose(B, g, dph, beam, N, seed, batch, **opt)
         assert np.array_equal(acc, ref_acc), (batch, opt)
