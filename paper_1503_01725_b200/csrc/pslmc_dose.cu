@@ -454,7 +454,7 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
   tm_us.end(MC_K_AUX); launches_us[MC_K_AUX] += 2;
   for (int p = 1; p < npipe; ++p) pipes[p].xs = r0.xs;
   L2Window l2w; l2w.set(us, (char *)ws + L.vox, 4 * nvox);
-  cudaEvent_t ev_fork = nullptr, ev_join[kMaxPipes] = {nullptr, nullptr};
+  cudaEvent_t ev_fork = nullptr, ev_join[kMaxPipes] = {};
   if (npipe > 1) {
     CUDA_TRY(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
     CUDA_TRY(cudaEventRecord(ev_fork, us));
