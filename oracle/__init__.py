@@ -66,6 +66,11 @@ def lib():
         L = C.CDLL(build())
         L.orc_psl_build.restype = C.c_void_p
         L.orc_psl_build.argtypes = [C.POINTER(_Psr), C.POINTER(_Jaws), C.c_int32]
+        L.orc_psl_build_grid.restype = C.c_void_p
+        L.orc_psl_build_grid.argtypes = [C.POINTER(_Psr), C.POINTER(_Jaws), C.c_double]
+        L.orc_psl_grid_n.argtypes = [C.c_void_p]
+        L.orc_psl_grid_x0.restype = C.c_double
+        L.orc_psl_grid_x0.argtypes = [C.c_void_p]
         L.orc_psl_free.argtypes = [C.c_void_p]
         L.orc_psl_n_groups.argtypes = [C.c_void_p]
         L.orc_psl_group_size.restype = C.c_int64
@@ -126,17 +131,25 @@ def _result(r: _Result) -> dict:
 
 
 class Psl:
-    def __init__(self, psr: dict, jaws: dict, n_sectors: int):
+    def __init__(self, psr: dict, jaws: dict, n_sectors: int, let_size: float = 0.0):
+        """n_sectors >= 1: ring-sector lets.  n_sectors == 0 and let_size > 0: the paper's Cartesian (Xbin, Ybin) lets
+        (PAPER.md:39-55); group()['ring'] / ['sector'] then hold Xbin / Ybin."""
         self._W = np.ascontiguousarray(psr["W"], np.float64)
         p = _Psr(psr["n_ebin"], psr["n_ring"], psr["e_min"], psr["e_bin_width"], psr["ring_width"], psr["z_phsp"],
                  self._W.ctypes.data_as(C.POINTER(C.c_double)), (C.c_double * 3)(*psr["sigma_src"]),
                  (C.c_double * 3)(*psr["z_src"]), (C.c_int32 * 3)(*psr["particle_type"]))
         j = _Jaws(*(jaws[k] for k in ("x1", "x2", "y1", "y2", "z_jx", "z_jy", "sad")))
-        self.h = lib().orc_psl_build(C.byref(p), C.byref(j), n_sectors)
+        if n_sectors == 0:
+            self.h = lib().orc_psl_build_grid(C.byref(p), C.byref(j), float(let_size))
+        else:
+            self.h = lib().orc_psl_build(C.byref(p), C.byref(j), n_sectors)
         if not self.h:
             raise ValueError("empty field: no active let")
         self.n_ebin, self.n_sectors = psr["n_ebin"], n_sectors
         self.n_groups = lib().orc_psl_n_groups(self.h)
+        self.let_size = float(let_size)
+        self.grid_n = lib().orc_psl_grid_n(self.h) if n_sectors == 0 else 0
+        self.grid_x0 = lib().orc_psl_grid_x0(self.h) if n_sectors == 0 else 0.0
 
     def __del__(self):
         if getattr(self, "h", None):

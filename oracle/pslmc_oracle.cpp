@@ -10,6 +10,7 @@
 // open — the paper gives no transport physics, BASELINE.json's north_star prescribes the analytic set):
 //   philox_block        DESIGN.md R1  (Philox4x32-10, Salmon et al. SC'11; keyed by seed, history)
 //   psl_build           PAPER.md:41-55 Eq. 1-2 (ring → let weights), :61-69 §2.1.2 (sampling areas)
+//   psl_build_grid      PAPER.md:39-55 steps 1-4: the paper's own Cartesian (Xbin, Ybin) let grid (NEXT-1)
 //   allocate            PAPER.md:76-80 Eq. 3 (group level, largest remainder)
 //   sample_history      PAPER.md:82-92 S3 Eq. 4-5, :94-116 S4-S5 (focal geometry reading), jaws :65/:92
 //   photon / electron   PAPER.md:161 (cut-offs); P1-P9 (Woodcock, Kahn, CSDA + Gaussian MS)
@@ -121,6 +122,9 @@ struct Psl {
   PsrParams p; std::vector<double> Wcopy; Jaws jaws; int n_sectors;
   std::vector<Group> groups;     // index = stype * n_ebin + ebin
   double rect[3][4];             // xlo, xhi, ylo, yhi per sub-source
+  // Cartesian (Xbin, Ybin) let grid of PAPER.md:39-55 (mode 1): n_xy x n_xy square lets of side let_size,
+  // lower-left corner of let (0,0) at (grid_x0, grid_x0); Group::ring holds Xbin, Group::sector holds Ybin.
+  int mode = 0, n_xy = 0; double let_size = 0, grid_x0 = 0;
 };
 
 // ---------------------------------------------------------------- psl_build
@@ -217,6 +221,60 @@ Psl *psl_build(const PsrParams &p, const Jaws &j, int n_sectors) {
   return psl;
 }
 
+// PAPER.md:55 steps 1-4: weight of the square let centred at radius r from the ring weights W[0..n_ring):
+// step 2 = linear interpolation of W_Rbin along the radius between ring centres (i + 1/2) dr, held constant
+// inside the first and beyond the last centre (A3 reading), step 3 = divide by 2 pi r.
+double grid_let_weight(const double *W, int n_ring, double dr, double r) {
+  double t = r / dr - 0.5;                        // position in units of ring centres
+  double w;
+  if (t <= 0) w = W[0];
+  else if (t >= n_ring - 1) w = W[n_ring - 1];
+  else { int i = (int)std::floor(t); double f = t - i; w = W[i] + f * (W[i + 1] - W[i]); }
+  return w / (2.0 * PI * r);
+}
+
+// PSR -> PSL on the paper's Cartesian grid (Eq. 1-2, steps 1-4) + sampling areas (:61-69).
+Psl *psl_build_grid(const PsrParams &p, const Jaws &j, double let_size) {
+  Psl *psl = new Psl;
+  psl->p = p; psl->jaws = j; psl->n_sectors = 0; psl->mode = 1; psl->let_size = let_size;
+  psl->Wcopy.assign(p.W, p.W + (size_t)3 * p.n_ebin * p.n_ring);
+  psl->p.W = psl->Wcopy.data();
+  psl->groups.resize((size_t)3 * p.n_ebin);
+  const double rmax = p.n_ring * p.ring_width;
+  const int half = (int)std::ceil(rmax / let_size);      // an even number of lets per side: no let centre on the axis
+  psl->n_xy = 2 * half; psl->grid_x0 = -half * let_size;
+  // step 4: one normalisation over all lets of all energies and sub-sources
+  double total = 0;
+  for (int s = 0; s < 3; ++s) for (int e = 0; e < p.n_ebin; ++e)
+    for (int X = 0; X < psl->n_xy; ++X) for (int Y = 0; Y < psl->n_xy; ++Y) {
+      double x = psl->grid_x0 + (X + 0.5) * let_size, y = psl->grid_x0 + (Y + 0.5) * let_size, r = std::sqrt(x * x + y * y);   // step 1
+      if (r < rmax) total += grid_let_weight(&psl->Wcopy[((size_t)s * p.n_ebin + e) * p.n_ring], p.n_ring, p.ring_width, r);
+    }
+  bool any = false;
+  for (int s = 0; s < 3; ++s) {
+    sampling_rect(p, j, s, psl->rect[s]);
+    const double *rc = psl->rect[s];
+    for (int e = 0; e < p.n_ebin; ++e) {
+      Group &g = psl->groups[(size_t)s * p.n_ebin + e];
+      g.stype = s; g.ebin = e;
+      std::vector<double> w;
+      for (int X = 0; X < psl->n_xy; ++X) for (int Y = 0; Y < psl->n_xy; ++Y) {
+        double xl = psl->grid_x0 + X * let_size, yl = psl->grid_x0 + Y * let_size;
+        double x = xl + 0.5 * let_size, y = yl + 0.5 * let_size, r = std::sqrt(x * x + y * y);
+        if (!(r < rmax)) continue;                               // outside the model's phase-space disc
+        bool overlap = xl <= rc[1] && xl + let_size >= rc[0] && yl <= rc[3] && yl + let_size >= rc[2];   // "any portion" (:69)
+        if (!overlap) continue;
+        double wl = grid_let_weight(&psl->Wcopy[((size_t)s * p.n_ebin + e) * p.n_ring], p.n_ring, p.ring_width, r) / total;
+        if (wl > 0) { g.ring.push_back((uint16_t)X); g.sector.push_back((uint16_t)Y); w.push_back(wl); }
+      }
+      g.W = 0; for (double x : w) g.W += x;
+      if (!w.empty()) { build_alias(w, g.thresh, g.alias); any = true; }
+    }
+  }
+  if (!any) { delete psl; return nullptr; }
+  return psl;
+}
+
 // Eq. 3 at group level with largest-remainder rounding (A2).
 void allocate(const Psl &psl, uint64_t N, uint64_t *off) {
   size_t G = psl.groups.size();
@@ -252,10 +310,16 @@ Sampled sample_history(const Psl &psl, const Beam &beam, const uint64_t *off, ui
   uint32_t col = (uint32_t)(m >> 32), frac = (uint32_t)m;
   uint32_t let = frac < grp.thresh[col] ? col : grp.alias[col];
   // 2. position, uniform in the let's area
-  double r0 = grp.ring[let] * p.ring_width, r1 = (grp.ring[let] + 1) * p.ring_width;
-  double r = std::sqrt(r0 * r0 + U_co(x1) * (r1 * r1 - r0 * r0));
-  double th = 2.0 * PI * ((double)grp.sector[let] + U_co(x2)) / psl.n_sectors;
-  double px = r * std::cos(th), py = r * std::sin(th), pz = p.z_phsp;
+  double px, py, pz = p.z_phsp;
+  if (psl.mode == 0) {
+    double r0 = grp.ring[let] * p.ring_width, r1 = (grp.ring[let] + 1) * p.ring_width;
+    double r = std::sqrt(r0 * r0 + U_co(x1) * (r1 * r1 - r0 * r0));
+    double th = 2.0 * PI * ((double)grp.sector[let] + U_co(x2)) / psl.n_sectors;
+    px = r * std::cos(th); py = r * std::sin(th);
+  } else {                                   // square let (Xbin, Ybin): uniform in x and in y (:82)
+    px = psl.grid_x0 + ((double)grp.ring[let] + U_co(x1)) * psl.let_size;
+    py = psl.grid_x0 + ((double)grp.sector[let] + U_co(x2)) * psl.let_size;
+  }
   // 3. energy, uniform in the bin
   double E = (p.e_min + grp.ebin * p.e_bin_width) + U_oc(x3) * p.e_bin_width;
   // 4. source point from the 2-D Gaussian of the sub-source (Eq. 4)
@@ -497,6 +561,9 @@ void orc_philox(uint64_t seed, uint64_t h, uint32_t track, uint32_t block, uint3
 uint32_t orc_child_track(uint32_t parent, uint32_t n, uint32_t c) { return child_track(parent, n, c); }
 
 void *orc_psl_build(const PsrParams *p, const Jaws *j, int32_t n_sectors) { return psl_build(*p, *j, n_sectors); }
+void *orc_psl_build_grid(const PsrParams *p, const Jaws *j, double let_size) { return psl_build_grid(*p, *j, let_size); }
+int32_t orc_psl_grid_n(const void *h) { return ((const Psl *)h)->n_xy; }
+double orc_psl_grid_x0(const void *h) { return ((const Psl *)h)->grid_x0; }
 void orc_psl_free(void *h) { delete (Psl *)h; }
 int32_t orc_psl_n_groups(const void *h) { return (int32_t)((const Psl *)h)->groups.size(); }
 int64_t orc_psl_group_size(const void *h, int32_t g) { return (int64_t)((const Psl *)h)->groups[g].ring.size(); }

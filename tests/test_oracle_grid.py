@@ -1,0 +1,138 @@
+"""Pins for the oracle's Cartesian (Xbin, Ybin) PSL grid — the paper's own let shape, Eq. 1-2,
+steps 1-4.  The sector form of psl_build is pinned in test_oracle_source.py."""
+import math
+
+import numpy as np
+import pytest
+from scipy import stats
+
+
+@pytest.fixture(scope="module")
+def c1(cfg):
+    return cfg("C1", False)
+
+
+def open_jaws(c):
+    return dict(c["jaws"], x1=-30.0, x2=30.0, y1=-30.0, y2=30.0)
+
+
+def test_grid_normalisation_and_eq2(orc, c1):
+    """Step 4: the weights of all lets of all energies and sub-sources sum to 1.  Steps 1-3 / Eq. 2: a let's weight
+    times 2 pi r is the ring weight interpolated at the let centre's radius — checked through the alias tables
+    (p_i reconstructed from thresholds) against numpy's own interpolation."""
+    psr, a = c1["psr"], 0.5
+    o = orc.Psl(psr, open_jaws(c1), 0, let_size=a)
+    assert o.grid_n == 64 and o.grid_x0 == -16.0                          # 2 ceil(16 / 0.5) lets per side, none centred on the axis
+    assert sum(o.group(g)["W"] for g in range(o.n_groups)) == pytest.approx(1.0, abs=1e-12)
+    W = np.asarray(psr["W"], np.float64).reshape(3, psr["n_ebin"], psr["n_ring"])
+    centres = (np.arange(psr["n_ring"]) + 0.5) * psr["ring_width"]
+    ref_all = {}
+    total = 0.0
+    for s in range(3):
+        for e in range(psr["n_ebin"]):
+            X, Y = np.meshgrid(np.arange(64), np.arange(64), indexing="ij")
+            x, y = -16.0 + (X + 0.5) * a, -16.0 + (Y + 0.5) * a
+            r = np.hypot(x, y)
+            w = np.where(r < 16.0, np.interp(r, centres, W[s, e]) / (2 * np.pi * r), 0.0)   # np.interp holds the end values
+            ref_all[(s, e)] = w
+            total += w.sum()
+    for s, e in ((0, 0), (0, 17), (1, 5), (2, 23)):
+        g = o.group(s * psr["n_ebin"] + e)
+        n = len(g["ring"])
+        ref = ref_all[(s, e)][g["ring"].astype(int), g["sector"].astype(int)] / total
+        assert g["W"] == pytest.approx(ref.sum(), rel=1e-12)
+        assert n == int((ref_all[(s, e)] > 0).sum())                       # every let with a centre inside the disc
+        # alias reconstruction: p_i = (thresh_i + sum over columns aliased to i of (2^32 - thresh_j)) / (n 2^32)
+        t = g["thresh"].astype(np.float64) + (g["thresh"] == 0xFFFFFFFF)
+        p = t.copy()
+        np.add.at(p, g["alias"].astype(int), 2.0 ** 32 - t)
+        p /= n * 2.0 ** 32
+        assert np.max(np.abs(p - ref / ref.sum())) < n * 2.0 ** -32 + 1e-12
+
+
+def test_grid_ring_sums_converge_to_ring_weights(orc, c1):
+    """Eq. 1: summed over the lets whose centre lies in ring i, the let weights approach the ring weight W_i as the
+    lets get small (the radial interpolation and the 1/(2 pi r) are both first-order consistent)."""
+    psr = c1["psr"]
+    W = np.asarray(psr["W"], np.float64).reshape(3, psr["n_ebin"], psr["n_ring"])
+    errs = []
+    for a in (0.5, 0.125):
+        o = orc.Psl(psr, open_jaws(c1), 0, let_size=a)
+        g = o.group(0 * psr["n_ebin"] + 4)
+        # reconstruct the per-let weights from the alias table
+        n = len(g["ring"])
+        t = g["thresh"].astype(np.float64) + (g["thresh"] == 0xFFFFFFFF)
+        p = t.copy(); np.add.at(p, g["alias"].astype(int), 2.0 ** 32 - t); p *= g["W"] / (n * 2.0 ** 32)
+        x = o.grid_x0 + (g["ring"] + 0.5) * a; y = o.grid_x0 + (g["sector"] + 0.5) * a
+        ring = np.floor(np.hypot(x, y) / psr["ring_width"]).astype(int)
+        sums = np.bincount(ring, weights=p, minlength=psr["n_ring"])
+        ref = W[0, 4] / W.sum()
+        errs.append(np.max(np.abs(sums[2:30] / ref[2:30] - 1)))
+    # (with lets as wide as the rings the number of let centres per ring fluctuates by tens of per cent: measured 0.29 -> 0.042)
+    assert errs[0] < 0.35 and errs[1] < 0.06 and errs[1] < 0.3 * errs[0], errs
+
+
+def test_grid_active_set_and_sampling(orc, c1):
+    """Active lets = squares with any portion inside the sampling rectangle, by brute force; sampled
+    positions are uniform inside their let (:82) and fall on the lets with the table's probabilities (chi-square)."""
+    psr, a = c1["psr"], 0.5
+    o = orc.Psl(psr, c1["jaws"], 0, let_size=a)
+    rect = o.rect()
+    rng = np.random.default_rng(5)
+    for s in range(3):
+        g = o.group(s * psr["n_ebin"] + 3)
+        act = set(zip(g["ring"].tolist(), g["sector"].tolist()))
+        xlo, xhi, ylo, yhi = rect[s]
+        for X in range(o.grid_n):
+            for Y in range(o.grid_n):
+                x0, y0 = o.grid_x0 + X * a, o.grid_x0 + Y * a
+                if math.hypot(x0 + a / 2, y0 + a / 2) >= 16.0:
+                    assert (X, Y) not in act
+                    continue
+                pts = np.column_stack([x0 + a * rng.random(64), y0 + a * rng.random(64)])
+                inside = ((pts[:, 0] >= xlo) & (pts[:, 0] <= xhi) & (pts[:, 1] >= ylo) & (pts[:, 1] <= yhi)).any()
+                if inside:
+                    assert (X, Y) in act                                   # a let with a point inside must be active
+                if (X, Y) in act:                                          # and an active let touches the closed rectangle
+                    assert x0 <= xhi and x0 + a >= xlo and y0 <= yhi and y0 + a >= ylo
+    # sampling: group 0 (primary, lowest energy bin) histories only
+    N = 4_000_000
+    off = o.allocate(N)
+    n0 = int(off[1])
+    rows = o.sample(c1["beams"][0], N, 9, 0, n0)
+    # undo the beam set-up (R = identity, translation by iso - (0, 0, SAD)): x, y on the phase-space plane
+    x, y = rows[:, 0] - c1["beams"][0]["iso"][0], rows[:, 1] - c1["beams"][0]["iso"][1]
+    fx, fy = (x - o.grid_x0) / a, (y - o.grid_x0) / a
+    X, Y = np.floor(fx).astype(int), np.floor(fy).astype(int)
+    assert stats.kstest(fx - X, "uniform").pvalue > 1e-3 and stats.kstest(fy - Y, "uniform").pvalue > 1e-3
+    g = o.group(0)
+    n = len(g["ring"])
+    t = g["thresh"].astype(np.float64) + (g["thresh"] == 0xFFFFFFFF)
+    p = t.copy(); np.add.at(p, g["alias"].astype(int), 2.0 ** 32 - t); p /= n * 2.0 ** 32
+    index = {(int(a_), int(b_)): i for i, (a_, b_) in enumerate(zip(g["ring"], g["sector"]))}
+    counts = np.zeros(n)
+    keys, cnt = np.unique(np.column_stack([X, Y]), axis=0, return_counts=True)
+    for (a_, b_), k in zip(keys.tolist(), cnt.tolist()):
+        counts[index[(a_, b_)]] = k                                        # a KeyError here = a sample outside the active lets
+    assert counts.sum() == n0
+    assert stats.chisquare(counts, p * n0).pvalue > 0.01
+
+
+def test_grid_and_sector_forms_describe_the_same_fluence(orc, c1):
+    """The two let shapes discretise one planar fluence f(r): radial histograms of positions sampled from each agree
+    with f(r) r dr (the closed form of the workload) to the discretisation error of 0.5 cm lets and rings."""
+    psr = c1["psr"]
+    f = lambda r: np.where(r <= 12, 1 + 0.04 * r * r, (1 + 0.04 * 144) * (16 - r) / 4)
+    edges = np.linspace(0, 15, 16)
+    mid = 0.5 * (edges[1:] + edges[:-1])
+    ref = f(mid) * mid
+    ref = ref / ref.sum()
+    for kw in (dict(n_sectors=16), dict(n_sectors=0, let_size=0.5)):
+        o = orc.Psl(psr, open_jaws(c1), **kw)
+        N = 3_000_000
+        off = o.allocate(N)
+        rows = o.sample(c1["beams"][0], N, 4, 0, int(off[24]))             # all primary histories
+        r = np.hypot(rows[:, 0], rows[:, 1])
+        h = np.histogram(r, edges)[0].astype(float)
+        h /= h.sum()
+        assert np.max(np.abs(h / ref - 1)) < 0.03, (kw, np.max(np.abs(h / ref - 1)))
