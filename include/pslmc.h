@@ -128,6 +128,14 @@ typedef struct {
  * (sub-source, energy bin) group and uploads the tables to the current CUDA device.
  * Returns MC_E_EMPTY_FIELD if no let is active.                                                 */
 int  psl_build(const psr_params_t *psr, const jaws_t *jaws, int32_t n_sectors, psl_t **out);
+/* psl_build_grid — host.  The paper's own let shape (steps 1-4): a Cartesian grid of square
+ * lets of side let_size (cm) over the phase-space disc, 2*ceil(r_max/let_size) lets per side (no let centre on
+ * the axis).  Let weight = ring weight linearly interpolated along the radius at the let centre (between ring
+ * centres; towards (0, 0) inside the first centre, constant beyond the last), divided by 2 pi r, normalised over all lets of all
+ * energies and sub-sources.  A let is active when any portion of its square lies in the sampling rectangle of
+ * its sub-source.  Everything else (alias tables, allocation, mc_dose) is as for psl_build; psl_export then
+ * reports Xbin in ring[] and Ybin in sector[].                                                    */
+int  psl_build_grid(const psr_params_t *psr, const jaws_t *jaws, double let_size, psl_t **out);
 void psl_free(psl_t *psl);
 
 /* psl_export — host.  Serialises the tables for inspection:

@@ -222,12 +222,14 @@ Psl *psl_build(const PsrParams &p, const Jaws &j, int n_sectors) {
 }
 
 // PAPER.md:55 steps 1-4: weight of the square let centred at radius r from the ring weights W[0..n_ring):
-// step 2 = linear interpolation of W_Rbin along the radius between ring centres (i + 1/2) dr, held constant
-// inside the first and beyond the last centre (A3 reading), step 3 = divide by 2 pi r.
+// step 2 = linear interpolation of W_Rbin along the radius between ring centres (i + 1/2) dr; inside the first
+// centre between (0, 0) and (dr/2, W_0) - a ring of radius 0 holds no particles, and any other anchor makes
+// W/(2 pi r) diverge on the axis - and held constant beyond the last centre (A3 reading);
+// step 3 = divide by 2 pi r.
 double grid_let_weight(const double *W, int n_ring, double dr, double r) {
   double t = r / dr - 0.5;                        // position in units of ring centres
   double w;
-  if (t <= 0) w = W[0];
+  if (t <= 0) w = W[0] * (r / (0.5 * dr));
   else if (t >= n_ring - 1) w = W[n_ring - 1];
   else { int i = (int)std::floor(t); double f = t - i; w = W[i] + f * (W[i + 1] - W[i]); }
   return w / (2.0 * PI * r);

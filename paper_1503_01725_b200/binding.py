@@ -18,7 +18,7 @@ MC_ORDER_SORTED, MC_ORDER_MIXED = 0, 1
 MC_FLAG_ELECTRONS_LOCAL, MC_FLAG_STATS, MC_FLAG_TIMING, MC_FLAG_STATIC_LANES, MC_FLAG_STAGE_SCORING = 1, 2, 4, 8, 16
 LEDGERS = ("incident", "deposited", "escaped", "jaw")
 KERNEL_CLASSES = ("sample", "photon", "electron", "finalise", "aux")
-EXPORTS = ("psl_build", "psl_free", "psl_export", "psl_allocate", "mc_workspace_bytes", "mc_dose", "mc_dose_host",
+EXPORTS = ("psl_build", "psl_build_grid", "psl_free", "psl_export", "psl_allocate", "mc_workspace_bytes", "mc_dose", "mc_dose_host",
            "mc_stats", "mc_last_error", "mc_sample_debug", "mc_transport_debug", "mc_philox_debug", "mc_xs_debug")
 
 
@@ -76,6 +76,7 @@ def lib():
                               "(or __graft_entry__.build()); there is no CPU fallback")
         L = C.CDLL(LIB_PATH)
         L.psl_build.argtypes = [C.POINTER(psr_params_t), C.POINTER(jaws_t), C.c_int32, C.POINTER(C.c_void_p)]
+        L.psl_build_grid.argtypes = [C.POINTER(psr_params_t), C.POINTER(jaws_t), C.c_double, C.POINTER(C.c_void_p)]
         L.psl_free.argtypes = [C.c_void_p]
         L.psl_free.restype = None
         L.psl_export.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
@@ -163,14 +164,18 @@ def _opts(stream=None, workspace=None, dose_acc=None, order=0, flags=0, fingerpr
 class Psl:
     """psl_build handle: active lets + alias tables, on the host and uploaded to the current device."""
 
-    def __init__(self, psr: dict, jaws: dict, n_sectors: int):
+    def __init__(self, psr: dict, jaws: dict, n_sectors: int, let_size: float = 0.0):
+        """n_sectors >= 1: ring-sector lets (psl_build); n_sectors == 0 and let_size > 0: the paper's Cartesian lets (psl_build_grid)."""
         self._W = np.ascontiguousarray(psr["W"], np.float64)
         p = psr_params_t(psr["n_ebin"], psr["n_ring"], psr["e_min"], psr["e_bin_width"], psr["ring_width"], psr["z_phsp"],
                          self._W.ctypes.data_as(C.POINTER(C.c_double)), (C.c_double * 3)(*psr["sigma_src"]),
                          (C.c_double * 3)(*psr["z_src"]), (C.c_int32 * 3)(*psr["particle_type"]))
         j = jaws_t(*(jaws[k] for k in ("x1", "x2", "y1", "y2", "z_jx", "z_jy", "sad")))
         self.h = C.c_void_p()
-        _check(lib().psl_build(C.byref(p), C.byref(j), n_sectors, C.byref(self.h)))
+        if n_sectors == 0:
+            _check(lib().psl_build_grid(C.byref(p), C.byref(j), float(let_size), C.byref(self.h)))
+        else:
+            _check(lib().psl_build(C.byref(p), C.byref(j), n_sectors, C.byref(self.h)))
         self.n_ebin, self.n_groups = psr["n_ebin"], 3 * psr["n_ebin"]
 
     def __del__(self):

@@ -103,7 +103,8 @@ static SourceModel source_model(const psl &P) {
   m.table = (const AliasEntry *)P.d_table; m.let_off = P.d_let_off; m.n_let = P.d_n_let;
   m.n_groups = (int)P.groups.size(); m.n_ebin = P.n_ebin; m.n_sectors = P.n_sectors;
   m.e_min = (float)P.psr.e_min; m.e_bin_width = (float)P.psr.e_bin_width; m.ring_width = (float)P.psr.ring_width;
-  m.z_phsp = (float)P.psr.z_phsp; m.inv_nsec = (float)(1.0 / P.n_sectors);
+  m.z_phsp = (float)P.psr.z_phsp; m.inv_nsec = P.n_sectors > 0 ? (float)(1.0 / P.n_sectors) : 0.0f;
+  m.let_mode = P.let_mode; m.grid_x0 = (float)P.grid_x0; m.let_size = (float)P.let_size;
   const jaws_t &j = P.jaws;
   for (int s = 0; s < 3; ++s) {
     m.sigma_src[s] = (float)P.psr.sigma_src[s]; m.z_src[s] = (float)P.psr.z_src[s]; m.particle_type[s] = P.psr.particle_type[s];

@@ -28,6 +28,9 @@ struct psl {
   jaws_t jaws{};
   std::vector<pslmc::HostGroup> groups;      // index = stype * n_ebin + ebin
   double rect[3][4] = {};
+  // let shape: 0 = ring sectors (ring, sector), 1 = the paper's Cartesian grid (Xbin, Ybin) of square lets
+  int let_mode = 0, n_xy = 0;
+  double let_size = 0, grid_x0 = 0;
   // device tables (uploaded once)
   int device = -1;
   void *d_table = nullptr;                   // AliasEntry[total lets]
@@ -37,6 +40,7 @@ struct psl {
 
 namespace pslmc {
 int build_host(const psr_params_t &p, const jaws_t &j, int n_sectors, psl *out);
+int build_host_grid(const psr_params_t &p, const jaws_t &j, double let_size, psl *out);
 void allocate_host(const psl &P, uint64_t N, uint64_t *off);
 int upload_tables(psl *P);                   // pslmc_dose.cu
 }  // namespace pslmc

@@ -46,6 +46,8 @@ struct SourceModel {               // read-only, uploaded once by psl_build
   const uint32_t *let_off;         // [G] first entry of group g
   const uint32_t *n_let;           // [G]
   int n_groups, n_ebin, n_sectors;
+  int let_mode;                    // 0: ring sectors; 1: Cartesian grid of square lets (entries hold Xbin, Ybin)
+  float grid_x0, let_size;
   float e_min, e_bin_width, ring_width, z_phsp, inv_nsec;
   float sigma_src[3], z_src[3];
   int particle_type[3];
@@ -123,11 +125,17 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
     const bool own = frac < e.thresh;
     const float ring = (float)(own ? e.ring_c : e.ring_a), sector = (float)(own ? e.sector_c : e.sector_a);
     // 2. position uniform in the let's area
-    const float r0 = ring * m.ring_width, r1 = (ring + 1.0f) * m.ring_width;
-    const float r = sqrtf(r0 * r0 + u_co(x1) * (r1 * r1 - r0 * r0));
-    float sn, cs;
-    sincospif(2.0f * (sector + u_co(x2)) * m.inv_nsec, &sn, &cs);
-    const float px = r * cs, py = r * sn, pz = m.z_phsp;
+    float sn, cs, px, py;
+    const float pz = m.z_phsp;
+    if (m.let_mode == 0) {
+      const float r0 = ring * m.ring_width, r1 = (ring + 1.0f) * m.ring_width;
+      const float r = sqrtf(r0 * r0 + u_co(x1) * (r1 * r1 - r0 * r0));
+      sincospif(2.0f * (sector + u_co(x2)) * m.inv_nsec, &sn, &cs);
+      px = r * cs; py = r * sn;
+    } else {                                 // square let (Xbin, Ybin) = (ring, sector) fields of the entry
+      px = m.grid_x0 + (ring + u_co(x1)) * m.let_size;
+      py = m.grid_x0 + (sector + u_co(x2)) * m.let_size;
+    }
     // 3. energy uniform in the bin
     const float E = (m.e_min + (float)ebin * m.e_bin_width) + u_oc(x3) * m.e_bin_width;
     // 4. source point on the sub-source's Gaussian (Eq. 4)

@@ -97,6 +97,67 @@ int build_host(const psr_params_t &p, const jaws_t &j, int n_sectors, psl *out) 
   return any ? MC_OK : MC_E_EMPTY_FIELD;
 }
 
+// The paper's own let shape: a Cartesian grid of square lets of side `a` over the phase-space
+// disc.  Weight of let (Xbin, Ybin), steps 1-4: radius of the let centre; ring weight at that radius by linear
+// interpolation between ring centres (towards (0, 0) inside the first centre, constant beyond the last); divided by
+// 2 pi r; one normalisation over all lets of all energies and sub-sources.  A let is active when any portion of
+// its square lies in the closed sampling rectangle (:69).  HostGroup::ring / ::sector hold Xbin / Ybin.
+static double grid_weight(const double *W, int n_ring, double dr, double r) {
+  const double t = r / dr - 0.5;
+  double w;
+  if (t <= 0) w = W[0] * (r / (0.5 * dr));             // towards (0, 0): a ring of radius 0 holds nothing
+  else if (t >= n_ring - 1) w = W[n_ring - 1];
+  else { const int i = (int)std::floor(t); const double f = t - i; w = W[i] + f * (W[i + 1] - W[i]); }
+  return w / (2.0 * kPiD * r);
+}
+
+int build_host_grid(const psr_params_t &p, const jaws_t &j, double a, psl *out) {
+  out->n_ebin = p.n_ebin; out->n_ring = p.n_ring; out->n_sectors = 0;
+  out->psr = p; out->W.assign(p.W, p.W + (size_t)3 * p.n_ebin * p.n_ring); out->psr.W = nullptr;
+  out->jaws = j;
+  out->groups.assign((size_t)3 * p.n_ebin, HostGroup());
+  const double rmax = p.n_ring * p.ring_width;
+  const int half = (int)std::ceil(rmax / a);             // even number of lets per side: no centre on the axis
+  out->let_mode = 1; out->let_size = a; out->n_xy = 2 * half; out->grid_x0 = -half * a;
+  const int n = out->n_xy;
+  // radius of every let centre, once
+  std::vector<double> rad((size_t)n * n);
+  for (int X = 0; X < n; ++X) for (int Y = 0; Y < n; ++Y) {
+    const double x = out->grid_x0 + (X + 0.5) * a, y = out->grid_x0 + (Y + 0.5) * a;
+    rad[(size_t)X * n + Y] = std::sqrt(x * x + y * y);
+  }
+  double total = 0;
+  for (int s = 0; s < 3; ++s) for (int e = 0; e < p.n_ebin; ++e) {
+    const double *Wr = &out->W[((size_t)s * p.n_ebin + e) * p.n_ring];
+    for (int X = 0; X < n; ++X) for (int Y = 0; Y < n; ++Y) {
+      const double r = rad[(size_t)X * n + Y];
+      if (r < rmax) total += grid_weight(Wr, p.n_ring, p.ring_width, r);
+    }
+  }
+  bool any = false;
+  for (int s = 0; s < 3; ++s) {
+    sampling_rect(p, j, s, out->rect[s]);
+    const double *rc = out->rect[s];
+    for (int e = 0; e < p.n_ebin; ++e) {
+      HostGroup &g = out->groups[(size_t)s * p.n_ebin + e];
+      g.stype = s; g.ebin = e;
+      const double *Wr = &out->W[((size_t)s * p.n_ebin + e) * p.n_ring];
+      std::vector<double> w;
+      for (int X = 0; X < n; ++X) for (int Y = 0; Y < n; ++Y) {
+        const double r = rad[(size_t)X * n + Y];
+        if (!(r < rmax)) continue;
+        const double xl = out->grid_x0 + X * a, yl = out->grid_x0 + Y * a;
+        if (!(xl <= rc[1] && xl + a >= rc[0] && yl <= rc[3] && yl + a >= rc[2])) continue;
+        const double wl = grid_weight(Wr, p.n_ring, p.ring_width, r) / total;
+        if (wl > 0) { g.ring.push_back((uint16_t)X); g.sector.push_back((uint16_t)Y); w.push_back(wl); }
+      }
+      g.W = 0; for (double x : w) g.W += x;
+      if (!w.empty()) { alias_table(w, g.thresh, g.alias); any = true; }
+    }
+  }
+  return any ? MC_OK : MC_E_EMPTY_FIELD;
+}
+
 // Eq. 3 at group level, largest-remainder rounding, ties to the lower group index.
 void allocate_host(const psl &P, uint64_t N, uint64_t *off) {
   const size_t G = P.groups.size();
@@ -132,6 +193,24 @@ extern "C" int psl_build(const psr_params_t *psr, const jaws_t *jaws, int32_t n_
   psl *P = new psl();
   int rc = build_host(*psr, *jaws, n_sectors, P);
   if (rc != MC_OK) { delete P; return fail(rc, "psl_build: no let is active for this jaw setting"); }
+  rc = upload_tables(P);
+  if (rc != MC_OK) { psl_free(P); return rc; }
+  *out = P;
+  return MC_OK;
+}
+
+extern "C" int psl_build_grid(const psr_params_t *psr, const jaws_t *jaws, double let_size, psl_t **out) {
+  if (!psr || !jaws || !out || !psr->W || psr->n_ebin < 1 || psr->n_ring < 1 || psr->n_ring > 65535 || 3 * psr->n_ebin > 159 ||
+      !(jaws->x1 < jaws->x2) || !(jaws->y1 < jaws->y2) || !(psr->ring_width > 0) || !(psr->e_bin_width > 0) || !(let_size > 0) ||
+      2.0 * std::ceil(psr->n_ring * psr->ring_width / let_size) > 4096.0)
+    return fail(MC_E_INVALID_ARG, "psl_build_grid: invalid argument");
+  for (int s = 0; s < 3; ++s)
+    if (!(psr->z_phsp > psr->z_src[s]) || !(jaws->z_jx > psr->z_src[s]) || !(jaws->z_jy > psr->z_src[s]) || psr->sigma_src[s] < 0 ||
+        (psr->particle_type[s] != 0 && psr->particle_type[s] != 1))
+      return fail(MC_E_INVALID_ARG, "psl_build_grid: sub-source geometry invalid");
+  psl *P = new psl();
+  int rc = build_host_grid(*psr, *jaws, let_size, P);
+  if (rc != MC_OK) { delete P; return fail(rc, "psl_build_grid: no let is active for this jaw setting"); }
   rc = upload_tables(P);
   if (rc != MC_OK) { psl_free(P); return rc; }
   *out = P;

@@ -33,7 +33,8 @@ def test_grid_normalisation_and_eq2(orc, c1):
             X, Y = np.meshgrid(np.arange(64), np.arange(64), indexing="ij")
             x, y = -16.0 + (X + 0.5) * a, -16.0 + (Y + 0.5) * a
             r = np.hypot(x, y)
-            w = np.where(r < 16.0, np.interp(r, centres, W[s, e]) / (2 * np.pi * r), 0.0)   # np.interp holds the end values
+            # np.interp with the extra node (0, 0): towards the axis the ring weight goes to zero; the last value is held
+            w = np.where(r < 16.0, np.interp(r, np.concatenate([[0.0], centres]), np.concatenate([[0.0], W[s, e]])) / (2 * np.pi * r), 0.0)
             ref_all[(s, e)] = w
             total += w.sum()
     for s, e in ((0, 0), (0, 17), (1, 5), (2, 23)):
