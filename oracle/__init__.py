@@ -71,6 +71,7 @@ def lib():
         L.orc_psl_grid_n.argtypes = [C.c_void_p]
         L.orc_psl_grid_x0.restype = C.c_double
         L.orc_psl_grid_x0.argtypes = [C.c_void_p]
+        L.orc_psl_set_direction.argtypes = [C.c_void_p, C.c_int32, C.c_int32] + [C.c_void_p] * 4
         L.orc_psl_free.argtypes = [C.c_void_p]
         L.orc_psl_n_groups.argtypes = [C.c_void_p]
         L.orc_psl_group_size.restype = C.c_int64
@@ -155,6 +156,13 @@ class Psl:
         if getattr(self, "h", None):
             lib().orc_psl_free(self.h)
             self.h = None
+
+    def set_direction_model(self, stype: int, c, mu, sigma_a, sigma_b):
+        """Eq. 6 / Eq. 7: arrays [n_ebin][n_ring][K] of component weights, means of alpha, sigmas."""
+        arrs = [np.ascontiguousarray(a, np.float64) for a in (c, mu, sigma_a, sigma_b)]
+        K = arrs[0].shape[-1]
+        assert all(a.shape == arrs[0].shape for a in arrs)
+        lib().orc_psl_set_direction(self.h, stype, K, *[_ptr(a) for a in arrs])
 
     def group(self, g: int) -> dict:
         n = lib().orc_psl_group_size(self.h, g)

@@ -12,7 +12,7 @@
 //   psl_build           PAPER.md:41-55 Eq. 1-2 (ring → let weights), :61-69 §2.1.2 (sampling areas)
 //   psl_build_grid      PAPER.md:39-55 steps 1-4: the paper's own Cartesian (Xbin, Ybin) let grid (NEXT-1)
 //   allocate            PAPER.md:76-80 Eq. 3 (group level, largest remainder)
-//   sample_history      PAPER.md:82-92 S3 Eq. 4-5, :94-116 S4-S5 (focal geometry reading), jaws :65/:92
+//   sample_history      PAPER.md:82-92 S3 Eq. 4-5, :94-116 S4-S5 (focal geometry reading, or Eq. 6-7 as printed: NEXT-2), jaws :65/:92
 //   photon / electron   PAPER.md:161 (cut-offs); P1-P9 (Woodcock, Kahn, CSDA + Gaussian MS)
 //   deposit / ledgers   DESIGN.md S1 (int64 fixed point, 2^-32 MeV)
 //   fingerprints        DESIGN.md F1
@@ -125,6 +125,10 @@ struct Psl {
   // Cartesian (Xbin, Ybin) let grid of PAPER.md:39-55 (mode 1): n_xy x n_xy square lets of side let_size,
   // lower-left corner of let (0,0) at (grid_x0, grid_x0); Group::ring holds Xbin, Group::sector holds Ybin.
   int mode = 0, n_xy = 0; double let_size = 0, grid_x0 = 0;
+  // Direction models of PAPER.md:94-116 (Eq. 6: K Gaussians in (alpha, beta) per (energy bin, ring); Eq. 7: K = 1,
+  // mean 0), one per sub-source, K = 0 = the focal-geometry model.  Arrays [n_ebin][n_ring][K]; P = the cumulative
+  // look-up table P_{i,k} = sum_{j<=k} c_{i,j} / sum_{j<=K} c_{i,j}  (:107 with the denominator read as the full sum).
+  struct DirModel { int K = 0; std::vector<double> P, mu, sa, sb; } dir[3];
 };
 
 // ---------------------------------------------------------------- psl_build
@@ -324,8 +328,43 @@ Sampled sample_history(const Psl &psl, const Beam &beam, const uint64_t *off, ui
   }
   // 3. energy, uniform in the bin
   double E = (p.e_min + grp.ebin * p.e_bin_width) + U_oc(x3) * p.e_bin_width;
-  // 4. source point from the 2-D Gaussian of the sub-source (Eq. 4)
   int s = grp.stype;
+  if (psl.dir[s].K > 0) {
+    // S4 / S5: direction from the Gaussian mixture of the PSR the position falls in
+    const Psl::DirModel &dm = psl.dir[s];
+    uint32_t y2 = st.next();
+    double r = std::sqrt(px * px + py * py);
+    int i = (int)std::floor(r / p.ring_width); if (i > p.n_ring - 1) i = p.n_ring - 1;      // ring index of the position (:94)
+    size_t base = ((size_t)grp.ebin * p.n_ring + i) * dm.K;
+    double t = U_co(y0); int k = 0;
+    while (k < dm.K - 1 && t >= dm.P[base + k]) ++k;                                         // sequential search of P_{i,k} (:107)
+    double rho_n = std::sqrt(-2.0 * std::log(U_oc(y1))), psi = 2.0 * PI * U_co(y2);
+    double alpha = dm.mu[base + k] + dm.sa[base + k] * rho_n * std::cos(psi);                // Eq. 6 / Eq. 7
+    double beta = dm.sb[base + k] * rho_n * std::sin(psi);
+    const double LIM = 1.5;                                                                  // keep tan() finite
+    alpha = std::fmax(-LIM, std::fmin(LIM, alpha)); beta = std::fmax(-LIM, std::fmin(LIM, beta));
+    double ul = std::tan(alpha), vl = std::tan(beta), wl = 1.0;                              // alpha = atan(u/w), beta = atan(v/w)
+    double nl = std::sqrt(ul * ul + vl * vl + wl * wl); ul /= nl; vl /= nl; wl /= nl;
+    double th = std::atan2(py, px);                                                          // local (u radial) -> global (:92)
+    double dx = ul * std::cos(th) - vl * std::sin(th), dy = ul * std::sin(th) + vl * std::cos(th), dz = wl;
+    // jaw rejection on the jaws' upper surfaces (:103): the ray from p along d at each jaw plane
+    const Jaws &j = psl.jaws;
+    double xj = px + dx / dz * (j.z_jx - pz), yj = py + dy / dz * (j.z_jy - pz);
+    bool pass = xj >= j.x1 * j.z_jx / j.sad && xj <= j.x2 * j.z_jx / j.sad &&
+                yj >= j.y1 * j.z_jy / j.sad && yj <= j.y2 * j.z_jy / j.sad;
+    const double *R = beam.R;
+    double bx = px, by = py, bz = pz - beam.sad;
+    Sampled o;
+    o.x = beam.iso[0] + R[0] * bx + R[1] * by + R[2] * bz;
+    o.y = beam.iso[1] + R[3] * bx + R[4] * by + R[5] * bz;
+    o.z = beam.iso[2] + R[6] * bx + R[7] * by + R[8] * bz;
+    o.u = R[0] * dx + R[1] * dy + R[2] * dz;
+    o.v = R[3] * dx + R[4] * dy + R[5] * dz;
+    o.w = R[6] * dx + R[7] * dy + R[8] * dz;
+    o.E = E; o.group = (int)g; o.rejected = !pass;
+    return o;
+  }
+  // 4. source point from the 2-D Gaussian of the sub-source (Eq. 4)
   double rho = p.sigma_src[s] * std::sqrt(-2.0 * std::log(U_oc(y0)));
   double psi = 2.0 * PI * U_co(y1);
   double qx = rho * std::cos(psi), qy = rho * std::sin(psi), qz = p.z_src[s];
@@ -563,6 +602,16 @@ void orc_philox(uint64_t seed, uint64_t h, uint32_t track, uint32_t block, uint3
 uint32_t orc_child_track(uint32_t parent, uint32_t n, uint32_t c) { return child_track(parent, n, c); }
 
 void *orc_psl_build(const PsrParams *p, const Jaws *j, int32_t n_sectors) { return psl_build(*p, *j, n_sectors); }
+// Eq. 6 / Eq. 7 parameters of one sub-source: c, mu, sigma_alpha, sigma_beta as [n_ebin][n_ring][K]; K = 0 switches back.
+void orc_psl_set_direction(void *h, int32_t stype, int32_t K, const double *c, const double *mu, const double *sa, const double *sb) {
+  Psl &psl = *(Psl *)h; Psl::DirModel &dm = psl.dir[stype];
+  dm.K = K; size_t n = (size_t)psl.p.n_ebin * psl.p.n_ring * (K > 0 ? K : 0);
+  dm.P.assign(n, 0); dm.mu.assign(mu, mu + n); dm.sa.assign(sa, sa + n); dm.sb.assign(sb, sb + n);
+  for (size_t b = 0; b < n; b += K) {
+    double tot = 0, run = 0; for (int k = 0; k < K; ++k) tot += c[b + k];
+    for (int k = 0; k < K; ++k) { run += c[b + k]; dm.P[b + k] = run / tot; }
+  }
+}
 void *orc_psl_build_grid(const PsrParams *p, const Jaws *j, double let_size) { return psl_build_grid(*p, *j, let_size); }
 int32_t orc_psl_grid_n(const void *h) { return ((const Psl *)h)->n_xy; }
 double orc_psl_grid_x0(const void *h) { return ((const Psl *)h)->grid_x0; }

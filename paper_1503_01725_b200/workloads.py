@@ -78,6 +78,27 @@ def psr_model(n_ebin: int, n_ring: int) -> dict:
                 sigma_src=SIGMA_SRC, z_src=Z_SRC, particle_type=PARTICLE_TYPE)
 
 
+def direction_model(stype: int, n_ebin: int, n_ring: int) -> dict:
+    """Synthetic parameters of the paper's direction models: Eq. 6, K = 3 Gaussians in
+    (alpha, beta) per (energy bin, ring) for the scattered photons (stype 1); Eq. 7, one zero-mean Gaussian for the
+    electrons (stype 2).  The fitted TrueBeam tables are not available; these follow the geometry of three extended
+    virtual sources at z = 12, 25, 45 cm seen from the ring centre, narrowing with energy.  Arrays [n_ebin][n_ring][K]."""
+    e = (np.arange(n_ebin) + 0.5) / n_ebin                                  # bin centre / E_max
+    r = (np.arange(n_ring) + 0.5) * (R_MAX / n_ring)
+    if stype == 1:
+        zk = np.array([12.0, 25.0, 45.0]); size = np.array([1.5, 2.5, 4.0]); wk = np.array([0.55, 0.30, 0.15])
+        c = np.broadcast_to(wk, (n_ebin, n_ring, 3)) * (1.0 + 0.2 * e[:, None, None] * np.array([1.0, 0.0, -1.0]))
+        mu = np.broadcast_to(np.arctan(r[:, None] / (Z_PHSP - zk)[None, :]), (n_ebin, n_ring, 3))
+        sig = (size / (Z_PHSP - zk))[None, None, :] * (1.0 - 0.3 * e[:, None, None]) * np.ones((1, n_ring, 1))
+        return dict(c=np.ascontiguousarray(c), mu=np.ascontiguousarray(mu), sigma_a=np.ascontiguousarray(sig),
+                    sigma_b=np.ascontiguousarray(0.8 * sig))
+    if stype == 2:
+        sig = 0.06 * (1.0 - 0.4 * e[:, None, None]) * (1.0 + 0.02 * r[None, :, None])
+        one = np.ones((n_ebin, n_ring, 1))
+        return dict(c=one, mu=0.0 * one, sigma_a=np.ascontiguousarray(sig), sigma_b=np.ascontiguousarray(sig))
+    raise ValueError("the primary sub-source keeps the focal model (Eq. 4-5)")
+
+
 def jaws(field_x: float, field_y: float | None = None) -> dict:
     fy = field_x if field_y is None else field_y
     return dict(x1=-field_x / 2, x2=field_x / 2, y1=-fy / 2, y2=fy / 2, z_jx=Z_JX, z_jy=Z_JY, sad=SAD)
