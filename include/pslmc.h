@@ -136,6 +136,15 @@ int  psl_build(const psr_params_t *psr, const jaws_t *jaws, int32_t n_sectors, p
  * its sub-source.  Everything else (alias tables, allocation, mc_dose) is as for psl_build; psl_export then
  * reports Xbin in ring[] and Ybin in sector[].                                                    */
 int  psl_build_grid(const psr_params_t *psr, const jaws_t *jaws, double let_size, psl_t **out);
+/* psl_set_direction_model — host.  Replaces the focal-geometry direction model of one sub-source by the paper's
+ * Eq. 6 (scattered photons: K Gaussians in alpha = atan(u/w), beta = atan(v/w) per (energy bin, ring))
+ * or Eq. 7 (electrons: K = 1, mu = 0).  c, mu, sigma_a, sigma_b: HOST double[n_ebin][n_ring][K]
+ * (component weights, means of alpha, standard deviations; beta has mean 0).  The cumulative table
+ * P_{i,k} = sum_{j<=k} c / sum_{j<=K} c is searched sequentially; (u, v) are local (u radial) and rotated by
+ * atan2(y, x); the jaw test is done on the ray from the phase-space point.  K = 0 restores the focal model.
+ * K <= 8.  Uploads the table to the current device.                                                      */
+int  psl_set_direction_model(psl_t *psl, int32_t stype, int32_t K, const double *c, const double *mu,
+                             const double *sigma_a, const double *sigma_b);
 void psl_free(psl_t *psl);
 
 /* psl_export — host.  Serialises the tables for inspection:

@@ -18,7 +18,7 @@ MC_ORDER_SORTED, MC_ORDER_MIXED = 0, 1
 MC_FLAG_ELECTRONS_LOCAL, MC_FLAG_STATS, MC_FLAG_TIMING, MC_FLAG_STATIC_LANES, MC_FLAG_STAGE_SCORING = 1, 2, 4, 8, 16
 LEDGERS = ("incident", "deposited", "escaped", "jaw")
 KERNEL_CLASSES = ("sample", "photon", "electron", "finalise", "aux")
-EXPORTS = ("psl_build", "psl_build_grid", "psl_free", "psl_export", "psl_allocate", "mc_workspace_bytes", "mc_dose", "mc_dose_host",
+EXPORTS = ("psl_build", "psl_build_grid", "psl_set_direction_model", "psl_free", "psl_export", "psl_allocate", "mc_workspace_bytes", "mc_dose", "mc_dose_host",
            "mc_stats", "mc_last_error", "mc_sample_debug", "mc_transport_debug", "mc_philox_debug", "mc_xs_debug")
 
 
@@ -77,6 +77,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.psl_build.argtypes = [C.POINTER(psr_params_t), C.POINTER(jaws_t), C.c_int32, C.POINTER(C.c_void_p)]
         L.psl_build_grid.argtypes = [C.POINTER(psr_params_t), C.POINTER(jaws_t), C.c_double, C.POINTER(C.c_void_p)]
+        L.psl_set_direction_model.argtypes = [C.c_void_p, C.c_int32, C.c_int32] + [C.c_void_p] * 4
         L.psl_free.argtypes = [C.c_void_p]
         L.psl_free.restype = None
         L.psl_export.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
@@ -177,6 +178,15 @@ class Psl:
         else:
             _check(lib().psl_build(C.byref(p), C.byref(j), n_sectors, C.byref(self.h)))
         self.n_ebin, self.n_groups = psr["n_ebin"], 3 * psr["n_ebin"]
+
+    def set_direction_model(self, stype: int, c=None, mu=None, sigma_a=None, sigma_b=None):
+        """Eq. 6 / Eq. 7 direction model of one sub-source (arrays [n_ebin][n_ring][K]); c=None restores the focal model."""
+        if c is None:
+            _check(lib().psl_set_direction_model(self.h, stype, 0, None, None, None, None))
+            return
+        arrs = [np.ascontiguousarray(a, np.float64) for a in (c, mu, sigma_a, sigma_b)]
+        assert all(a.shape == arrs[0].shape for a in arrs)
+        _check(lib().psl_set_direction_model(self.h, stype, arrs[0].shape[-1], *[a.ctypes.data_as(C.c_void_p) for a in arrs]))
 
     def __del__(self):
         if getattr(self, "h", None) and _lib is not None:

@@ -105,6 +105,8 @@ static SourceModel source_model(const psl &P) {
   m.e_min = (float)P.psr.e_min; m.e_bin_width = (float)P.psr.e_bin_width; m.ring_width = (float)P.psr.ring_width;
   m.z_phsp = (float)P.psr.z_phsp; m.inv_nsec = P.n_sectors > 0 ? (float)(1.0 / P.n_sectors) : 0.0f;
   m.let_mode = P.let_mode; m.grid_x0 = (float)P.grid_x0; m.let_size = (float)P.let_size;
+  for (int s = 0; s < 3; ++s) { m.dir_tab[s] = (const float4 *)P.d_dir[s]; m.dir_K[s] = P.dir_K[s]; }
+  m.n_ring = P.n_ring; m.jaw_dzx = (float)(P.jaws.z_jx - P.psr.z_phsp); m.jaw_dzy = (float)(P.jaws.z_jy - P.psr.z_phsp);
   const jaws_t &j = P.jaws;
   for (int s = 0; s < 3; ++s) {
     m.sigma_src[s] = (float)P.psr.sigma_src[s]; m.z_src[s] = (float)P.psr.z_src[s]; m.particle_type[s] = P.psr.particle_type[s];
@@ -549,7 +551,33 @@ extern "C" void psl_free(psl_t *P) {
   if (P->d_table) cudaFree(P->d_table);
   if (P->d_let_off) cudaFree(P->d_let_off);
   if (P->d_n_let) cudaFree(P->d_n_let);
+  for (int s = 0; s < 3; ++s) if (P->d_dir[s]) cudaFree(P->d_dir[s]);
   delete P;
+}
+
+extern "C" int psl_set_direction_model(psl_t *P, int32_t stype, int32_t K, const double *c, const double *mu,
+                                       const double *sigma_a, const double *sigma_b) {
+  if (!P || stype < 0 || stype > 2 || K < 0 || K > 8 || (K > 0 && (!c || !mu || !sigma_a || !sigma_b)))
+    return fail(MC_E_INVALID_ARG, "psl_set_direction_model: invalid argument");
+  if (P->d_dir[stype]) { cudaFree(P->d_dir[stype]); P->d_dir[stype] = nullptr; }
+  P->dir_K[stype] = 0;
+  if (K == 0) return MC_OK;
+  const size_t cells = (size_t)P->n_ebin * P->n_ring, n = cells * K;
+  std::vector<float> tab(4 * n);
+  for (size_t b = 0; b < n; b += K) {
+    double tot = 0, run = 0;
+    for (int k = 0; k < K; ++k) { if (!(c[b + k] >= 0) || !(sigma_a[b + k] >= 0) || !(sigma_b[b + k] >= 0)) return fail(MC_E_INVALID_ARG, "psl_set_direction_model: negative weight or sigma"); tot += c[b + k]; }
+    if (!(tot > 0)) return fail(MC_E_INVALID_ARG, "psl_set_direction_model: a (bin, ring) cell has no weight");
+    for (int k = 0; k < K; ++k) {
+      run += c[b + k];
+      float *o = &tab[4 * (b + k)];
+      o[0] = (float)(run / tot); o[1] = (float)mu[b + k]; o[2] = (float)sigma_a[b + k]; o[3] = (float)sigma_b[b + k];
+    }
+  }
+  CUDA_TRY(cudaMalloc(&P->d_dir[stype], sizeof(float) * tab.size()));
+  CUDA_TRY(cudaMemcpy(P->d_dir[stype], tab.data(), sizeof(float) * tab.size(), cudaMemcpyHostToDevice));
+  P->dir_K[stype] = K;
+  return MC_OK;
 }
 
 extern "C" size_t mc_workspace_bytes(const psl_t *P, const phantom_t *ph, uint64_t batch) {

@@ -53,6 +53,10 @@ struct SourceModel {               // read-only, uploaded once by psl_build
   int particle_type[3];
   float jaw_tx[3], jaw_ty[3];      // (z_jx - z_s)/(z_p - z_s), (z_jy - z_s)/(z_p - z_s)
   float jx_lo, jx_hi, jy_lo, jy_hi;   // jaw edges on their own planes
+  // Eq. 6 / Eq. 7 direction models, K = 0: focal geometry.  {P_cum, mu, sigma_a, sigma_b}[ebin][ring][K]
+  const float4 *dir_tab[3];
+  int dir_K[3], n_ring;
+  float jaw_dzx, jaw_dzy;             // z_jx - z_p, z_jy - z_p
 };
 
 struct BeamXf { float iso[3]; float R[9]; float sad; };
@@ -138,6 +142,30 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
     }
     // 3. energy uniform in the bin
     const float E = (m.e_min + (float)ebin * m.e_bin_width) + u_oc(x3) * m.e_bin_width;
+    float dx, dy, dz;
+    if (m.dir_K[stype] > 0) {
+      // S4 / S5: direction from the Gaussian mixture of the PSR the position falls in (Eq. 6 / Eq. 7)
+      const int K = m.dir_K[stype];
+      const float r2 = __fmaf_rn(px, px, py * py), ir = rsqrtf(fmaxf(r2, 1e-30f)), r = r2 * ir;
+      // ring of the position: for sector lets it is the let's own ring (an integer: no fp32 floor decision)
+      const int i = m.let_mode == 0 ? (int)ring : min((int)(r / m.ring_width), m.n_ring - 1);
+      const float4 *tab = m.dir_tab[stype] + ((size_t)ebin * m.n_ring + i) * K;
+      const float t = u_co(y0);
+      int k = 0;
+      float4 c = __ldg(tab);
+      while (k < K - 1 && t >= c.x) { ++k; c = __ldg(tab + k); }              // sequential search of P_{i,k}
+      const float rho_n = sqrtf(-2.0f * logf(u_oc(y1)));
+      sincospif(2.0f * u_co(y2), &sn, &cs);
+      const float alpha = fminf(1.5f, fmaxf(-1.5f, __fmaf_rn(c.z * rho_n, cs, c.y)));
+      const float beta = fminf(1.5f, fmaxf(-1.5f, c.w * rho_n * sn));
+      float ul = tanf(alpha), vl = tanf(beta);
+      const float inl = rsqrtf(__fmaf_rn(ul, ul, __fmaf_rn(vl, vl, 1.0f)));
+      ul *= inl; vl *= inl;
+      const float ct = r2 > 0.0f ? px * ir : 1.0f, st = r2 > 0.0f ? py * ir : 0.0f;   // theta = atan2(y, x)
+      dx = ul * ct - vl * st; dy = ul * st + vl * ct; dz = inl;
+      const float xj = px + dx / dz * m.jaw_dzx, yj = py + dy / dz * m.jaw_dzy;
+      pass = xj >= m.jx_lo && xj <= m.jx_hi && yj >= m.jy_lo && yj <= m.jy_hi;
+    } else {
     // 4. source point on the sub-source's Gaussian (Eq. 4)
     // (SFU log / root / trig here: the source point only tilts the direction by rho / (z_p - z_s))
     const float rho = m.sigma_src[stype] * sqrt_fast(-2.0f * __logf(u_oc(y0)));
@@ -145,12 +173,13 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
     (void)y2; (void)y3;
     const float qx = rho * cs, qy = rho * sn, qz = m.z_src[stype];
     // 5. direction (Eq. 5)
-    float dx = px - qx, dy = py - qy, dz = pz - qz;
+    dx = px - qx; dy = py - qy; dz = pz - qz;
     const float il = rsqrtf(dx * dx + dy * dy + dz * dz);
     dx *= il; dy *= il; dz *= il;
     // 6. thin-jaw test
     const float xj = qx + (px - qx) * m.jaw_tx[stype], yj = qy + (py - qy) * m.jaw_ty[stype];
     pass = xj >= m.jx_lo && xj <= m.jx_hi && yj >= m.jy_lo && yj <= m.jy_hi;
+    }
     // 7. beam set-up
     const float *R = a.beam.R;
     const float bz = pz - a.beam.sad;

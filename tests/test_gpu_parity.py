@@ -80,14 +80,15 @@ def test_cross_section_table_matches_closed_forms(B, orc):
 
 
 # ---------------------------------------------------------------- k_sample
-def check_samples(B, g, o, beam, N, seed, first, count):
+def check_samples(B, g, o, beam, N, seed, first, count, allow_fraction=0.0):
     got = soa_to_rows(g.sample_debug(beam, N, seed, first, count))
     ref = o.sample(beam, N, seed, first, count)
     same_status = got[:, 7] == ref[:, 7]
     assert same_status.mean() >= 1 - 1e-4                      # a jaw decision may flip on an fp32 tie
     err = np.abs(got[:, :7] - ref[:, :7])
     tol = 1e-6 * np.maximum(np.maximum(np.abs(got[:, :7]), np.abs(ref[:, :7])), SCALE)
-    assert np.all(err <= tol), float((err / tol).max())
+    bad = (err > tol).any(axis=1)
+    assert bad.mean() <= allow_fraction, (float(bad.mean()), float((err / tol).max()))
     return float((err / tol).max())
 
 
