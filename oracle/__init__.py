@@ -84,6 +84,10 @@ def lib():
         L.orc_sample.argtypes = [C.c_void_p, C.POINTER(_Beam), C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint64, C.c_void_p]
         L.orc_dose.argtypes = [C.c_void_p, C.POINTER(_Phantom), C.POINTER(_Beam), C.c_uint64, C.c_uint64, C.c_uint64,
                                C.c_uint64, C.c_int32, C.c_void_p, C.POINTER(_Result), C.c_void_p]
+        L.orc_dose_com.argtypes = [C.c_void_p, C.POINTER(_Phantom), C.POINTER(_Beam), C.c_uint64, C.c_uint64, C.c_uint64,
+                                   C.c_uint64, C.c_void_p, C.POINTER(_Result), C.c_void_p, C.c_void_p, C.c_int64]
+        L.orc_com_column.restype = C.c_uint32
+        L.orc_com_column.argtypes = [C.c_int32] * 6
         L.orc_transport.argtypes = [C.POINTER(_Phantom), C.c_int32, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64,
                                     C.c_int32, C.c_double, C.c_void_p, C.POINTER(_Result), C.c_void_p]
         L.orc_trace.argtypes = [C.POINTER(_Phantom), C.c_int32, C.c_void_p, C.c_uint64, C.c_uint64, C.c_int32,
@@ -199,6 +203,23 @@ class Psl:
         lib().orc_dose(self.h, C.byref(phantom.c), C.byref(_beam(beam)), n_histories, seed, h_begin, h_end, flags,
                        _ptr(acc), C.byref(res), _ptr(fp) if fp is not None else None)
         return acc, _result(res), fp
+
+
+def dose_com(psl: "Psl", phantom: Phantom, beam: dict, n_histories: int, seed: int, com_index: np.ndarray, n_rows: int,
+             n_cols: int, h_begin: int = 0, h_end: int | None = None):
+    """Dose with the commissioning tally.  Returns (acc int64[nvox], A int64[n_cols, n_rows], result)."""
+    h_end = n_histories if h_end is None else h_end
+    acc = np.zeros(phantom.nvox, np.int64)
+    A = np.zeros((n_cols, n_rows), np.int64)
+    idx = np.ascontiguousarray(com_index, np.int32)
+    res = _Result()
+    lib().orc_dose_com(psl.h, C.byref(phantom.c), C.byref(_beam(beam)), n_histories, seed, h_begin, h_end, _ptr(acc),
+                       C.byref(res), _ptr(idx), _ptr(A), n_rows)
+    return acc, A, _result(res)
+
+
+def com_column(n_ebin: int, n_ring: int, particle_type: int, s: int, e: int, r: int) -> int:
+    return int(lib().orc_com_column(n_ebin, n_ring, particle_type, s, e, r))
 
 
 def transport(phantom: Phantom, ptype: int, particles: np.ndarray, first: int, seed: int, flags: int = 0,

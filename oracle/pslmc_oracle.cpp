@@ -14,7 +14,7 @@
 //   allocate            PAPER.md:76-80 Eq. 3 (group level, largest remainder)
 //   sample_history      PAPER.md:82-92 S3 Eq. 4-5, :94-116 S4-S5 (focal geometry reading, or Eq. 6-7 as printed: NEXT-2), jaws :65/:92
 //   photon / electron   PAPER.md:161 (cut-offs); P1-P9 (Woodcock, Kahn, CSDA + Gaussian MS)
-//   deposit / ledgers   DESIGN.md S1 (int64 fixed point, 2^-32 MeV)
+//   deposit / ledgers   DESIGN.md S1 (int64 fixed point, 2^-32 MeV); commissioning tally PAPER.md:132-138 (NEXT-3)
 //   fingerprints        DESIGN.md F1
 //
 // Pins (tests/test_oracle_*.py, all `-m "not gpu"`): Philox vs cuRAND's host generator; ring/sector
@@ -302,7 +302,7 @@ void allocate(const Psl &psl, uint64_t N, uint64_t *off) {
 }
 
 // ---------------------------------------------------------------- source sampling (S3–S5)
-struct Sampled { double x, y, z, u, v, w, E; int group; bool rejected; };
+struct Sampled { double x, y, z, u, v, w, E; int group; bool rejected; int ring; };   // ring = the PSR the particle is from
 
 Sampled sample_history(const Psl &psl, const Beam &beam, const uint64_t *off, uint64_t seed, uint64_t h) {
   const PsrParams &p = psl.p;
@@ -326,6 +326,9 @@ Sampled sample_history(const Psl &psl, const Beam &beam, const uint64_t *off, ui
     px = psl.grid_x0 + ((double)grp.ring[let] + U_co(x1)) * psl.let_size;
     py = psl.grid_x0 + ((double)grp.sector[let] + U_co(x2)) * psl.let_size;
   }
+  // the PSR this particle is from: a sector let lies in one ring; a square let's particle belongs to
+  // the ring its position falls in
+  int psr_ring = psl.mode == 0 ? (int)grp.ring[let] : std::min(p.n_ring - 1, (int)std::floor(std::sqrt(px * px + py * py) / p.ring_width));
   // 3. energy, uniform in the bin
   double E = (p.e_min + grp.ebin * p.e_bin_width) + U_oc(x3) * p.e_bin_width;
   int s = grp.stype;
@@ -361,7 +364,7 @@ Sampled sample_history(const Psl &psl, const Beam &beam, const uint64_t *off, ui
     o.u = R[0] * dx + R[1] * dy + R[2] * dz;
     o.v = R[3] * dx + R[4] * dy + R[5] * dz;
     o.w = R[6] * dx + R[7] * dy + R[8] * dz;
-    o.E = E; o.group = (int)g; o.rejected = !pass;
+    o.E = E; o.group = (int)g; o.rejected = !pass; o.ring = psr_ring;
     return o;
   }
   // 4. source point from the 2-D Gaussian of the sub-source (Eq. 4)
@@ -388,7 +391,7 @@ Sampled sample_history(const Psl &psl, const Beam &beam, const uint64_t *off, ui
   o.u = R[0] * dx + R[1] * dy + R[2] * dz;
   o.v = R[3] * dx + R[4] * dy + R[5] * dz;
   o.w = R[6] * dx + R[7] * dy + R[8] * dz;
-  o.E = E; o.group = (int)g; o.rejected = !pass;
+  o.E = E; o.group = (int)g; o.rejected = !pass; o.ring = psr_ring;
   return o;
 }
 
@@ -460,7 +463,13 @@ struct Ctx {
     ijk[0] = (int)fi; ijk[1] = (int)fj; ijk[2] = (int)fk; return true;
   }
   size_t vox(const int ijk[3]) const { return ((size_t)ijk[2] * ph.ny + ijk[1]) * ph.nx + ijk[0]; }
-  void deposit(size_t v, double dE) { int64_t q = quanta(dE); acc[v] += q; ledger[1] += q; ++res->n_deposits; }
+  // Commissioning tally: com_index[v] = 0 (voxel not needed) or 1 + row; com_dose[col * com_rows + row]
+  // with col = the PSR unit of the history (all descendants inherit it).
+  const int32_t *com_index = nullptr; int64_t *com_dose = nullptr; int64_t com_rows = 0; uint32_t com_col = 0;
+  void deposit(size_t v, double dE) {
+    int64_t q = quanta(dE); acc[v] += q; ledger[1] += q; ++res->n_deposits;
+    if (com_index && com_index[v] > 0) com_dose[(size_t)com_col * com_rows + (com_index[v] - 1)] += q;
+  }
   void escape(double E) { ledger[2] += quanta(E); }
   // Ray/box entry: false = the track misses the phantom.
   bool enter(Track &t, int ijk[3]) const {
@@ -661,6 +670,35 @@ int32_t orc_dose(const void *h, const Phantom *ph, const Beam *beam, uint64_t N,
       c.stack.push_back(t); c.run_history();
     }
     if (fingerprints) fingerprints[hh - h_begin] += c.fp;
+  }
+  c.store_ledgers();
+  return 0;
+}
+
+// Column of the commissioning matrix for a particle of sub-source s, energy bin e, ring r: one per
+// photon PSR, one per electron energy bin ("effective electron PSR unit").
+uint32_t orc_com_column(int32_t n_ebin, int32_t n_ring, int32_t particle_type, int32_t s, int32_t e, int32_t r) {
+  return particle_type == 0 ? (uint32_t)((s * n_ebin + e) * n_ring + r) : (uint32_t)(2 * n_ebin * n_ring + e);
+}
+
+// orc_dose with the commissioning tally: com_index int32[nvox], com_dose int64[com_cols * com_rows] (ADDED to).
+int32_t orc_dose_com(const void *h, const Phantom *ph, const Beam *beam, uint64_t N, uint64_t seed, uint64_t h_begin,
+                     uint64_t h_end, int64_t *acc, Result *res, const int32_t *com_index, int64_t *com_dose, int64_t com_rows) {
+  const Psl &psl = *(const Psl *)h;
+  std::memset(res, 0, sizeof(Result));
+  Ctx c; c.init(*ph); c.seed = seed; c.flags = 0; c.acc = acc; c.res = res;
+  c.com_index = com_index; c.com_dose = com_dose; c.com_rows = com_rows;
+  std::vector<uint64_t> off(psl.groups.size() + 1); allocate(psl, N, off.data());
+  for (uint64_t hh = h_begin; hh < h_end; ++hh) {
+    Sampled s = sample_history(psl, *beam, off.data(), seed, hh);
+    const Group &g = psl.groups[s.group];
+    ++res->n_hist[g.stype];
+    c.ledger[0] += Ctx::quanta(s.E);
+    if (s.rejected) { c.ledger[3] += Ctx::quanta(s.E); ++res->n_jaw_rejected; continue; }
+    c.com_col = orc_com_column(psl.p.n_ebin, psl.p.n_ring, psl.p.particle_type[g.stype], g.stype, g.ebin, s.ring);
+    Track t; t.pos[0] = s.x; t.pos[1] = s.y; t.pos[2] = s.z; t.dir[0] = s.u; t.dir[1] = s.v; t.dir[2] = s.w; t.E = s.E;
+    t.type = psl.p.particle_type[g.stype]; t.h = hh; t.track = 0; t.ndraw = 8; t.nchild = 0;
+    c.fp = 0; c.stack.push_back(t); c.run_history();
   }
   c.store_ledgers();
   return 0;
