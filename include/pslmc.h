@@ -96,6 +96,13 @@ typedef struct {
                                    /* on cuda_stream (per-kernel times in mc_stats are then        */
                                    /* disjoint).  Same bits either way.                            */
   int32_t   reserved;              /* must be 0                                                    */
+  /* commissioning tally, off when com_index is NULL: every history carries the */
+  /* column of the PSR it was sampled from (its descendants inherit it): (stype*n_ebin+ebin)*n_ring */
+  /* + ring for the photon sub-sources, 2*n_ebin*n_ring + ebin for electrons; a deposit in a voxel */
+  /* with com_index[v] = 1 + row > 0 is also ADDED to com_dose[col * com_rows + row].              */
+  const int32_t *com_index;        /* DEVICE int32[nx*ny*nz]                                       */
+  int64_t  *com_dose;              /* DEVICE int64[com_cols * com_rows], quanta of 2^-32 MeV       */
+  int32_t   com_rows, com_cols;    /* com_cols must be 2*n_ebin*n_ring + n_ebin                    */
 } mc_opts_t;
 
 /* Ledger / kernel-class indices of mc_stats_t.                                                  */

@@ -51,7 +51,8 @@ class beam_geom_t(C.Structure):
 class mc_opts_t(C.Structure):
     _fields_ = [("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("cuda_stream", C.c_void_p),
                 ("dose_acc", C.c_void_p), ("order", C.c_int32), ("flags", C.c_int32), ("fingerprints", C.c_void_p),
-                ("history_begin", C.c_uint64), ("history_end", C.c_uint64), ("pipelines", C.c_int32), ("reserved", C.c_int32)]
+                ("history_begin", C.c_uint64), ("history_end", C.c_uint64), ("pipelines", C.c_int32), ("reserved", C.c_int32),
+                ("com_index", C.c_void_p), ("com_dose", C.c_void_p), ("com_rows", C.c_int32), ("com_cols", C.c_int32)]
 
 
 class mc_stats_t(C.Structure):
@@ -149,7 +150,7 @@ def stats() -> dict:
 
 
 def _opts(stream=None, workspace=None, dose_acc=None, order=0, flags=0, fingerprints=None, history_begin=0,
-          history_end=0, pipelines=0) -> mc_opts_t:
+          history_end=0, pipelines=0, com_index=None, com_dose=None) -> mc_opts_t:
     o = mc_opts_t()
     if workspace is not None:
         o.workspace, o.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
@@ -159,6 +160,9 @@ def _opts(stream=None, workspace=None, dose_acc=None, order=0, flags=0, fingerpr
     o.fingerprints = fingerprints.data_ptr() if fingerprints is not None else None
     o.history_begin, o.history_end = history_begin, history_end
     o.pipelines = pipelines
+    if com_index is not None:                            # commissioning tally: int32[nvox] index, int64[cols, rows] matrix (torch, device)
+        o.com_index, o.com_dose = com_index.data_ptr(), com_dose.data_ptr()
+        o.com_cols, o.com_rows = com_dose.shape[0], com_dose.shape[1]
     return o
 
 

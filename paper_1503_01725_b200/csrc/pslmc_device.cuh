@@ -129,6 +129,9 @@ struct Grid {
   const uint32_t *vox;                               // packed phantom, one gather per voxel: density bits rounded to a
                                                      // 22-bit mantissa | material index in the two low bits
   unsigned long long *acc;                           // int64 fixed-point dose accumulator (2^-32 MeV)
+  // commissioning tally, off when com_index is null: com_index[v] = 0 or 1 + row,
+  // com_dose[col * com_rows + row], col = the PSR unit the history was sampled from
+  const int *com_index; unsigned long long *com_dose; int com_rows;
 };
 
 __device__ __forceinline__ long long quanta(float e) { return __float2ll_rn(e * 4294967296.0f); }

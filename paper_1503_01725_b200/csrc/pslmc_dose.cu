@@ -48,7 +48,7 @@ static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 // queues (capacity B each), 3 planes per queue.
 constexpr int kMaxPipes = 2;
 struct Layout {
-  size_t ctl, off, xs, vox, p0, p1, eq[3], pq[2][3], acc, total;
+  size_t ctl, off, xs, vox, p0, p1, p2, eq[3], pq[2][3], acc, total;
   unsigned eq_cap, pq_cap;
 };
 static void make_layouts(uint64_t batch, size_t nvox, bool with_acc, Layout out[kMaxPipes]) {
@@ -60,7 +60,7 @@ static void make_layouts(uint64_t batch, size_t nvox, bool with_acc, Layout out[
   for (int p = 0; p < kMaxPipes; ++p) {
     Layout &Q = out[p]; Q = L;
     Q.ctl = take(sizeof(Control));
-    Q.p0 = take(16 * batch); Q.p1 = take(16 * batch);
+    Q.p0 = take(16 * batch); Q.p1 = take(16 * batch); Q.p2 = take(4 * batch);
     for (int k = 0; k < 3; ++k) Q.eq[k] = take((size_t)16 * L.eq_cap);
     for (int b = 0; b < 2; ++b) for (int k = 0; k < 3; ++k) Q.pq[b][k] = take((size_t)16 * L.pq_cap);
   }
@@ -216,7 +216,7 @@ struct Run {
     TransportArgs a{};
     a.g = g; a.ctl = ctl; a.seed = seed; a.n_total = n_total; a.perm_a = perm_a;
     round_keys(seed, a.ks);
-    a.p0 = (const float4 *)(ws + L.p0); a.p1 = (const float4 *)(ws + L.p1);
+    a.p0 = (const float4 *)(ws + L.p0); a.p1 = (const float4 *)(ws + L.p1); a.p2 = g.com_index ? (const uint32_t *)(ws + L.p2) : nullptr;
     a.eq = queue(L.eq, &ctl->n_eq, L.eq_cap); a.pq = queue(L.pq[pq_fill], &ctl->n_pq, L.pq_cap);
     a.fp = fp; a.fp_base = fp_base;
     a.electrons_local = (flags & MC_FLAG_ELECTRONS_LOCAL) ? 1 : 0;
@@ -402,6 +402,9 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
   const bool mixed = opts->order == MC_ORDER_MIXED;
   if (mixed && (N >> 32)) return fail(MC_E_INVALID_ARG, "mc_dose: mixed order needs n_histories < 2^32");
   if (mixed && opts->fingerprints && (hb != 0 || he != N)) return fail(MC_E_INVALID_ARG, "mc_dose: mixed order + fingerprints needs the full range");
+  if (opts->com_index && (!opts->com_dose || opts->com_rows < 1 || opts->com_cols != 2 * P->n_ebin * P->n_ring + P->n_ebin))
+    return fail(MC_E_INVALID_ARG, "mc_dose: commissioning tally needs com_dose, com_rows >= 1 and com_cols = 2*n_ebin*n_ring + n_ebin");
+  if (opts->com_index && mixed) return fail(MC_E_INVALID_ARG, "mc_dose: the commissioning tally runs in sorted order");
   int dev = 0; CUDA_TRY(cudaGetDevice(&dev));
   if (dev != P->device) return fail(MC_E_INVALID_ARG, "mc_dose: psl_t was built on another device");
 
@@ -429,9 +432,10 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
     Run &r = pipes[p];
     r.st = npipe > 1 ? (*pstreams)[p] : us; r.ws = (char *)ws; r.L = Ls[p]; r.ctl = (Control *)(r.ws + Ls[p].ctl);
     r.g = make_grid(*ph, acc); r.g.vox = (const uint32_t *)(r.ws + L.vox);
+    r.g.com_index = (const int *)opts->com_index; r.g.com_dose = (unsigned long long *)opts->com_dose; r.g.com_rows = opts->com_rows;
     r.seed = seed; r.n_total = N; r.perm_a = mixed ? mixed_multiplier(N) : 0; r.flags = opts->flags; r.batch = batch;
     r.fp = (unsigned long long *)opts->fingerprints; r.fp_base = hb;
-    r.dbg = (opts->flags & MC_FLAG_STATS) || opts->fingerprints;
+    r.dbg = (opts->flags & MC_FLAG_STATS) || opts->fingerprints || opts->com_index;   // the tally lives in the stats variants
     r.tm.on = (opts->flags & MC_FLAG_TIMING) != 0; r.tm.st = r.st;
     if (p == 0) r.init_blocks();
     else { for (int k = 0; k < 2; ++k) { r.blocks_photon[k] = pipes[0].blocks_photon[k]; r.blocks_electron[k] = pipes[0].blocks_electron[k]; } }
@@ -469,6 +473,7 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
     Run &r = pipes[p]; SampleArgs &a = sa[p]; a = SampleArgs{};
     a.m = source_model(*P); a.beam = beam_xf(*beam); a.off_g = d_off; a.seed = seed; round_keys(seed, a.ks); a.n_total = N; a.perm_a = r.perm_a;
     a.p0 = (float4 *)(r.ws + r.L.p0); a.p1 = (float4 *)(r.ws + r.L.p1); a.ctl = r.ctl; a.fp = r.fp; a.fp_base = hb; a.compact = 1; a.g = r.g; a.stats = r.dbg ? 1 : 0;
+    a.p2 = r.g.com_index ? (uint32_t *)(r.ws + r.L.p2) : nullptr;
   }
 
   memset(&g_stats, 0, sizeof g_stats);

@@ -69,6 +69,7 @@ struct SampleArgs {
   unsigned long long seed, first, n_total, perm_a;   // perm_a != 0 → mixed order: h = (perm_a * t) mod n_total
   unsigned count;
   float4 *p0, *p1;                   // outputs (two float4 planes)
+  uint32_t *p2;                      // compact mode, commissioning tally: column (PSR unit) of every packed particle, or null
   Control *ctl;
   unsigned long long *fp;            // fingerprints or null
   unsigned long long fp_base;
@@ -106,6 +107,7 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
   bool pass = false, missed = false;
   float4 o0 = make_float4(0.f, 0.f, 0.f, 0.f), o1 = o0;
   int g = 0, ptype = 0;
+  uint32_t com_col = 0u;
   if (live) {
     const unsigned long long h = history_of(a.first + t, a.perm_a, a.n_total);
     if (a.perm_a == 0) {
@@ -139,6 +141,10 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
     } else {                                 // square let (Xbin, Ybin) = (ring, sector) fields of the entry
       px = m.grid_x0 + (ring + u_co(x1)) * m.let_size;
       py = m.grid_x0 + (sector + u_co(x2)) * m.let_size;
+    }
+    if (a.p2) {                                // the PSR this particle is from: one column per photon PSR, one per electron energy bin
+      const int pr = m.let_mode == 0 ? (int)ring : min((int)(sqrtf(__fmaf_rn(px, px, py * py)) / m.ring_width), m.n_ring - 1);
+      com_col = ptype == 0 ? (uint32_t)((stype * m.n_ebin + ebin) * m.n_ring + pr) : (uint32_t)(2 * m.n_ebin * m.n_ring + ebin);
     }
     // 3. energy uniform in the bin
     const float E = (m.e_min + (float)ebin * m.e_bin_width) + u_oc(x3) * m.e_bin_width;
@@ -221,6 +227,7 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
       const unsigned dst = base + __popc(keep & ((1u << lane) - 1u));
       o1.w = __uint_as_float(t | ((unsigned)ptype << 31));
       a.p0[dst] = o0; a.p1[dst] = o1;
+      if (a.p2) a.p2[dst] = com_col;
     }
   } else if (live) {
     o1.w = pass ? (float)g : -(float)g - 1.0f;

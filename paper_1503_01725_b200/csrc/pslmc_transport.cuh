@@ -37,6 +37,7 @@ struct TransportArgs {
   int src_kind;                       // SRC_BUFFER: p0/p1 planes from k_sample;  SRC_QUEUE: src queue
   int buffer_is_debug;                // SRC_BUFFER only: 1 = indexed by history, p1.w = status (skip < 0)
   const float4 *p0, *p1;
+  const uint32_t *p2;                 // commissioning column per buffer entry, or null
   Queue src;
   const unsigned *src_count;          // entries available (device)
   const unsigned *src2_count;         // SRC_BUFFER only, or null: `src` holds this many extra tracks, consumed after the buffer
@@ -109,9 +110,19 @@ struct ScoreStage {
 };
 
 // Pending deposit: consecutive deposits into one voxel are merged before the atomic (integers: exact).
+template <bool COM>                                   // COM: the kernel variant that may carry a commissioning tally (= DBG)
 struct Pending {
-  int v; long long q;
-  template <bool ON> __device__ __forceinline__ void flush(const Grid &g, const ScoreStage<ON> &st) { if (q) st.add(g, v, (unsigned long long)q); q = 0; }
+  int v; long long q; uint32_t col;                  // col: commissioning column of the lane's current history
+  template <bool ON> __device__ __forceinline__ void flush(const Grid &g, const ScoreStage<ON> &st) {
+    if (q) {
+      st.add(g, v, (unsigned long long)q);
+      if (COM && g.com_index) {                      // only the stats/fingerprint kernel variants are launched with a tally
+        const int row = __ldg(g.com_index + v);
+        if (row > 0) atomicAdd(g.com_dose + (size_t)col * g.com_rows + (row - 1), (unsigned long long)q);
+      }
+    }
+    q = 0;
+  }
   template <bool ON> __device__ __forceinline__ void add(const Grid &g, const ScoreStage<ON> &st, int vox, long long dq) {
     if (vox != v) { flush(g, st); v = vox; }
     q += dq;
@@ -214,7 +225,7 @@ __device__ __forceinline__ unsigned refill_index(const TransportArgs &a, bool id
   return (idle && rank < avail) ? idx : 0xffffffffu;
 }
 
-struct TrackIn { float x, y, z, u, v, w, E; unsigned long long h; uint32_t track, ndraw; bool ok; };
+struct TrackIn { float x, y, z, u, v, w, E; unsigned long long h; uint32_t track, ndraw, col; bool ok; };
 
 __device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned idx, unsigned n1) {
   TrackIn t;
@@ -225,12 +236,12 @@ __device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned i
     if (a.buffer_is_debug) { tt = idx; t.ok = B.w >= 0.0f; }
     else { const unsigned bits = __float_as_uint(B.w); tt = bits & 0x7fffffffu; t.ok = (int)(bits >> 31) == a.want_type; }
     t.h = history_of(a.first + tt, a.perm_a, a.n_total);
-    t.track = 0u; t.ndraw = 8u;
+    t.track = 0u; t.ndraw = 8u; t.col = a.p2 ? a.p2[idx] : 0u;
   } else {
     if (a.src_kind == SRC_BUFFER) idx -= n1;
     const float4 A = a.src.a[idx], B = a.src.b[idx]; const uint4 C = a.src.c[idx];
     t.x = A.x; t.y = A.y; t.z = A.z; t.E = A.w; t.u = B.x; t.v = B.y; t.w = B.z;
-    t.h = ((unsigned long long)C.y << 32) | C.x; t.track = C.z; t.ndraw = 0u; t.ok = true;
+    t.h = ((unsigned long long)C.y << 32) | C.x; t.track = C.z; t.ndraw = 0u; t.col = C.w; t.ok = true;
   }
   return t;
 }
@@ -261,7 +272,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
   StageCursor stg; stg.head = stg.n = stg.base_raw = 0u; stg.pending = false;
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
-  Pending pend; pend.v = 0; pend.q = 0;
+  Pending<DBG> pend; pend.v = 0; pend.q = 0; pend.col = 0u;
   int state = PH_IDLE; bool exhausted = false, collided = false;
   float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, E = 0;
   int cvox = 0;                                          // voxel of the current position
@@ -276,6 +287,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
       const TrackIn t = load_track(a, idx, n1);
       if (t.ok) {
         x = t.x; y = t.y; z = t.z; u = t.u; v = t.v; w = t.w; E = t.E; h = t.h; nchild = 0; collided = false;
+        if (DBG && g.com_index) { pend.flush(g, stage); pend.col = t.col; }
         rng.init(h, t.track, t.ndraw);
         if (DBG) fnv.init(t.track);
         if (a.buffer_is_debug) tl.inc += (unsigned long long)quanta(E);
@@ -397,7 +409,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
     }
     // ---- secondaries, convergent: Compton electrons through the staging ring ...
     stage_push(a.eq, a.ctl, ring, stg, push_e, make_float4(x, y, z, eT), make_float4(ex, ey, ez, 0.f),
-               make_uint4((uint32_t)h, (uint32_t)(h >> 32), etrack, 0u));
+               make_uint4((uint32_t)h, (uint32_t)(h >> 32), etrack, DBG ? pend.col : 0u));
     // ... and, in the rare iteration with a pair production in the warp, the e-/e+ through the same ring and
     // the two annihilation photons behind ONE warp-aggregated tail atomic (the lane's x, y, z, u, v, w, h,
     // nchild are still those of the converting photon: it only refills at the top of the next iteration)
@@ -406,7 +418,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
 #pragma unroll
       for (int sl = 0; sl < 2; ++sl)
         stage_push(a.eq, a.ctl, ring, stg, pairT[sl] > 0.0f, make_float4(x, y, z, pairT[sl]), make_float4(u, v, w, 0.f),
-                   make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, (uint32_t)sl), 0u));
+                   make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, (uint32_t)sl), DBG ? pend.col : 0u));
       const unsigned lane = threadIdx.x & 31u, leader = __ffs(mp) - 1;
       unsigned base = 0;
       if (lane == leader) base = atomicAdd(a.pq.count, 2u * __popc(mp));
@@ -417,8 +429,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
         else {
           a.pq.a[slot] = a.pq.a[slot + 1] = make_float4(x, y, z, kEAnnih);
           a.pq.b[slot] = make_float4(ex, ey, ez, 0.f); a.pq.b[slot + 1] = make_float4(-ex, -ey, -ez, 0.f);
-          a.pq.c[slot] = make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, 2u), 0u);
-          a.pq.c[slot + 1] = make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, 3u), 0u);
+          a.pq.c[slot] = make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, 2u), DBG ? pend.col : 0u);
+          a.pq.c[slot + 1] = make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, 3u), DBG ? pend.col : 0u);
         }
       }
     }
@@ -445,7 +457,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
   SrcCursor sc; sc.next = sc.end = 0u;
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
-  Pending pend; pend.v = 0; pend.q = 0;
+  Pending<DBG> pend; pend.v = 0; pend.q = 0; pend.col = 0u;
   bool active = false, exhausted = false;
   float lx = 0, ly = 0, lz = 0, u = 0, v = 0, w = 1, T = 0;      // offset inside voxel (vi,vj,vk), direction, energy
   float iu = 0, iv = 0, iw = 1;                                   // reciprocal direction cosines (refreshed when the direction changes)
@@ -463,6 +475,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
       if (t.ok) {
         float x = t.x, y = t.y, z = t.z;
         u = t.u; v = t.v; w = t.w; T = t.E; h = t.h; steps = 0; fresh = true;
+        if (DBG && g.com_index) { pend.flush(g, stage); pend.col = t.col; }
         rng.init(h, t.track, t.ndraw);
         if (DBG) { fnv.init(t.track); ++tl.st[ST_ETRACKS]; }
         if (a.buffer_is_debug) tl.inc += (unsigned long long)quanta(T);
