@@ -165,6 +165,12 @@ int  psl_export(const psl_t *psl, void *host_buf, size_t *bytes);
  * off_out: HOST u64[n_groups+1], prefix offsets of the contiguous history-id ranges.            */
 int  psl_allocate(const psl_t *psl, uint64_t n_histories, uint64_t *off_out);
 
+/* mc_plan_allocate — host.  Eq. 3 across the beams of a treatment plan (the denominator of Eq. 3 runs
+ * over the sampling areas of all beams): beam i gets n_histories * W_i / sum_j W_j histories, W_i = the sum of the
+ * active group weights of psls[i]; largest-remainder rounding, ties to the lower index.  n_out: HOST u64[n_beams].
+ * Run mc_dose once per beam with n_out[i] histories into one opts->dose_acc, then scale by the plan total.      */
+int  mc_plan_allocate(const psl_t *const *psls, int32_t n_beams, uint64_t n_histories, uint64_t *n_out);
+
 /* Workspace bytes mc_dose needs for this batch size (0 on invalid arguments).                   */
 size_t mc_workspace_bytes(const psl_t *psl, const phantom_t *ph, uint64_t batch);
 

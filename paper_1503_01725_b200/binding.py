@@ -18,7 +18,7 @@ MC_ORDER_SORTED, MC_ORDER_MIXED = 0, 1
 MC_FLAG_ELECTRONS_LOCAL, MC_FLAG_STATS, MC_FLAG_TIMING, MC_FLAG_STATIC_LANES, MC_FLAG_STAGE_SCORING = 1, 2, 4, 8, 16
 LEDGERS = ("incident", "deposited", "escaped", "jaw")
 KERNEL_CLASSES = ("sample", "photon", "electron", "finalise", "aux")
-EXPORTS = ("psl_build", "psl_build_grid", "psl_set_direction_model", "psl_free", "psl_export", "psl_allocate", "mc_workspace_bytes", "mc_dose", "mc_dose_host",
+EXPORTS = ("psl_build", "psl_build_grid", "psl_set_direction_model", "mc_plan_allocate", "psl_free", "psl_export", "psl_allocate", "mc_workspace_bytes", "mc_dose", "mc_dose_host",
            "mc_stats", "mc_last_error", "mc_sample_debug", "mc_transport_debug", "mc_philox_debug", "mc_xs_debug")
 
 
@@ -78,6 +78,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.psl_build.argtypes = [C.POINTER(psr_params_t), C.POINTER(jaws_t), C.c_int32, C.POINTER(C.c_void_p)]
         L.psl_build_grid.argtypes = [C.POINTER(psr_params_t), C.POINTER(jaws_t), C.c_double, C.POINTER(C.c_void_p)]
+        L.mc_plan_allocate.argtypes = [C.c_void_p, C.c_int32, C.c_uint64, C.c_void_p]
         L.psl_set_direction_model.argtypes = [C.c_void_p, C.c_int32, C.c_int32] + [C.c_void_p] * 4
         L.psl_free.argtypes = [C.c_void_p]
         L.psl_free.restype = None
@@ -279,6 +280,32 @@ def xs_debug(rhomax, e_max: float, energies) -> np.ndarray:
     out = np.empty((e.size, 3), np.float32)
     _check(lib().mc_xs_debug(rm.ctypes.data_as(C.c_void_p), float(e_max), e.ctypes.data_as(C.c_void_p), e.size, out.ctypes.data_as(C.c_void_p)))
     return out
+
+
+def plan_allocate(psls, n_histories: int) -> np.ndarray:
+    """Eq. 3 across the beams of a plan: histories per beam, proportional to each beam's active weight."""
+    arr = (C.c_void_p * len(psls))(*[p.h for p in psls])
+    out = np.zeros(len(psls), np.uint64)
+    _check(lib().mc_plan_allocate(arr, len(psls), n_histories, out.ctypes.data_as(C.c_void_p)))
+    return out
+
+
+def plan_dose(psls, phantom, beams, n_histories: int, seed: int, batch: int = 1 << 22, rank: int = 0, world: int = 1, **opt):
+    """A multi-beam plan (PAPER.md:75-80 S1-S2): Eq. 3 over all beams, one mc_dose per beam (seed + beam index) into one int64
+    grid.  With world > 1 every rank runs its contiguous share of each beam's histories; the caller all-reduces the returned
+    grid (int64, SUM: bit-exact).  Returns (acc int64 on the device, histories per beam)."""
+    import torch
+    n_beam = plan_allocate(psls, n_histories)
+    acc = torch.zeros(phantom.nvox, dtype=torch.int64, device=phantom.device)
+    for i, (psl, beam) in enumerate(zip(psls, beams)):
+        n = int(n_beam[i])
+        if n == 0:
+            continue
+        hb, he = shard_range(n, rank, world)
+        if hb == he:
+            continue
+        psl.dose(phantom, beam, n, seed + i, batch=batch, dose_acc=acc, history_begin=hb, history_end=he, **opt)
+    return acc, n_beam
 
 
 def shard_range(n_histories: int, rank: int, world: int) -> tuple[int, int]:

@@ -223,6 +223,32 @@ extern "C" int psl_allocate(const psl_t *P, uint64_t n_histories, uint64_t *off_
   return MC_OK;
 }
 
+// Eq. 3 across the beams of a plan (the denominator runs over the sampling areas of ALL beams):
+// beam i gets N * W_i / sum_j W_j histories, W_i = sum of its active group weights, largest-remainder rounding,
+// ties to the lower beam index.
+extern "C" int mc_plan_allocate(const psl_t *const *psls, int32_t n_beams, uint64_t n_histories, uint64_t *n_out) {
+  if (!psls || !n_out || n_beams < 1) return fail(MC_E_INVALID_ARG, "mc_plan_allocate: invalid argument");
+  std::vector<double> W(n_beams, 0.0), frac(n_beams);
+  double tot = 0;
+  for (int i = 0; i < n_beams; ++i) {
+    if (!psls[i]) return fail(MC_E_INVALID_ARG, "mc_plan_allocate: null beam");
+    for (const HostGroup &g : psls[i]->groups) W[i] += g.W;
+    tot += W[i];
+  }
+  if (!(tot > 0)) return fail(MC_E_EMPTY_FIELD, "mc_plan_allocate: no active let in any beam");
+  uint64_t used = 0;
+  for (int i = 0; i < n_beams; ++i) {
+    const double q = (double)n_histories * W[i] / tot, f = std::floor(q);
+    n_out[i] = (uint64_t)f; frac[i] = q - f; used += n_out[i];
+  }
+  std::vector<int> order(n_beams);
+  for (int i = 0; i < n_beams; ++i) order[i] = i;
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return frac[a] > frac[b]; });
+  const uint64_t rem = n_histories - used;
+  for (uint64_t r = 0; r < rem; ++r) ++n_out[order[r % n_beams]];
+  return MC_OK;
+}
+
 extern "C" int psl_export(const psl_t *P, void *host_buf, size_t *bytes) {
   if (!P || !bytes) return fail(MC_E_INVALID_ARG, "psl_export: null argument");
   auto pad8 = [](size_t b) { return (b + 7) & ~(size_t)7; };

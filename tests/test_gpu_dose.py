@@ -174,3 +174,27 @@ def test_vacuum_and_queue_stats(B, orc, cfg, wl):
     compare_with_oracle(B, orc, g, o, ph, c["beams"][0], 300_000, 8, batch=1 << 16, frac_vox=0.98)
     st = B.stats()
     assert 0 < st["queue_high_water"][0] < 4 * (1 << 16) and st["launches"]["photon"] > 0
+
+
+# ---------------------------------------------------------------- plan level (NEXT-4)
+def test_plan_allocation_eq3_and_sharded_plan(B, cfg):
+    """Eq. 3 across beams: histories per beam proportional to the beam's active weight; a 7-beam plan
+    sharded over two 'ranks' (history ranges of every beam) adds up to the single-rank plan bit for bit."""
+    import torch
+    c = cfg("C3")
+    fields = (4.0, 8.0, 12.0)
+    psls = [B.Psl(c["psr"], dict(c["jaws"], x1=-f / 2, x2=f / 2, y1=-f / 2, y2=f / 2), c["n_sectors"]) for f in fields]
+    W = np.array([sum(g["W"] for g in p.export()["groups"]) for p in psls])
+    N = 1_000_003
+    n = B.plan_allocate(psls, N).astype(np.int64)
+    assert n.sum() == N and np.all(np.abs(n - N * W / W.sum()) < 1) and n[0] < n[1] < n[2]
+    # C3: seven coplanar beams, one jaw setting
+    dph = B.DevicePhantom(c["phantom"])
+    g = B.Psl(c["psr"], c["jaws"], c["n_sectors"])
+    beams = c["beams"]
+    acc, nb = B.plan_dose([g] * len(beams), dph, beams, 2_100_000, 40, batch=1 << 18)
+    assert nb.tolist() == [300_000] * 7
+    parts = [B.plan_dose([g] * len(beams), dph, beams, 2_100_000, 40, batch=1 << 17, rank=r, world=2)[0] for r in range(2)]
+    assert torch.equal(parts[0] + parts[1], acc)
+    d = acc.cpu().numpy().reshape(120, 256, 256)
+    assert d[50:70, 118:138, 118:138].mean() > 5 * d[50:70, :20, :20].mean()
