@@ -98,6 +98,13 @@ struct RngWin {
     d2 = s == 0u ? c2 : (s == 1u ? c3 : (s == 2u ? g0 : g1));
     d3 = s == 0u ? c3 : (s == 1u ? g0 : (s == 2u ? g1 : g2));
   }
+  // Streams that are only ever read two draws at a time from an even draw number (k_electron: one pair per
+  // deflection): the pair is words 0,1 of a fresh block or the cached words 2,3 of the last one.
+  __device__ __forceinline__ void pair(const uint32_t (&ks)[20], uint32_t &d0, uint32_t &d1) {
+    if ((n & 2u) == 0u) { uint32_t g0, g1; gen(ks, n >> 2, g0, g1, c2, c3); d0 = g0; d1 = g1; }
+    else { d0 = c2; d1 = c3; }
+    n += 2u;
+  }
   __device__ __forceinline__ void consume(uint32_t k, uint32_t g0, uint32_t g1, uint32_t g2, uint32_t g3) {
     const uint32_t m = n + k;
     if ((m >> 2) != (n >> 2)) { c0 = g0; c1 = g1; c2 = g2; c3 = g3; }

@@ -526,9 +526,8 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
           if (DBG) { fnv.u32(steps); fnv.byte('E'); ++tl.st[ST_EESC]; }
           done = true;
         } else if (turn) {
-          uint32_t d0, d1, d2, d3, g0, g1, g2, g3;
-          rng.window<2>(a.ks, d0, d1, d2, d3, g0, g1, g2, g3);
-          rng.consume(2u, g0, g1, g2, g3);
+          uint32_t d0, d1;
+          rng.pair(a.ks, d0, d1);
           // theta = (13.6 / p beta) sqrt(tacc) sqrt(-2 ln a), p beta = Tms (Tms + 2 me)/(Tms + me): one division, one root
           const float c = __fdividef(13.6f * (Tms + kMe), Tms * (Tms + 2.0f * kMe));
           const float th = fminf(kPi, c * sqrt_fast(tacc * (-2.0f * __logf(u_oc(d0)))));
