@@ -198,3 +198,25 @@ def test_plan_allocation_eq3_and_sharded_plan(B, cfg):
     assert torch.equal(parts[0] + parts[1], acc)
     d = acc.cpu().numpy().reshape(120, 256, 256)
     assert d[50:70, 118:138, 118:138].mean() > 5 * d[50:70, :20, :20].mean()
+
+
+def test_history_ids_beyond_32_bits(B, orc, gpsl, opsl, cfg):
+    """A slice of a 2^33-history run: history ids, the Philox counter words and the group offsets are 64-bit on both sides."""
+    import torch
+    c = cfg("C0")
+    N = 1 << 33
+    dph, oph = B.DevicePhantom(c["phantom"]), orc.Phantom(c["phantom"])
+    assert np.array_equal(gpsl("C0").allocate(N), opsl("C0").allocate(N))
+    for hb in (N - 20_000, (1 << 32) - 10_000):
+        he = hb + 20_000
+        fp = torch.zeros(he - hb, dtype=torch.int64, device="cuda")
+        acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
+        gpsl("C0").dose(dph, c["beams"][0], N, 77, batch=6000, dose_acc=acc, fingerprints=fp, history_begin=hb, history_end=he)
+        oacc = np.zeros(oph.nvox, np.int64)
+        _, _, ofp = opsl("C0").dose(oph, c["beams"][0], N, 77, h_begin=hb, h_end=he, acc=oacc, fingerprints=True)
+        assert (fp.cpu().numpy().view(np.uint64) == ofp).mean() >= 0.999
+        a = acc.cpu().numpy()
+        assert abs(int(a.sum()) - int(oacc.sum())) <= 2e-3 * int(oacc.sum())
+    got = gpsl("C0").sample_debug(c["beams"][0], N, 77, (1 << 32) - 5, 10).cpu().numpy().astype(np.float64)
+    ref = opsl("C0").sample(c["beams"][0], N, 77, (1 << 32) - 5, 10)
+    assert np.allclose(got[0, :, :3], ref[:, :3], atol=2e-5) and np.array_equal(got[1, :, 3], ref[:, 7])
