@@ -140,9 +140,9 @@ class ClockSampler:
 # and the bytes k_sample must write per history (32 B per particle that passes the jaws).
 ALG_THREAD_INST_PER_HISTORY = {"C1": {"photon": 724.0, "electron": 846.0, "sample": 507.0},      # profiles/r1c_launches.md
                                "C4": {"photon": 2575.0, "electron": 2604.0, "sample": 600.0}}    # profiles/r1b_ablation_c4.md (batch 2^22, sorted)
-# DRAM bytes (read + write) per step of each kernel class, from the ncu --set full captures of profiles/r1b_top_kernels.md
+# DRAM bytes (read + write) per step of each kernel class, from the ncu --set full captures of profiles/r1c_top_kernels.md
 # (the two primary-batch launches; the path's working set is L2-resident, so this is far below any HBM bound)
-NCU_DRAM_BYTES_PER_STEP = {"C1": {"photon": 2.21e8, "electron": 1.42e8, "sample": 4.5e7}}
+NCU_DRAM_BYTES_PER_STEP = {"C1": {"photon": 2.17e8, "electron": 1.42e8, "sample": 6.5e7}}
 SAMPLE_BYTES_PER_PARTICLE = 32.0
 
 
