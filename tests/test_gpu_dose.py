@@ -220,3 +220,40 @@ def test_history_ids_beyond_32_bits(B, orc, gpsl, opsl, cfg):
     got = gpsl("C0").sample_debug(c["beams"][0], N, 77, (1 << 32) - 5, 10).cpu().numpy().astype(np.float64)
     ref = opsl("C0").sample(c["beams"][0], N, 77, (1 << 32) - 5, 10)
     assert np.allclose(got[0, :, :3], ref[:, :3], atol=2e-5) and np.array_equal(got[1, :, 3], ref[:, 7])
+
+
+def test_full_size_c1_in_the_bench_configuration(B, orc, gpsl, opsl, cfg):
+    """BASELINE.json configs[1] at its full 1e7 histories in the launch configuration bench.py times (batch 2^22, two
+    pipelines, sorted order): (a) the interaction sequences of sampled history ranges match the oracle history by
+    history; (b) the dose grid is bit-identical to a serial small-batch run; (c) the ledger identities hold."""
+    import torch
+    c = cfg("C1")
+    N, seed = c["n_histories"], c["seed"]
+    assert N == 10_000_000
+    dph, oph = B.DevicePhantom(c["phantom"]), orc.Phantom(c["phantom"])
+    fp = torch.zeros(N, dtype=torch.int64, device="cuda")
+    acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
+    gpsl("C1").dose(dph, c["beams"][0], N, seed, batch=1 << 22, dose_acc=acc, fingerprints=fp)
+    st = B.stats()
+    L = st["ledger"]
+    assert int(acc.sum().item()) == L["deposited"]
+    assert abs(L["deposited"] + L["escaped"] + L["jaw"] - L["incident"]) <= 1e-5 * L["incident"]
+    # (a) 64 equally spaced ranges of 2000 histories: all three sub-sources, all energy bins
+    gfp = fp.cpu().numpy().view(np.uint64)
+    same = total = 0
+    oacc = np.zeros(oph.nvox, np.int64)
+    for i in range(64):
+        a = int(i * N / 64) + 137
+        _, _, ofp = opsl("C1").dose(oph, c["beams"][0], N, seed, h_begin=a, h_end=a + 2000, acc=oacc, fingerprints=True)
+        same += int((gfp[a:a + 2000] == ofp).sum()); total += 2000
+    last = N - 1500                                                        # the contamination-electron tail
+    _, _, ofp = opsl("C1").dose(oph, c["beams"][0], N, seed, h_begin=last, h_end=N, acc=oacc, fingerprints=True)
+    same += int((gfp[last:] == ofp).sum()); total += N - last
+    assert same / total >= 0.999, same / total
+    # (b) same bits without fingerprints (the plain kernel variants bench.py times), and serial with a small batch
+    acc2 = torch.zeros_like(acc)
+    gpsl("C1").dose(dph, c["beams"][0], N, seed, batch=1 << 22, dose_acc=acc2)
+    assert torch.equal(acc, acc2)
+    acc3 = torch.zeros_like(acc)
+    gpsl("C1").dose(dph, c["beams"][0], N, seed, batch=1 << 18, dose_acc=acc3, pipelines=1)
+    assert torch.equal(acc, acc3) and B.stats()["ledger"] == L
