@@ -34,40 +34,11 @@ __constant__ Materials c_mat = {
     {1.0f / 36.08f, 1.0f / 36.08f, 1.0f / 27.2f}};
 
 // ------------------------------------------------------------------ R1: Philox4x32-10
-struct Philox {
-  uint32_t k0, k1;             // key = seed
-  uint32_t track, hlo, hhi;    // counter words 1..3
-  uint32_t n;                  // next draw number of this stream (block n>>2, word n&3)
-  uint32_t w0, w1, w2, w3;     // cached block
-
-  __device__ __forceinline__ void block(uint32_t j) {
-    uint32_t c0 = j, c1 = track, c2 = hlo, c3 = hhi, a = k0, b = k1;
-#pragma unroll
-    for (int r = 0; r < 10; ++r) {
-      uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
-      uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
-      c0 = h1 ^ c1 ^ a; c1 = l1; c2 = h0 ^ c3 ^ b; c3 = l0;
-      a += 0x9E3779B9u; b += 0xBB67AE85u;
-    }
-    w0 = c0; w1 = c1; w2 = c2; w3 = c3;
-  }
-  __device__ __forceinline__ void init(uint64_t seed, uint64_t h, uint32_t trk, uint32_t ndraw) {
-    k0 = (uint32_t)seed; k1 = (uint32_t)(seed >> 32);
-    hlo = (uint32_t)h; hhi = (uint32_t)(h >> 32); track = trk; n = ndraw;
-    if (ndraw & 3u) block(ndraw >> 2);
-  }
-  __device__ __forceinline__ uint32_t next() {
-    uint32_t i = n & 3u;
-    if (i == 0) block(n >> 2);
-    ++n;
-    return i == 0 ? w0 : (i == 1 ? w1 : (i == 2 ? w2 : w3));
-  }
-};
-// The same stream, consumed through ONE generation site per event: window<K>() returns draws
+// The stream of a track, consumed through ONE generation site per event: window<K>() returns draws
 // n..n+3 of the track's stream without consuming them (the caller may consume up to K <= 4 of
 // them), generating at most one Philox block; consume(k, ...) advances.  c0..c3 cache the block that
 // holds draw n whenever n & 3 != 0.  Draw numbering is exactly DESIGN.md R1 (draw n = word n & 3 of
-// block n >> 2): only where the blocks are generated differs from Philox::next().
+// block n >> 2).
 struct RngWin {
   uint32_t track, hlo, hhi, n;
   uint32_t c0, c1, c2, c3;
@@ -175,30 +146,6 @@ __device__ __forceinline__ bool enter(const Grid &g, float &x, float &y, float &
 }
 
 // ------------------------------------------------------------------ physics
-// Klein–Nishina total cross-section per electron (cm^2).  The bracket cancels ~1.5/alpha^2-fold at low
-// energy, so it is evaluated in double (once per photon energy change, not per flight).
-__device__ __forceinline__ float sigma_kn(float E) {
-  double a = (double)E / kMeD, L = log1p(2.0 * a), t = 1.0 + 2.0 * a;
-  double s = (1.0 + a) / (a * a) * (2.0 * (1.0 + a) / t - L / a) + L / (2.0 * a) - (1.0 + 3.0 * a) / (t * t);
-  return (float)(kTwoPiRe2 * s);
-}
-
-// Per-energy photon data, recomputed after every energy change.
-struct PhotonXs {
-  float skn, inv_e3, lp2, mu_max;     // sigma_KN, 1/E^3, ln^2(E/1.022) (0 below threshold), Woodcock majorant
-  __device__ __forceinline__ void set(float E, const float rhomax[3]) {
-    skn = sigma_kn(E);
-    inv_e3 = 1.0f / (E * E * E);
-    float l = E > kEPair ? logf(E / kEPair) : 0.0f;
-    lp2 = l * l;
-    float m = 0.0f;
-#pragma unroll
-    for (int k = 0; k < 3; ++k)
-      m = fmaxf(m, rhomax[k] * (c_mat.ne[k] * skn + c_mat.cphoto[k] * inv_e3 + c_mat.ppair[k] * lp2));
-    mu_max = m;
-  }
-};
-
 __device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 
 // Photon cross-section data (built per mc_dose call on the device, in double, by k_build_xs), kept in shared
@@ -248,22 +195,6 @@ __device__ __forceinline__ void rotate(float &u, float &v, float &w, float ct, f
   }
   const float inv = rsqrtf(__fmaf_rn(nx, nx, __fmaf_rn(ny, ny, nz * nz)));
   u = nx * inv; v = ny * inv; w = nz * inv;
-}
-
-// Kahn's rejection for Klein–Nishina: returns eta = E/E'.  3 draws per trial.
-__device__ __forceinline__ float kahn(float alpha, Philox &rng) {
-  const float ta = 2.0f * alpha, pb = (ta + 1.0f) / (ta + 9.0f);
-  for (;;) {
-    float r1 = u_co(rng.next()), r2 = u_co(rng.next()), r3 = u_co(rng.next());
-    if (r1 <= pb) {
-      float eta = 1.0f + ta * r2, ie = 1.0f / eta;
-      if (r3 <= 4.0f * (ie - ie * ie)) return eta;
-    } else {
-      float eta = (ta + 1.0f) / (1.0f + ta * r2);
-      float ct = 1.0f - (eta - 1.0f) / alpha;
-      if (r3 <= 0.5f * (ct * ct + 1.0f / eta)) return eta;
-    }
-  }
 }
 
 // ------------------------------------------------------------------ warp helpers

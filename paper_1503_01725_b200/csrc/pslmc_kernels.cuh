@@ -311,8 +311,10 @@ __global__ void k_finalise(const long long *acc, const float *density, size_t n,
 }
 
 __global__ void k_philox_debug(unsigned long long seed, unsigned long long h, uint32_t track, uint32_t block, uint32_t *out) {
-  Philox r; r.init(seed, h, track, 0u); r.block(block);
-  out[0] = r.w0; out[1] = r.w1; out[2] = r.w2; out[3] = r.w3;
+  uint32_t ks[20];
+  for (int r = 0; r < 10; ++r) { ks[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; ks[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u; }
+  RngWin r; r.init(h, track, 0u);
+  r.gen(ks, block, out[0], out[1], out[2], out[3]);
 }
 
 }  // namespace pslmc
