@@ -76,14 +76,12 @@ void philox_block(uint64_t seed, uint64_t h, uint32_t track, uint32_t block, uin
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// Draw number n of the stream of (seed, history, track): word n&3 of block n>>2.
+// The stream of a track (seed, history, track) is its sequence of Philox blocks 0, 1, 2, ...  Every EVENT of the
+// track takes the next whole block and uses its first words in the order stated at the event; the words it does
+// not use are discarded (R1).  `j` = the next block.
 struct Stream {
-  uint64_t seed, h; uint32_t track, n;
-  uint32_t next() {
-    uint32_t w[4];
-    philox_block(seed, h, track, n >> 2, w);
-    return w[(n++) & 3];
-  }
+  uint64_t seed, h; uint32_t track, j;
+  void next_block(uint32_t w[4]) { philox_block(seed, h, track, j++, w); }
 };
 inline double U_co(uint32_t x) { return (double)(x >> 8) * (1.0 / 16777216.0); }          // [0,1)
 inline double U_oc(uint32_t x) { return (double)((x >> 8) + 1) * (1.0 / 16777216.0); }    // (0,1]
@@ -310,7 +308,9 @@ Sampled sample_history(const Psl &psl, const Beam &beam, const uint64_t *off, ui
   while (g + 1 < G && !(h >= off[g] && h < off[g + 1])) ++g;       // group of history h
   const Group &grp = psl.groups[g];
   Stream st{seed, h, 0, 0};
-  uint32_t x0 = st.next(), x1 = st.next(), x2 = st.next(), x3 = st.next(), y0 = st.next(), y1 = st.next();
+  uint32_t blk0[4], blk1[4];
+  st.next_block(blk0); st.next_block(blk1);           // blocks 0 and 1 of track 0 are the source draws
+  uint32_t x0 = blk0[0], x1 = blk0[1], x2 = blk0[2], x3 = blk0[3], y0 = blk1[0], y1 = blk1[1];
   // 1. let through the alias table
   uint64_t m = (uint64_t)x0 * (uint64_t)grp.thresh.size();
   uint32_t col = (uint32_t)(m >> 32), frac = (uint32_t)m;
@@ -335,7 +335,7 @@ Sampled sample_history(const Psl &psl, const Beam &beam, const uint64_t *off, ui
   if (psl.dir[s].K > 0) {
     // S4 / S5: direction from the Gaussian mixture of the PSR the position falls in
     const Psl::DirModel &dm = psl.dir[s];
-    uint32_t y2 = st.next();
+    uint32_t y2 = blk1[2];
     double r = std::sqrt(px * px + py * py);
     int i = (int)std::floor(r / p.ring_width); if (i > p.n_ring - 1) i = p.n_ring - 1;      // ring index of the position (:94)
     size_t base = ((size_t)grp.ebin * p.n_ring + i) * dm.K;
@@ -424,10 +424,13 @@ void rotate(double d[3], double ct, double st, double phi) {
   d[0] = nx / n; d[1] = ny / n; d[2] = nz / n;
 }
 
-// Kahn's rejection for Klein–Nishina; returns eta = E/E'.  Consumes 3 draws per trial.
-double kahn(double alpha, Stream &st) {
+// Kahn's rejection for Klein–Nishina; returns eta = E/E'.  One block per trial: words 0, 1, 2 = r1, r2, r3; word 3
+// of the ACCEPTED trial is returned in `w_phi` (the caller's azimuth draw).
+double kahn(double alpha, Stream &st, uint32_t &w_phi) {
   for (;;) {
-    double r1 = U_co(st.next()), r2 = U_co(st.next()), r3 = U_co(st.next());
+    uint32_t w[4]; st.next_block(w);
+    double r1 = U_co(w[0]), r2 = U_co(w[1]), r3 = U_co(w[2]);
+    w_phi = w[3];
     if (r1 <= (2.0 * alpha + 1.0) / (2.0 * alpha + 9.0)) {
       double eta = 1.0 + 2.0 * alpha * r2;
       if (r3 <= 4.0 * (1.0 / eta - 1.0 / (eta * eta))) return eta;
@@ -439,7 +442,7 @@ double kahn(double alpha, Stream &st) {
   }
 }
 
-struct Track { double pos[3], dir[3], E; int type; uint64_t h; uint32_t track, ndraw, nchild; };
+struct Track { double pos[3], dir[3], E; int type; uint64_t h; uint32_t track, nblk, nchild; };   // nblk: first stream block of the track's transport
 struct Event { uint32_t track; char code; double pos[3], dir[3], E, aux; };
 
 struct Ctx {
@@ -495,33 +498,34 @@ struct Ctx {
   void charged_secondary(const Track &parent, const double dir[3], double T, uint32_t slot, size_t v) {
     if (T >= ECUT && !(flags & FLAG_ELECTRONS_LOCAL)) {
       Track c; std::memcpy(c.pos, parent.pos, 24); std::memcpy(c.dir, dir, 24); c.E = T; c.type = 1; c.h = parent.h;
-      c.track = child_track(parent.track, parent.nchild, slot); c.ndraw = 0; c.nchild = 0;
+      c.track = child_track(parent.track, parent.nchild, slot); c.nblk = 0; c.nchild = 0;
       stack.push_back(c); ++res->n_sec_electrons;
     } else deposit(v, T);
   }
 
   void photon(Track t) {
     Fnv f; f.u32(t.track);
-    Stream st{seed, t.h, t.track, t.ndraw};
+    Stream st{seed, t.h, t.track, t.nblk};
     int ijk[3]; bool collided = false;
     if (!locate(t.pos, ijk) && !enter(t, ijk)) { escape(t.E); f.byte('M'); ev(t, 'M'); ++res->n_missed; fp += f.v; return; }
     for (;;) {
       if (t.E < PCUT) { deposit(vox(ijk), t.E); f.byte('A'); ev(t, 'A'); ++res->n_photon_cutoff; break; }
       double mmax = mu_max(t.E);
       if (!(mmax > 0.0)) { escape(t.E); f.byte('E'); ev(t, 'E'); ++res->n_photon_escape; if (!collided && t.track == 0) ++res->n_uncollided_escape; break; }
-      double s = -std::log(U_oc(st.next())) / mmax;
+      uint32_t wf[4]; st.next_block(wf);               // flight: word 0 = free path, word 1 = choice of interaction
+      double s = -std::log(U_oc(wf[0])) / mmax;
       for (int a = 0; a < 3; ++a) t.pos[a] += s * t.dir[a];
       ++res->n_flights;
       if (!locate(t.pos, ijk)) { escape(t.E); f.byte('E'); ev(t, 'E', s); ++res->n_photon_escape; if (!collided && t.track == 0) ++res->n_uncollided_escape; break; }
       size_t v = vox(ijk); double rho = ph.density[v]; int m = ph.material[v];
       double c[3]; mu_over_rho(m, t.E, c);
       double muC = rho * c[0], muT = rho * c[1], muK = rho * c[2];
-      double tt = U_co(st.next()) * mmax;
+      double tt = U_co(wf[1]) * mmax;
       if (tt < muC) {                                  // Compton, Klein–Nishina by Kahn
         collided = true; ++res->n_compton; f.byte('C');
-        double alpha = t.E / ME, eta = kahn(alpha, st);
+        uint32_t w_phi; double alpha = t.E / ME, eta = kahn(alpha, st, w_phi);
         double k = (eta - 1.0) / alpha, ct = 1.0 - k, sn = std::sqrt(std::fmax(0.0, k * (2.0 - k)));
-        double phi = 2.0 * PI * U_co(st.next());
+        double phi = 2.0 * PI * U_co(w_phi);
         double Ep = t.E / eta, T = t.E - Ep, d0[3] = {t.dir[0], t.dir[1], t.dir[2]};
         rotate(t.dir, ct, sn, phi);
         double de[3] = {t.E * d0[0] - Ep * t.dir[0], t.E * d0[1] - Ep * t.dir[1], t.E * d0[2] - Ep * t.dir[2]};
@@ -534,15 +538,16 @@ struct Ctx {
         ++res->n_photo; f.byte('P'); ev(t, 'P'); deposit(v, t.E); break;
       } else if (tt < muC + muT + muK) {               // pair production
         ++res->n_pair; f.byte('X'); ev(t, 'X');
-        double Tsum = t.E - E_PAIR, Tm = U_co(st.next()) * Tsum, Tp = Tsum - Tm;
+        uint32_t wp[4]; st.next_block(wp);             // pair: word 0 = energy split, 1 = cos, 2 = azimuth of the annihilation pair
+        double Tsum = t.E - E_PAIR, Tm = U_co(wp[0]) * Tsum, Tp = Tsum - Tm;
         charged_secondary(t, t.dir, Tm, 0, v);
         charged_secondary(t, t.dir, Tp, 1, v);
-        double cz = 2.0 * U_co(st.next()) - 1.0, sz = std::sqrt(std::fmax(0.0, 1.0 - cz * cz)), az = 2.0 * PI * U_co(st.next());
+        double cz = 2.0 * U_co(wp[1]) - 1.0, sz = std::sqrt(std::fmax(0.0, 1.0 - cz * cz)), az = 2.0 * PI * U_co(wp[2]);
         double nrm[3] = {sz * std::cos(az), sz * std::sin(az), cz};
         for (uint32_t slot = 2; slot < 4; ++slot) {
           Track c; std::memcpy(c.pos, t.pos, 24); double sg = slot == 2 ? 1.0 : -1.0;
           for (int a = 0; a < 3; ++a) c.dir[a] = sg * nrm[a];
-          c.E = E_ANNIH; c.type = 0; c.h = t.h; c.track = child_track(t.track, t.nchild, slot); c.ndraw = 0; c.nchild = 0;
+          c.E = E_ANNIH; c.type = 0; c.h = t.h; c.track = child_track(t.track, t.nchild, slot); c.nblk = 0; c.nchild = 0;
           stack.push_back(c); ++res->n_sec_photons;
         }
         ++t.nchild; break;
@@ -553,7 +558,7 @@ struct Ctx {
 
   void electron(Track t) {
     Fnv f; f.u32(t.track);
-    Stream st{seed, t.h, t.track, t.ndraw};
+    Stream st{seed, t.h, t.track, t.nblk};
     ++res->n_electron_tracks;
     int ijk[3]; uint32_t steps = 0;
     if (!locate(t.pos, ijk) && !enter(t, ijk)) { escape(t.E); f.u32(0); f.byte('M'); ev(t, 'M'); ++res->n_missed; fp += f.v; return; }
@@ -584,7 +589,8 @@ struct Ctx {
       if (turn) {
         double pbeta = Tms * (Tms + 2.0 * ME) / (Tms + ME);
         double th0 = 13.6 / pbeta * std::sqrt(tacc);
-        double a1 = U_oc(st.next()), b1 = U_co(st.next());
+        uint32_t wd[4]; st.next_block(wd);             // deflection: word 0 = Gaussian radius, word 1 = azimuth
+        double a1 = U_oc(wd[0]), b1 = U_co(wd[1]);
         double th = std::fmin(PI, th0 * std::sqrt(-2.0 * std::log(a1)));
         rotate(t.dir, std::cos(th), std::sin(th), 2.0 * PI * b1);
         fresh = true;
@@ -666,7 +672,7 @@ int32_t orc_dose(const void *h, const Phantom *ph, const Beam *beam, uint64_t N,
       Fnv f; f.u32(0); f.byte('J'); c.fp += f.v;
     } else {
       Track t; t.pos[0] = s.x; t.pos[1] = s.y; t.pos[2] = s.z; t.dir[0] = s.u; t.dir[1] = s.v; t.dir[2] = s.w; t.E = s.E;
-      t.type = psl.p.particle_type[stype]; t.h = hh; t.track = 0; t.ndraw = 8; t.nchild = 0;
+      t.type = psl.p.particle_type[stype]; t.h = hh; t.track = 0; t.nblk = 2; t.nchild = 0;
       c.stack.push_back(t); c.run_history();
     }
     if (fingerprints) fingerprints[hh - h_begin] += c.fp;
@@ -697,7 +703,7 @@ int32_t orc_dose_com(const void *h, const Phantom *ph, const Beam *beam, uint64_
     if (s.rejected) { c.ledger[3] += Ctx::quanta(s.E); ++res->n_jaw_rejected; continue; }
     c.com_col = orc_com_column(psl.p.n_ebin, psl.p.n_ring, psl.p.particle_type[g.stype], g.stype, g.ebin, s.ring);
     Track t; t.pos[0] = s.x; t.pos[1] = s.y; t.pos[2] = s.z; t.dir[0] = s.u; t.dir[1] = s.v; t.dir[2] = s.w; t.E = s.E;
-    t.type = psl.p.particle_type[g.stype]; t.h = hh; t.track = 0; t.ndraw = 8; t.nchild = 0;
+    t.type = psl.p.particle_type[g.stype]; t.h = hh; t.track = 0; t.nblk = 2; t.nchild = 0;
     c.fp = 0; c.stack.push_back(t); c.run_history();
   }
   c.store_ledgers();
@@ -713,7 +719,7 @@ int32_t orc_transport(const Phantom *ph, int32_t type, const double *particles, 
     const double *p = particles + 8 * i;
     if (p[7] < 0) continue;
     Track t; for (int a = 0; a < 3; ++a) { t.pos[a] = p[a]; t.dir[a] = p[3 + a]; }
-    t.E = p[6]; t.type = type; t.h = first + i; t.track = 0; t.ndraw = 8; t.nchild = 0;
+    t.E = p[6]; t.type = type; t.h = first + i; t.track = 0; t.nblk = 2; t.nchild = 0;
     c.ledger[0] += Ctx::quanta(t.E); c.fp = 0;
     c.stack.push_back(t); c.run_history();
     if (fingerprints) fingerprints[i] += c.fp;
@@ -730,7 +736,7 @@ int32_t orc_trace(const Phantom *ph, int32_t type, const double *particle, uint6
   std::vector<Event> tr;
   Ctx c; c.init(*ph); c.seed = seed; c.flags = flags; c.acc = acc.data(); c.res = &res; c.trace = &tr; if (fE > 0) c.fE = fE;
   Track t; for (int a = 0; a < 3; ++a) { t.pos[a] = particle[a]; t.dir[a] = particle[3 + a]; }
-  t.E = particle[6]; t.type = type; t.h = history; t.track = 0; t.ndraw = 8; t.nchild = 0;
+  t.E = particle[6]; t.type = type; t.h = history; t.track = 0; t.nblk = 2; t.nchild = 0;
   c.fp = 0; c.stack.push_back(t); c.run_history();
   for (size_t i = 0; i < tr.size() && (int32_t)i < max_events; ++i) {
     double *o = events + 10 * i; const Event &e = tr[i];
@@ -744,11 +750,12 @@ int32_t orc_trace(const Phantom *ph, int32_t type, const double *particle, uint6
 double orc_sigma_kn(double E) { return sigma_kn(E); }
 void orc_mu_over_rho(int32_t m, double E, double *out3) { mu_over_rho(m, E, out3); }
 double orc_stopping(int32_t m, double T) { return stopping(m, T); }
-// Kahn sampling at fixed E: stream of history first+i, track 0, starting at draw 0; 3 draws per trial.
+// Kahn sampling at fixed E: stream of history first+i, track 0, starting at block 0; one block per trial.
 void orc_kahn(double E, uint64_t seed, uint64_t first, uint64_t count, double *cos_out, double *eprime_out) {
   for (uint64_t i = 0; i < count; ++i) {
     Stream st{seed, first + i, 0, 0};
-    double alpha = E / ME, eta = kahn(alpha, st);
+    uint32_t w_phi;
+    double alpha = E / ME, eta = kahn(alpha, st, w_phi);
     cos_out[i] = 1.0 - (eta - 1.0) / alpha; eprime_out[i] = E / eta;
   }
 }

@@ -98,18 +98,18 @@ def test_kahn_matches_klein_nishina(orc, E):
     assert (ep / E).mean() == pytest.approx(mean_ratio, abs=5 * (ep / E).std() / math.sqrt(n))
 
 
-def test_kahn_draw_count_is_three_per_trial(orc):
-    """The photon azimuth is the draw after the accepted trial: trace one Compton and recompute."""
+def test_kahn_one_block_per_trial(orc):
+    """DESIGN.md R1: the flight is block 2 (words 0, 1), every Kahn trial takes one block (words 0-2) and the photon
+    azimuth is word 3 of the accepted trial's block: trace one Compton and recompute."""
     ph = one_voxel(orc)
     ev = orc.trace(ph, 0, [0, 0, 0, 0, 0, 1, 2.0, 0], 5, 99, flags=1)
     assert ev[0]["code"] == "C"
-    w = np.concatenate([orc.philox(99, 5, 0, b) for b in range(2, 12)])
-    u = (w >> 8) / 2.0 ** 24
     a = 2.0 / ME
-    i = 2                                  # draws 8, 9 were the flight distance and the selector
+    b = 3                                  # block 2 was the flight (distance, selector)
     while True:
-        r1, r2, r3 = u[i:i + 3]
-        i += 3
+        u = (orc.philox(99, 5, 0, b) >> 8) / 2.0 ** 24
+        r1, r2, r3 = u[:3]
+        b += 1
         if r1 <= (2 * a + 1) / (2 * a + 9):
             eta = 1 + 2 * a * r2
             ok = r3 <= 4 * (1 / eta - 1 / eta ** 2)
@@ -120,7 +120,7 @@ def test_kahn_draw_count_is_three_per_trial(orc):
         if ok:
             break
     ct = 1 - (eta - 1) / a
-    phi = 2 * math.pi * u[i]
+    phi = 2 * math.pi * u[3]
     assert ev[0]["aux"] == pytest.approx(ct, abs=1e-14)
     assert ev[0]["E"] == pytest.approx(2.0, abs=0)          # event logged with the pre-collision energy
     st = math.sqrt(max(0.0, 1 - ct * ct))

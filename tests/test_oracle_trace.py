@@ -26,8 +26,8 @@ def philox(seed, h, track, block):
     return c
 
 
-def draw(seed, h, track, n):
-    return philox(seed, h, track, n >> 2)[n & 3]
+def block(seed, h, track, j):
+    return philox(seed, h, track, j)
 
 
 def u_co(x):
@@ -60,7 +60,7 @@ def test_hand_trace_of_one_history(orc, opsl, cfg):
     assert grp["stype"] == 0                                                     # a primary photon
 
     # ---- source draw (S3-S5; Eq. 4-5)
-    x = [draw(seed, h, 0, n) for n in range(6)]
+    x = block(seed, h, 0, 0) + block(seed, h, 0, 1)[:2]                          # blocks 0, 1: the source draws
     m = x[0] * len(grp["ring"])
     col, frac = m >> 32, m & M32
     let = col if frac < int(grp["thresh"][col]) else int(grp["alias"][col])
@@ -95,15 +95,17 @@ def test_hand_trace_of_one_history(orc, opsl, cfg):
     mu_t = 1.0 * 2.77e-6 / E ** 3
     assert E < 1.022                                                             # no pair term at this energy
     mu = mu_c + mu_t                                                             # homogeneous water: mu_max = mu
-    s = -math.log(u_oc(draw(seed, h, 0, 8))) / mu                                # transport starts at draw 8
+    flight = block(seed, h, 0, 2)                                                # transport starts at block 2: one block per event
+    s = -math.log(u_oc(flight[0])) / mu
     site = [pos[i] + (t_in + s) * d[i] for i in range(3)]
     assert np.allclose(ev[0]["pos"], site, rtol=0, atol=2e-9), (ev[0]["pos"], site)
-    assert u_co(draw(seed, h, 0, 9)) * mu < mu_c                                 # Compton was the interaction chosen
-    # Kahn's rejection replayed: 3 draws per trial from draw 10 on, then one azimuth draw
-    a, n = E / ME, 10
+    assert u_co(flight[1]) * mu < mu_c                                           # Compton was the interaction chosen
+    # Kahn's rejection replayed: one block per trial from block 3 on (words 0-2), word 3 of the accepted trial = azimuth
+    a, n = E / ME, 3
     while True:
-        k1, k2, k3 = (u_co(draw(seed, h, 0, n + i)) for i in range(3))
-        n += 3
+        trial = block(seed, h, 0, n)
+        k1, k2, k3 = (u_co(w) for w in trial[:3])
+        n += 1
         if k1 <= (2 * a + 1) / (2 * a + 9):
             eta = 1 + 2 * a * k2
             if k3 <= 4 * (1 / eta - 1 / eta ** 2):
@@ -117,8 +119,8 @@ def test_hand_trace_of_one_history(orc, opsl, cfg):
     assert abs(ev[0]["aux"] - ct) < 1e-12                                        # the trace records cos(theta) of the scatter
     assert abs(float(np.dot(ev[0]["dir"], d)) - ct) < 1e-12                      # and the photon really turned by it
     assert abs(ev[1]["E"] - E / eta) < 1e-13                                     # Compton energy E' = E / eta
-    # the azimuth draw follows the accepted trial: the scattered direction's azimuth about d is 2 pi U
-    phi = 2.0 * math.pi * u_co(draw(seed, h, 0, n))
+    # the azimuth is word 3 of the accepted trial's block: the scattered direction's azimuth about d is 2 pi U
+    phi = 2.0 * math.pi * u_co(trial[3])
     sxy = math.hypot(d[0], d[1])
     e1 = np.array([d[0] * d[2] / sxy, d[1] * d[2] / sxy, -sxy])                  # the frame of DESIGN.md P8
     e2 = np.array([-d[1] / sxy, d[0] / sxy, 0.0])
