@@ -34,19 +34,16 @@ __constant__ Materials c_mat = {
     {1.0f / 36.08f, 1.0f / 36.08f, 1.0f / 27.2f}};
 
 // ------------------------------------------------------------------ R1: Philox4x32-10
-// The stream of a track, consumed through ONE generation site per event: window<K>() returns draws
-// n..n+3 of the track's stream without consuming them (the caller may consume up to K <= 4 of
-// them), generating at most one Philox block; consume(k, ...) advances.  c0..c3 cache the block that
-// holds draw n whenever n & 3 != 0.  Draw numbering is exactly DESIGN.md R1 (draw n = word n & 3 of
-// block n >> 2).
-struct RngWin {
-  uint32_t track, hlo, hhi, n;
-  uint32_t c0, c1, c2, c3;
-  __device__ __forceinline__ void init(uint64_t h, uint32_t trk, uint32_t ndraw) {
-    hlo = (uint32_t)h; hhi = (uint32_t)(h >> 32); track = trk; n = ndraw; c0 = c1 = c2 = c3 = 0u;   // ndraw & 3 == 0
+// The stream of a track (R1): blocks 0, 1, 2, ... of Philox4x32-10 keyed by the seed with counter
+// (block, track, history lo, history hi).  Every event takes the next whole block, so an event site is one
+// unconditional generation for all its lanes and the per-lane state is just the block counter.  ks = the 10
+// round keys (k0 + r*0x9E3779B9, k1 + r*0xBB67AE85), host-computed kernel parameters: the XORs take them straight
+// from the constant bank.
+struct Rng {
+  uint32_t track, hlo, hhi, blk;
+  __device__ __forceinline__ void init(uint64_t h, uint32_t trk, uint32_t first_block) {
+    hlo = (uint32_t)h; hhi = (uint32_t)(h >> 32); track = trk; blk = first_block;
   }
-  // ks = the 10 round keys (k0 + r*0x9E3779B9, k1 + r*0xBB67AE85), host-computed kernel parameters:
-  // the XORs then take them straight from the constant bank.
   __device__ __forceinline__ void gen(const uint32_t (&ks)[20], uint32_t j, uint32_t &g0, uint32_t &g1, uint32_t &g2, uint32_t &g3) const {
     uint32_t x0 = j, x1 = track, x2 = hlo, x3 = hhi;
 #pragma unroll
@@ -57,29 +54,8 @@ struct RngWin {
     }
     g0 = x0; g1 = x1; g2 = x2; g3 = x3;
   }
-  template <int K>
-  __device__ __forceinline__ void window(const uint32_t (&ks)[20], uint32_t &d0, uint32_t &d1, uint32_t &d2, uint32_t &d3,
-                                         uint32_t &g0, uint32_t &g1, uint32_t &g2, uint32_t &g3) {
-    const uint32_t s = n & 3u;
-    g0 = g1 = g2 = g3 = 0u;
-    if (s == 0u || s + K > 4u) gen(ks, (n + 3u) >> 2, g0, g1, g2, g3);
-    if (s == 0u) { c0 = g0; c1 = g1; c2 = g2; c3 = g3; }
-    d0 = s == 0u ? c0 : (s == 1u ? c1 : (s == 2u ? c2 : c3));
-    d1 = s == 0u ? c1 : (s == 1u ? c2 : (s == 2u ? c3 : g0));
-    d2 = s == 0u ? c2 : (s == 1u ? c3 : (s == 2u ? g0 : g1));
-    d3 = s == 0u ? c3 : (s == 1u ? g0 : (s == 2u ? g1 : g2));
-  }
-  // Streams that are only ever read two draws at a time from an even draw number (k_electron: one pair per
-  // deflection): the pair is words 0,1 of a fresh block or the cached words 2,3 of the last one.
-  __device__ __forceinline__ void pair(const uint32_t (&ks)[20], uint32_t &d0, uint32_t &d1) {
-    if ((n & 2u) == 0u) { uint32_t g0, g1; gen(ks, n >> 2, g0, g1, c2, c3); d0 = g0; d1 = g1; }
-    else { d0 = c2; d1 = c3; }
-    n += 2u;
-  }
-  __device__ __forceinline__ void consume(uint32_t k, uint32_t g0, uint32_t g1, uint32_t g2, uint32_t g3) {
-    const uint32_t m = n + k;
-    if ((m >> 2) != (n >> 2)) { c0 = g0; c1 = g1; c2 = g2; c3 = g3; }
-    n = m;
+  __device__ __forceinline__ void next(const uint32_t (&ks)[20], uint32_t &g0, uint32_t &g1, uint32_t &g2, uint32_t &g3) {
+    gen(ks, blk, g0, g1, g2, g3); ++blk;
   }
 };
 

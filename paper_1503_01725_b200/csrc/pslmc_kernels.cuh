@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
     }
     const int stype = (g >= m.n_ebin) + (g >= 2 * m.n_ebin), ebin = g - stype * m.n_ebin;     // three sub-sources
     ptype = m.particle_type[stype];
-    RngWin rng; rng.init(h, 0u, 0u);
+    Rng rng; rng.init(h, 0u, 0u);
     uint32_t x0, x1, x2, x3, y0, y1, y2, y3;
     rng.gen(a.ks, 0u, x0, x1, x2, x3);
     rng.gen(a.ks, 1u, y0, y1, y2, y3);
@@ -313,7 +313,7 @@ __global__ void k_finalise(const long long *acc, const float *density, size_t n,
 __global__ void k_philox_debug(unsigned long long seed, unsigned long long h, uint32_t track, uint32_t block, uint32_t *out) {
   uint32_t ks[20];
   for (int r = 0; r < 10; ++r) { ks[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; ks[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u; }
-  RngWin r; r.init(h, track, 0u);
+  Rng r; r.init(h, track, 0u);
   r.gen(ks, block, out[0], out[1], out[2], out[3]);
 }
 

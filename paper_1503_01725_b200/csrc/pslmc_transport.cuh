@@ -219,7 +219,7 @@ __device__ __forceinline__ unsigned refill_index(const TransportArgs &a, bool id
   return (idle && rank < avail) ? idx : 0xffffffffu;
 }
 
-struct TrackIn { float x, y, z, u, v, w, E; unsigned long long h; uint32_t track, ndraw, col; bool ok; };
+struct TrackIn { float x, y, z, u, v, w, E; unsigned long long h; uint32_t track, blk, col; bool ok; };
 
 __device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned idx, unsigned n1) {
   TrackIn t;
@@ -230,12 +230,12 @@ __device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned i
     if (a.buffer_is_debug) { tt = idx; t.ok = B.w >= 0.0f; }
     else { const unsigned bits = __float_as_uint(B.w); tt = bits & 0x7fffffffu; t.ok = (int)(bits >> 31) == a.want_type; }
     t.h = history_of(a.first + tt, a.perm_a, a.n_total);
-    t.track = 0u; t.ndraw = 8u; t.col = a.p2 ? a.p2[idx] : 0u;
+    t.track = 0u; t.blk = 2u; t.col = a.p2 ? a.p2[idx] : 0u;      // blocks 0, 1 were the source draws
   } else {
     if (a.src_kind == SRC_BUFFER) idx -= n1;
     const float4 A = a.src.a[idx], B = a.src.b[idx]; const uint4 C = a.src.c[idx];
     t.x = A.x; t.y = A.y; t.z = A.z; t.E = A.w; t.u = B.x; t.v = B.y; t.w = B.z;
-    t.h = ((unsigned long long)C.y << 32) | C.x; t.track = C.z; t.ndraw = 0u; t.col = C.w; t.ok = true;
+    t.h = ((unsigned long long)C.y << 32) | C.x; t.track = C.z; t.blk = 0u; t.col = C.w; t.ok = true;
   }
   return t;
 }
@@ -271,7 +271,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
   float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, E = 0;
   int cvox = 0;                                          // voxel of the current position
   unsigned long long h = 0; uint32_t nchild = 0;
-  RngWin rng; rng.init(0ull, 0u, 0u);
+  Rng rng; rng.init(0ull, 0u, 0u);
   Fnv fnv; fnv.v = 0;
 
   for (;;) {
@@ -282,7 +282,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
       if (t.ok) {
         x = t.x; y = t.y; z = t.z; u = t.u; v = t.v; w = t.w; E = t.E; h = t.h; nchild = 0; collided = false;
         if (DBG && g.com_index) { pend.flush(g, stage); pend.col = t.col; }
-        rng.init(h, t.track, t.ndraw);
+        rng.init(h, t.track, t.blk);
         if (DBG) fnv.init(t.track);
         if (a.buffer_is_debug) tl.inc += (unsigned long long)quanta(E);
         int vi, vj, vk;
@@ -312,9 +312,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
         if (DBG) { fnv.byte('E'); ++tl.st[ST_PESC]; if (!collided && rng.track == 0u) ++tl.st[ST_UNCOLLIDED]; }
         done = true;
       } else {
-        uint32_t d0, d1, d2, d3, g0, g1, g2, g3;
-        rng.window<2>(a.ks, d0, d1, d2, d3, g0, g1, g2, g3);
-        rng.consume(2u, g0, g1, g2, g3);
+        uint32_t d0, d1, d2, d3;
+        rng.next(a.ks, d0, d1, d2, d3);                  // flight block: free path, choice of interaction
         const float s = -logf(u_oc(d0)) / mu_max;
         x = __fmaf_rn(s, u, x); y = __fmaf_rn(s, v, y); z = __fmaf_rn(s, w, z);
         if (DBG) ++tl.st[ST_FLIGHTS];
@@ -348,8 +347,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
     bool push_e = false, push_p = false; float ex = 0, ey = 0, ez = 0, eT = 0; uint32_t etrack = 0;
     float pairT[2] = {0.f, 0.f};
     if (state >= PH_KAHN) {
-      uint32_t d0, d1, d2, d3, g0, g1, g2, g3;
-      rng.window<4>(a.ks, d0, d1, d2, d3, g0, g1, g2, g3);
+      uint32_t d0, d1, d2, d3;
+      rng.next(a.ks, d0, d1, d2, d3);                    // trial block (r1, r2, r3, azimuth) or pair block (split, cos, azimuth)
       if (state == PH_KAHN) {
         // Kahn's rejection (P5).  With dn = 1 + 2 alpha r2:  branch A: eta = dn, branch B:
         // eta = (2 alpha + 1)/dn.  k = (eta - 1)/alpha is 2 r2 (A) or 2 (1 - r2)/dn (B) in exact
@@ -363,7 +362,6 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
         const float ct = 1.0f - k;
         const bool accept = brA ? (r3 <= 4.0f * (ie - ie * ie)) : (r3 <= 0.5f * (ct * ct + ie));
         if (accept) {
-          rng.consume(4u, g0, g1, g2, g3);
           const float sn = sqrt_fast(fmaxf(0.0f, k * (2.0f - k)));
           const float Ep = E * ie, T = E - Ep, u0 = u, v0 = v, w0 = w;
           rotate(u, v, w, ct, sn, u_co(d3));
@@ -379,9 +377,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
             if (DBG) ++tl.st[ST_DEPOSITS];
           }
           ++nchild; E = Ep; state = PH_FLIGHT;
-        } else rng.consume(3u, g0, g1, g2, g3);
+        }
       } else {                                           // pair production: the pushes happen below, convergently
-        rng.consume(3u, g0, g1, g2, g3);
         const float Tsum = E - kEPair, Tm = u_co(d0) * Tsum, Tp = Tsum - Tm;
         const float Tc[2] = {Tm, Tp};
 #pragma unroll
@@ -459,7 +456,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
   unsigned long long h = 0; uint32_t steps = 0;
   // condensed step (P7): energy still to lose in it, rho*s/X0 accumulated, energy at its start
   float budget = 0, tacc = 0, Tms = 0; bool fresh = true;
-  RngWin rng; rng.init(0ull, 0u, 0u);
+  Rng rng; rng.init(0ull, 0u, 0u);
   Fnv fnv; fnv.v = 0;
 
   for (;;) {
@@ -470,7 +467,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
         float x = t.x, y = t.y, z = t.z;
         u = t.u; v = t.v; w = t.w; T = t.E; h = t.h; steps = 0; fresh = true;
         if (DBG && g.com_index) { pend.flush(g, stage); pend.col = t.col; }
-        rng.init(h, t.track, t.ndraw);
+        rng.init(h, t.track, t.blk);
         if (DBG) { fnv.init(t.track); ++tl.st[ST_ETRACKS]; }
         if (a.buffer_is_debug) tl.inc += (unsigned long long)quanta(T);
         active = true;
@@ -520,8 +517,8 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
           if (DBG) { fnv.u32(steps); fnv.byte('E'); ++tl.st[ST_EESC]; }
           done = true;
         } else if (turn) {
-          uint32_t d0, d1;
-          rng.pair(a.ks, d0, d1);
+          uint32_t d0, d1, d2, d3;
+          rng.next(a.ks, d0, d1, d2, d3);                // deflection block: Gaussian radius, azimuth
           // theta = (13.6 / p beta) sqrt(tacc) sqrt(-2 ln a), p beta = Tms (Tms + 2 me)/(Tms + me): one division, one root
           const float c = __fdividef(13.6f * (Tms + kMe), Tms * (Tms + 2.0f * kMe));
           const float th = fminf(kPi, c * sqrt_fast(tacc * (-2.0f * __logf(u_oc(d0)))));
