@@ -204,7 +204,7 @@ int  mc_sample_debug(const psl_t *psl, const beam_geom_t *beam, uint64_t first_h
 
 /* Transport only.  Takes `count` particles in the layout of mc_sample_debug (status < 0 entries
  * are skipped), particle_type 0 photon / 1 electron, as track 0 of histories first_history + i
- * with the stream positioned at draw 8, and scores into opts->dose_acc (required).  Ledgers and
+ * with the stream positioned at block 2, and scores into opts->dose_acc (required).  Ledgers and
  * counters go to mc_stats; the incident ledger counts the particles given.                      */
 int  mc_transport_debug(const phantom_t *ph, int32_t particle_type, const float *soa_in,
                         uint64_t first_history, uint64_t count, uint64_t seed,
