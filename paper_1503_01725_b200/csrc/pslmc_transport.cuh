@@ -500,12 +500,12 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
       ++steps;
       if (DBG) { ++tl.st[ST_ESTEPS]; ++tl.st[ST_DEPOSITS]; }
       bool done = false;
-      if (T - dT <= kEcut) {
-        const long long q = quanta(T); pend.add(g, stage, vox, q); tl.dep += (unsigned long long)q;
+      const bool stop = T - dT <= kEcut;               // below the cut-off after this sub-step: everything left is deposited here
+      const long long q = quanta(stop ? T : dT); pend.add(g, stage, vox, q); tl.dep += (unsigned long long)q;
+      if (stop) {
         if (DBG) { fnv.u32(steps); fnv.byte('A'); }
         done = true;
       } else {
-        const long long q = quanta(dT); pend.add(g, stage, vox, q); tl.dep += (unsigned long long)q;
         lx = __fmaf_rn(s, u, lx); ly = __fmaf_rn(s, v, ly); lz = __fmaf_rn(s, w, lz);
         T -= dT; budget -= dT; tacc = __fmaf_rn(rho * s, c_mat.inv_x0[mt], tacc);
         // re-home: a step ends at most eps beyond the face it was limited by
