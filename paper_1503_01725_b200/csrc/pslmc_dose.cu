@@ -45,7 +45,7 @@ static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 // Workspace layout for a batch of B primaries.  Shared by the whole call: group offsets, cross-section
 // data, packed phantom, (optionally) the int64 dose grid.  Per pipeline (kMaxPipes of them, see run_dose):
 // control block, the particle buffer (2 planes), the electron queue (capacity 4B) and the two photon
-// queues (capacity B each), 3 planes per queue.
+// queues (capacity 2B each: cannot overflow), 3 planes per queue.
 constexpr int kMaxPipes = 2;
 struct Layout {
   size_t ctl, off, xs, vox, p0, p1, p2, eq[3], pq[2][3], acc, total;
@@ -54,7 +54,9 @@ struct Layout {
 static void make_layouts(uint64_t batch, size_t nvox, bool with_acc, Layout out[kMaxPipes]) {
   Layout L; size_t o = 0;
   auto take = [&](size_t b) { size_t at = o; o += align_up(b); return at; };
-  L.eq_cap = (unsigned)std::min<uint64_t>(4 * batch, 0x7fffffffu); L.pq_cap = (unsigned)batch;
+  L.eq_cap = (unsigned)std::min<uint64_t>(4 * batch, 0x7fffffffu);
+  if (const char *e = getenv("PSLMC_TEST_EQ_CAP")) L.eq_cap = (unsigned)std::max(1, atoi(e));   // test hook: exercises MC_E_OVERFLOW (the planes keep their full size)
+  L.pq_cap = (unsigned)std::min<uint64_t>(2 * batch, 0x7fffffffu);   // a photon converts at most once: two annihilation photons each, never more
   L.off = take(sizeof(uint64_t) * 160); L.xs = take(kXsBytes); L.vox = take(4 * nvox);
   L.acc = take(with_acc ? 8 * nvox : 0);
   for (int p = 0; p < kMaxPipes; ++p) {

@@ -198,3 +198,35 @@ def test_transport_electron_beam(B, orc, wl):
     out = run_transport(B, orc, wl.slab_phantom(48, 0.25), 1, rows, 0, 9)
     assert_close_run(*out)
     assert out[1]["n_missed"] == 5 and out[1]["n_electron_tracks"] == n
+
+
+def test_queue_overflow_is_reported_not_corrupting(B, orc, monkeypatch):
+    """The electron queue holds 4 entries per batch particle: enough for any source this library is for (2.3 per 6 MeV
+    photon in bone, measured; still below 4 at 50 MeV).  With the capacity cut by the test hook PSLMC_TEST_EQ_CAP the call
+    must fail with MC_E_OVERFLOW, write nothing out of bounds, and leave the library usable.  The photon queue (2 per
+    batch particle: a photon converts at most once) cannot overflow."""
+    import torch
+    n = 64
+    ph = dict(nx=n, ny=n, nz=n, dx=1.0, dy=1.0, dz=1.0, ox=-32.0, oy=-32.0, oz=0.0,
+              density=np.full(n ** 3, 1.85, np.float32), material=np.full(n ** 3, 2, np.uint8))
+    dph = B.DevicePhantom(ph)
+
+    def run(E, cnt=20000):
+        soa = np.zeros((2, cnt, 4), np.float32); soa[0, :, 2] = 1.0; soa[0, :, 3] = E; soa[1, :, 2] = 1.0
+        acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
+        B.transport_debug(dph, 0, torch.as_tensor(soa).cuda(), 0, 5, acc)
+        return acc, B.stats()
+
+    a0, st0 = run(6.0)
+    assert st0["queue_high_water"][0] < 4 * 20000 and st0["n_pair"] > 0
+    monkeypatch.setenv("PSLMC_TEST_EQ_CAP", "1000")
+    with pytest.raises(B.PslmcError) as e:
+        run(6.0)
+    assert e.value.code == -5
+    monkeypatch.delenv("PSLMC_TEST_EQ_CAP")
+    a1, st1 = run(6.0)                                     # same bits as before the failed call
+    assert torch.equal(a0, a1) and st0["ledger"] == st1["ledger"]
+    # pair-dominated energies: two photon-queue entries per conversion, never more than 2 per batch particle
+    a2, st2 = run(50.0, cnt=5000)
+    assert st2["n_pair"] > 2500 and st2["n_sec_photons"] == 2 * st2["n_pair"] and st2["queue_high_water"][1] <= 2 * 5000
+    assert st2["queue_high_water"][0] < 4 * 5000
