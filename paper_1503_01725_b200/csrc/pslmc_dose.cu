@@ -495,10 +495,12 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
       const uint64_t lo = std::max(hb, off[(size_t)s * ne]), hi = std::min(he, off[(size_t)(s + 1) * ne]);
       if (lo >= hi) continue;
       g_stats.n_hist[s] = hi - lo;
-      for (uint64_t first = lo; first < hi; first += batch, ++task) {
+      // equal batches: ceil(n / batch) launches of the same size (a short last batch is mostly tail)
+      const uint64_t nb = (hi - lo + batch - 1) / batch, even = std::min(batch, (((hi - lo + nb - 1) / nb) + kThreads - 1) / kThreads * kThreads);
+      for (uint64_t first = lo; first < hi; first += even, ++task) {
         const int p = (int)(task % npipe); Run &r = pipes[p];
         if (P->psr.particle_type[s] != 0 && r.pq_pending) { r.next_batch(); r.drain_photon_queue(); }   // no photon launch ahead to carry them
-        sample_batch(p, first, std::min(batch, hi - first));
+        sample_batch(p, first, std::min(even, hi - first));
         if (P->psr.particle_type[s] == 0) r.transport_photon_batch(first);
         else r.transport_electron_buffer(first, false, &r.ctl->n_pb, &r.ctl->head_pb);
       }
