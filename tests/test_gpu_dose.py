@@ -257,3 +257,25 @@ def test_full_size_c1_in_the_bench_configuration(B, orc, gpsl, opsl, cfg):
     acc3 = torch.zeros_like(acc)
     gpsl("C1").dose(dph, c["beams"][0], N, seed, batch=1 << 18, dose_acc=acc3, pipelines=1)
     assert torch.equal(acc, acc3) and B.stats()["ledger"] == L
+
+
+def test_ledgers_beyond_64_bits(B, gpsl, cfg):
+    """2^33 histories on C0: the energy ledgers pass 2^64 quanta (128-bit sums in the control block, folded on the host);
+    the integer identity sum(acc) == deposited and energy conservation still hold, and the result is the sum of two halves."""
+    import torch
+    c = cfg("C0")
+    dph = B.DevicePhantom(c["phantom"])
+    N = 1 << 33
+    acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
+    gpsl("C0").dose(dph, c["beams"][0], N, 3, batch=1 << 23, dose_acc=acc)
+    L = B.stats()["ledger"]
+    assert L["incident"] > 1 << 64 and L["deposited"] > 1 << 62
+    total = sum(int(v) for v in acc.cpu().numpy().astype(object))
+    assert total == L["deposited"]
+    assert abs(L["deposited"] + L["escaped"] + L["jaw"] - L["incident"]) <= 1e-5 * L["incident"]
+    acc2 = torch.zeros_like(acc)
+    led = 0
+    for hb, he in ((0, N // 2), (N // 2, N)):
+        gpsl("C0").dose(dph, c["beams"][0], N, 3, batch=1 << 22, dose_acc=acc2, history_begin=hb, history_end=he)
+        led += B.stats()["ledger"]["deposited"]
+    assert torch.equal(acc, acc2) and led == L["deposited"]
