@@ -3,11 +3,15 @@
  *
  * The operations are those of Tian et al., "An Analytic Linear Accelerator Source Model for Monte
  * Carlo dose calculations. II", in the reading fixed by DESIGN.md:
- *   psl_build          PAPER.md:35-57  §2.1.1 (PSR→PSL conversion, Eq. 1-2),
+ *   psl_build          PAPER.md:35-57  §2.1.1 (PSR→PSL conversion, Eq. 1-2; ring-sector lets),
  *                      PAPER.md:61-69  §2.1.2 (sampling areas), :75-80 S1-S2 (Eq. 3)
+ *   psl_build_grid     PAPER.md:39-55  the paper's own Cartesian (Xbin, Ybin) lets, steps 1-4
+ *   psl_set_direction_model  PAPER.md:94-116 S4-S5, Eq. 6-7 (Gaussian mixtures in (alpha, beta))
+ *   mc_plan_allocate   PAPER.md:76-80  Eq. 3 across the beams of a plan
  *   mc_sample_debug    PAPER.md:82-92  S3 (Eq. 4-5), :94-116 S4-S5, jaw rejection :65/:92, set-up :173
  *   mc_dose            PAPER.md:118-120 §2.1.3 (iterated source kernel / transport kernel, M per
  *                      launch, type-major / energy-ascending order), :161 (cut-offs 50 keV / 200 keV)
+ *                      mc_opts_t.com_*: the commissioning tally, §2.2.2
  *   mc_stats           PAPER.md:177-191 Table 1 (per-phase timing breakdown)
  *
  * Conventions
@@ -21,7 +25,7 @@
  *   - Calls on one psl_t are not re-entrant.  mc_dose is synchronous with respect to the given
  *     stream when it returns.
  *   - Determinism: for fixed inputs and seed, dose, ledgers and counters are bitwise identical for
- *     every `batch`, every `order` and every partition [history_begin,history_end) summed.
+ *     every `batch`, every `order`, every `pipelines` and every partition [history_begin,history_end) summed.
  *   - There is no CPU fallback: every entry point that computes needs a CUDA device (sm_100a).
  */
 #ifndef PSLMC_H
