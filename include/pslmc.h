@@ -221,6 +221,11 @@ int  mc_transport_debug(const phantom_t *ph, int32_t particle_type, const float 
  * ln^2(E/1.022) or 0 below threshold, mu_max cm^-1) per energy.                                  */
 int  mc_xs_debug(const float rhomax[3], double e_max, const float *E_host, uint64_t n, float *out_host);
 
+/* Measurement probe: the rate of nothing but int64 scoring atomics (RED.64) on pseudo-random voxels of a grid of
+ * nvox voxels — the ceiling the scoring of the transport kernels is compared with.  acc: DEVICE int64[nvox] (its
+ * contents are destroyed).  ms_out: HOST float[2] = (milliseconds by CUDA events, atomics actually issued).     */
+int  mc_atomic_peak_debug(int64_t *acc, uint64_t nvox, uint64_t n_ops, uint64_t seed, float *ms_out);
+
 /* One Philox4x32-10 block computed ON THE DEVICE: key = seed, counter = (block, track, h_lo, h_hi).
  * out: HOST u32[4].                                                                             */
 int  mc_philox_debug(uint64_t seed, uint64_t history, uint32_t track, uint32_t block,

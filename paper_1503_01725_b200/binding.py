@@ -19,7 +19,7 @@ MC_FLAG_ELECTRONS_LOCAL, MC_FLAG_STATS, MC_FLAG_TIMING, MC_FLAG_STATIC_LANES, MC
 LEDGERS = ("incident", "deposited", "escaped", "jaw")
 KERNEL_CLASSES = ("sample", "photon", "electron", "finalise", "aux")
 EXPORTS = ("psl_build", "psl_build_grid", "psl_set_direction_model", "mc_plan_allocate", "psl_free", "psl_export", "psl_allocate", "mc_workspace_bytes", "mc_dose", "mc_dose_host",
-           "mc_stats", "mc_last_error", "mc_sample_debug", "mc_transport_debug", "mc_philox_debug", "mc_xs_debug")
+           "mc_stats", "mc_last_error", "mc_sample_debug", "mc_transport_debug", "mc_philox_debug", "mc_xs_debug", "mc_atomic_peak_debug")
 
 
 class PslmcError(RuntimeError):
@@ -97,6 +97,7 @@ def lib():
         L.mc_transport_debug.argtypes = [C.POINTER(phantom_t), C.c_int32, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64,
                                          C.POINTER(mc_opts_t)]
         L.mc_philox_debug.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
+        L.mc_atomic_peak_debug.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64, C.c_void_p]
         L.mc_xs_debug.argtypes = [C.c_void_p, C.c_double, C.c_void_p, C.c_uint64, C.c_void_p]
         _lib = L
     return _lib
@@ -306,6 +307,15 @@ def plan_dose(psls, phantom, beams, n_histories: int, seed: int, batch: int = 1 
             continue
         psl.dose(phantom, beam, n, seed + i, batch=batch, dose_acc=acc, history_begin=hb, history_end=he, **opt)
     return acc, n_beam
+
+
+def atomic_peak(nvox: int, n_ops: int = 1 << 28, seed: int = 1) -> float:
+    """int64 scoring atomics per second on random voxels of an nvox grid (measurement probe)."""
+    import torch
+    acc = torch.zeros(nvox, dtype=torch.int64, device="cuda")
+    out = np.zeros(2, np.float32)
+    _check(lib().mc_atomic_peak_debug(acc.data_ptr(), nvox, n_ops, seed, out.ctypes.data_as(C.c_void_p)))
+    return float(out[1]) / (float(out[0]) * 1e-3)
 
 
 def shard_range(n_histories: int, rank: int, world: int) -> tuple[int, int]:

@@ -717,6 +717,24 @@ extern "C" int mc_xs_debug(const float rhomax[3], double e_max, const float *E_h
   return MC_OK;
 }
 
+extern "C" int mc_atomic_peak_debug(int64_t *acc, uint64_t nvox, uint64_t n_ops, uint64_t seed, float *ms_out) {
+  if (!acc || !ms_out || nvox == 0 || nvox >= 0x7fffffffull || n_ops == 0) return fail(MC_E_INVALID_ARG, "mc_atomic_peak_debug: invalid argument");
+  int dev = 0, sms = 0; CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const unsigned blocks = (unsigned)sms * 8, threads = blocks * kThreads;
+  const unsigned per_thread = (unsigned)std::max<uint64_t>(1, n_ops / threads);
+  cudaEvent_t e0, e1; CUDA_TRY(cudaEventCreate(&e0)); CUDA_TRY(cudaEventCreate(&e1));
+  k_atomic_peak<<<blocks, kThreads>>>((unsigned long long *)acc, (unsigned)nvox, 16u, (unsigned)seed);      // warm-up
+  CUDA_TRY(cudaEventRecord(e0));
+  k_atomic_peak<<<blocks, kThreads>>>((unsigned long long *)acc, (unsigned)nvox, per_thread, (unsigned)seed + 1u);
+  CUDA_TRY(cudaEventRecord(e1));
+  CUDA_TRY(cudaEventSynchronize(e1));
+  CUDA_TRY(cudaEventElapsedTime(ms_out, e0, e1));
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  ms_out[1] = (float)((double)per_thread * threads);
+  return MC_OK;
+}
+
 extern "C" int mc_philox_debug(uint64_t seed, uint64_t history, uint32_t track, uint32_t block, uint32_t *out) {
   if (!out) return fail(MC_E_INVALID_ARG, "mc_philox_debug: null argument");
   uint32_t *d = nullptr;

@@ -293,6 +293,16 @@ __global__ void k_build_xs(const Control *c, float *data, double x0, double h, i
   data[kXsHead + i] = (float)skn;
 }
 
+// Measurement probe: nothing but int64 scoring atomics on pseudo-random voxels of [0, nvox) - the ceiling the scoring of
+// the transport kernels is compared with.  Each thread issues `per_thread` REDs.
+__global__ void k_atomic_peak(unsigned long long *acc, unsigned nvox, unsigned per_thread, unsigned seed) {
+  unsigned x = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + seed;
+  for (unsigned i = 0; i < per_thread; ++i) {
+    x = x * 1664525u + 1013904223u;
+    atomicAdd(acc + (unsigned)(((unsigned long long)(x ^ (x >> 15)) * nvox) >> 32), 1ull + i);
+  }
+}
+
 // Parity probe: the table lookup k_photon does, for a list of energies.  out: (sigma_KN, ln^2(E/1.022), mu_max) per energy.
 __global__ void k_xs_debug(XsTable xs, const float *E, size_t n, float *out) {
   const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
