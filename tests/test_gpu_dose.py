@@ -279,3 +279,50 @@ def test_ledgers_beyond_64_bits(B, gpsl, cfg):
         gpsl("C0").dose(dph, c["beams"][0], N, 3, batch=1 << 22, dose_acc=acc2, history_begin=hb, history_end=he)
         led += B.stats()["ledger"]["deposited"]
     assert torch.equal(acc, acc2) and led == L["deposited"]
+
+
+# ---------------------------------------------------------------- degenerate inputs
+def test_degenerate_phantoms_and_sources(B, orc, cfg, wl):
+    """All-vacuum and single-voxel phantoms, an off-axis asymmetric field, and a model whose electron sub-source has no
+    weight: tables bit-exact, sequences and ledgers as the oracle's."""
+    c = cfg("C1", False)
+    # (1) off-axis asymmetric jaws
+    jaws = dict(c["jaws"], x1=1.0, x2=6.0, y1=-3.0, y2=0.5)
+    g, o = B.Psl(c["psr"], jaws, 16), orc.Psl(c["psr"], jaws, 16)
+    ex = g.export()
+    assert np.array_equal(ex["rect"], o.rect())
+    for gi, gg in enumerate(ex["groups"]):
+        og = o.group(gi)
+        assert gg["W"] == og["W"] and all(np.array_equal(gg[k], og[k]) for k in ("ring", "sector", "thresh", "alias"))
+    n = 40
+    ph = dict(nx=n, ny=n, nz=n, dx=0.5, dy=0.5, dz=0.5, ox=-10.0, oy=-10.0, oz=0.0,
+              density=np.ones(n ** 3, np.float32), material=np.zeros(n ** 3, np.uint8))
+    same, _, _ = compare_with_oracle(B, orc, g, o, ph, c["beams"][0], 300_000, 5, batch=1 << 16, frac_vox=0.98)
+    acc = gpu_dose(B, g, B.DevicePhantom(ph), c["beams"][0], 300_000, 5, 1 << 16, want_fp=False)[0].reshape(n, n, n)
+    assert acc[:, :, 22:32].sum() > 20 * acc[:, :, 0:10].sum()               # the dose sits at positive x
+    # (2) all vacuum: nothing is deposited, everything that passes the jaws escapes
+    vac = dict(ph, density=np.zeros(n ** 3, np.float32))
+    dph = B.DevicePhantom(vac)
+    acc, dose, st, fp = gpu_dose(B, g, dph, c["beams"][0], 50_000, 6, 1 << 14)
+    oacc, ores, ofp = o.dose(orc.Phantom(vac), c["beams"][0], 50_000, 6, fingerprints=True)
+    # (primaries sampled below the 50 keV cut-off are absorbed in their entry voxel even in vacuum: energy deposited, dose 0)
+    assert not dose.any() and np.array_equal(fp, ofp) and np.array_equal(acc != 0, oacc != 0)
+    assert abs(st["ledger"]["deposited"] - ores["ledger"]["deposited"]) <= 1e-6 * ores["ledger"]["incident"]
+    assert st["ledger"]["deposited"] < 1e-3 * st["ledger"]["incident"] and st["n_flights"] == 0
+    assert st["ledger"]["deposited"] + st["ledger"]["escaped"] + st["ledger"]["jaw"] == st["ledger"]["incident"]
+    # (3) one voxel
+    one = dict(nx=1, ny=1, nz=1, dx=30.0, dy=30.0, dz=30.0, ox=-15.0, oy=-15.0, oz=0.0,
+               density=np.ones(1, np.float32), material=np.zeros(1, np.uint8))
+    acc, dose, st, fp = gpu_dose(B, g, B.DevicePhantom(one), c["beams"][0], 50_000, 7, 1 << 14)
+    oacc, ores, ofp = o.dose(orc.Phantom(one), c["beams"][0], 50_000, 7, fingerprints=True)
+    assert (fp == ofp).mean() >= 0.999 and abs(int(acc[0]) - int(oacc[0])) <= 1e-3 * int(oacc[0]) and int(acc[0]) == st["ledger"]["deposited"]
+    # (4) a sub-source without weight: its groups are empty, its histories do not exist
+    psr = dict(c["psr"], W=np.array(c["psr"]["W"], copy=True))
+    psr["W"][2] = 0.0
+    g2, o2 = B.Psl(psr, c["jaws"], 16), orc.Psl(psr, c["jaws"], 16)
+    N = 100_000
+    off = g2.allocate(N)
+    assert np.array_equal(off, o2.allocate(N)) and off[2 * psr["n_ebin"]] == N
+    acc, dose, st, fp = gpu_dose(B, g2, B.DevicePhantom(ph), c["beams"][0], N, 8, 1 << 15)
+    oacc, ores, ofp = o2.dose(orc.Phantom(ph), c["beams"][0], N, 8, fingerprints=True)
+    assert st["n_hist"] == ores["n_hist"] and st["n_hist"][2] == 0 and (fp == ofp).mean() >= 0.999
