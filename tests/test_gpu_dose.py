@@ -326,3 +326,30 @@ def test_degenerate_phantoms_and_sources(B, orc, cfg, wl):
     acc, dose, st, fp = gpu_dose(B, g2, B.DevicePhantom(ph), c["beams"][0], N, 8, 1 << 15)
     oacc, ores, ofp = o2.dose(orc.Phantom(ph), c["beams"][0], N, 8, fingerprints=True)
     assert st["n_hist"] == ores["n_hist"] and st["n_hist"][2] == 0 and (fp == ofp).mean() >= 0.999
+
+
+@pytest.mark.parametrize("name,beam,seed", [("C2", 0, 3), ("C3", 3, 43), ("C4", 0, 5)])
+def test_full_size_sampled_parity_c2_c3_c4(name, beam, seed, B, orc, cfg):
+    """BASELINE.json's other configurations at their full history counts (1e8, 1e8 per beam, 1e9) in the bench launch
+    configuration: the fingerprints of sampled history ranges against the oracle, and the ledger identities."""
+    import torch
+    c = cfg(name)
+    N = c["n_histories"]
+    g, o = B.Psl(c["psr"], c["jaws"], c["n_sectors"]), orc.Psl(c["psr"], c["jaws"], c["n_sectors"])
+    dph, oph = B.DevicePhantom(c["phantom"]), orc.Phantom(c["phantom"])
+    fp = torch.zeros(N, dtype=torch.int64, device="cuda")
+    acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
+    g.dose(dph, c["beams"][beam], N, seed, batch=1 << 22, dose_acc=acc, fingerprints=fp)
+    L = B.stats()["ledger"]
+    assert int(acc.sum().item()) == L["deposited"]
+    assert abs(L["deposited"] + L["escaped"] + L["jaw"] - L["incident"]) <= 1e-5 * L["incident"]
+    same = total = 0
+    oacc = np.zeros(oph.nvox, np.int64)
+    for i in range(48):
+        a = int(i * N / 48) + 911
+        gfp = fp[a:a + 1000].cpu().numpy().view(np.uint64)
+        _, _, ofp = o.dose(oph, c["beams"][beam], N, seed, h_begin=a, h_end=a + 1000, acc=oacc, fingerprints=True)
+        same += int((gfp == ofp).sum()); total += 1000
+    _, _, ofp = o.dose(oph, c["beams"][beam], N, seed, h_begin=N - 1000, h_end=N, acc=oacc, fingerprints=True)
+    same += int((fp[N - 1000:].cpu().numpy().view(np.uint64) == ofp).sum()); total += 1000
+    assert same / total >= 0.999, same / total
