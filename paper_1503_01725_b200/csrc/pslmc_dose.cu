@@ -228,7 +228,7 @@ struct Run {
     return a;
   }
   XsTable xs{};
-  static constexpr size_t kXsSmem = kXsBytes + sizeof(StageRing) * (kThreads / 32);   // k_photon dynamic shared memory
+  static constexpr size_t kXsSmem = kXsBytes + sizeof(StageRing) * (kThreads / 32) + kAnnihBytes;   // k_photon dynamic shared memory
   // Builds the cross-section table of this call (after k_rhomax) for photon energies up to e_max.
   void build_xs(double e_max) {
     const double x0 = std::log2(0.045), x1 = std::log2(e_max * 1.001), hh = (x1 - x0) / kXsIntervals;
@@ -285,10 +285,6 @@ struct Run {
     a.src_kind = SRC_BUFFER; a.buffer_is_debug = 1; a.first = first; a.want_type = 0;
     a.src_count = count_ptr; a.src_head = &ctl->head_pb; a.p0 = dbg_p0; a.p1 = dbg_p1;
     photon(a);
-    TransportArgs b = base_args();
-    b.src_kind = SRC_QUEUE; b.src = b.pq; b.src_count = &ctl->n_pq; b.src_head = &ctl->head_pq;
-    b.pq.cap = 0;                              // 0.511 MeV photons cannot pair-produce; a push would flag overflow
-    photon(b);
     drain_electrons();
   }
   // mc_dose: call right after k_next_batch + k_sample.  The photons of the particle buffer and the
@@ -298,9 +294,7 @@ struct Run {
     TransportArgs a = base_args();
     a.src_kind = SRC_BUFFER; a.buffer_is_debug = 0; a.first = first; a.want_type = 0;
     a.src_count = &ctl->n_pb; a.src_head = &ctl->head_pb;
-    a.src = queue(L.pq[pq_fill ^ 1], &ctl->n_pq_prev, L.pq_cap); a.src2_count = &ctl->n_pq_prev;
-    photon(a);
-    pq_pending = true;
+    photon(a);                                 // (annihilation photons are transported inside the launch, by the converting lane)
     drain_electrons();
   }
   // Annihilation photons still queued after the last photon batch (call after a k_next_batch).

@@ -20,6 +20,7 @@ enum { SRC_BUFFER = 0, SRC_QUEUE = 1 };
 constexpr int kElectronRefillMin = 8;          // k_electron refills in groups of >= 8 idle lanes (measured best of 1, 4, 8, 16)
 constexpr unsigned kElectronChunk = 32;        // largest source chunk a k_electron warp reserves at once
 constexpr int kXsIntervals = 4096;
+constexpr size_t kAnnihBytes = 2 * sizeof(float4) * kThreads;   // k_photon: one pending annihilation photon per lane
 constexpr size_t kXsBytes = sizeof(float) * (kXsHead + kXsIntervals + 4);     // head + n + 1 nodes, padded to 16 bytes
 
 struct TransportArgs {
@@ -257,7 +258,9 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
   float *s_xs = reinterpret_cast<float *>(s_raw);
   for (int i = threadIdx.x; i <= kXsHead + a.xs.n; i += kThreads) s_xs[i] = a.xs.data[i];
   __syncthreads();
-  ScoreStage<STAGE> stage; stage.init(s_raw + kXsBytes + sizeof(StageRing) * (kThreads / 32));
+  // the second annihilation photon of a pair waits here, one slot per lane: (x, y, z, track id), (u, v, w, -)
+  float4 *s_annih = reinterpret_cast<float4 *>(s_raw + kXsBytes + sizeof(StageRing) * (kThreads / 32)) + 2 * threadIdx.x;
+  ScoreStage<STAGE> stage; stage.init(s_raw + kXsBytes + sizeof(StageRing) * (kThreads / 32) + kAnnihBytes);
   const Grid &g = a.g;
   const unsigned n1 = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
   const unsigned count = n1 + ((a.src_kind == SRC_BUFFER && a.src2_count) ? min(*a.src2_count, a.src.cap) : 0u);
@@ -267,7 +270,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
   Pending<DBG> pend; pend.v = 0; pend.q = 0; pend.col = 0u;
-  int state = PH_IDLE; bool exhausted = false, collided = false;
+  int state = PH_IDLE; bool exhausted = false, collided = false, pend2 = false;
   float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, E = 0;
   int cvox = 0;                                          // voxel of the current position
   unsigned long long h = 0; uint32_t nchild = 0;
@@ -275,6 +278,15 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
   Fnv fnv; fnv.v = 0;
 
   for (;;) {
+    // ---- a lane whose photon ended and that still holds the second annihilation photon of a pair takes that one
+    if (state == PH_IDLE && pend2) {
+      const float4 A = s_annih[0], Bv = s_annih[1];
+      x = A.x; y = A.y; z = A.z; u = Bv.x; v = Bv.y; w = Bv.z; E = kEAnnih; nchild = 0; collided = false; pend2 = false;
+      rng.init(h, __float_as_uint(A.w), 0u);
+      if (DBG) fnv.init(__float_as_uint(A.w));
+      int vi, vj, vk; locate(g, x, y, z, vi, vj, vk);       // the conversion site: inside the grid
+      cvox = vox_index(g, vi, vj, vk); state = PH_FLIGHT;
+    }
     // ---- refill idle lanes
     const unsigned idx = refill_index<1, 128u>(a, state == PH_IDLE, n1, count, sc, exhausted);
     if (idx != 0xffffffffu) {
@@ -401,28 +413,24 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
     // ---- secondaries, convergent: Compton electrons through the staging ring ...
     stage_push(a.eq, a.ctl, ring, stg, push_e, make_float4(x, y, z, eT), make_float4(ex, ey, ez, 0.f),
                make_uint4((uint32_t)h, (uint32_t)(h >> 32), etrack, DBG ? pend.col : 0u));
-    // ... and, in the rare iteration with a pair production in the warp, the e-/e+ through the same ring and
-    // the two annihilation photons behind ONE warp-aggregated tail atomic (the lane's x, y, z, u, v, w, h,
-    // nchild are still those of the converting photon: it only refills at the top of the next iteration)
+    // ... and, in the rare iteration with a pair production in the warp, the e-/e+ through the same ring (the lane's
+    // x, y, z, u, v, w, h, track and nchild are still those of the converting photon)
     const unsigned mp = __ballot_sync(kFull, push_p);
     if (mp) {
 #pragma unroll
       for (int sl = 0; sl < 2; ++sl)
         stage_push(a.eq, a.ctl, ring, stg, pairT[sl] > 0.0f, make_float4(x, y, z, pairT[sl]), make_float4(u, v, w, 0.f),
                    make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, (uint32_t)sl), DBG ? pend.col : 0u));
-      const unsigned lane = threadIdx.x & 31u, leader = __ffs(mp) - 1;
-      unsigned base = 0;
-      if (lane == leader) base = atomicAdd(a.pq.count, 2u * __popc(mp));
-      base = __shfl_sync(kFull, base, leader);
+      // the two 0.511 MeV annihilation photons (tracks: slots 2, 3 of this conversion) stay in the lane: it continues
+      // as the first at once and keeps the second in its shared-memory slot until the first has ended
       if (push_p) {
-        const unsigned slot = base + 2u * __popc(mp & ((1u << lane) - 1u));
-        if (slot + 2u > a.pq.cap) a.ctl->overflow = 1u;
-        else {
-          a.pq.a[slot] = a.pq.a[slot + 1] = make_float4(x, y, z, kEAnnih);
-          a.pq.b[slot] = make_float4(ex, ey, ez, 0.f); a.pq.b[slot + 1] = make_float4(-ex, -ey, -ez, 0.f);
-          a.pq.c[slot] = make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, 2u), DBG ? pend.col : 0u);
-          a.pq.c[slot + 1] = make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, 3u), DBG ? pend.col : 0u);
-        }
+        const uint32_t t1 = child_track(rng.track, nchild, 2u), t2 = child_track(rng.track, nchild, 3u);
+        s_annih[0] = make_float4(x, y, z, __uint_as_float(t2)); s_annih[1] = make_float4(-ex, -ey, -ez, 0.f);
+        pend2 = true;
+        u = ex; v = ey; w = ez; E = kEAnnih; nchild = 0; collided = false;
+        rng.init(h, t1, 0u);
+        if (DBG) fnv.init(t1);
+        state = PH_FLIGHT;
       }
     }
   }
