@@ -126,7 +126,8 @@ typedef struct {
   uint64_t n_sec_electrons, n_sec_photons;
   uint64_t n_electron_tracks, n_electron_steps, n_electron_escape;
   uint64_t n_deposits;
-  uint64_t queue_high_water[2];    /* electron queue, photon queue (entries)                     */
+  uint64_t queue_high_water[2];    /* [0] electron queue (entries); [1] always 0 (there is no     */
+                                   /* photon queue: annihilation photons stay in their lane)       */
   uint64_t launches[5];            /* per MC_K_* class                                           */
   float    ms[5];                  /* per MC_K_* class (MC_FLAG_TIMING); with pipelines > 1 the    */
                                    /* classes overlap in time and their sum exceeds ms_total       */

@@ -44,19 +44,17 @@ static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 // Workspace layout for a batch of B primaries.  Shared by the whole call: group offsets, cross-section
 // data, packed phantom, (optionally) the int64 dose grid.  Per pipeline (kMaxPipes of them, see run_dose):
-// control block, the particle buffer (2 planes), the electron queue (capacity 4B) and the two photon
-// queues (capacity 2B each: cannot overflow), 3 planes per queue.
+// control block, the particle buffer (2 planes + the commissioning column), the electron queue (capacity 4B, 3 planes).
 constexpr int kMaxPipes = 2;
 struct Layout {
-  size_t ctl, off, xs, vox, p0, p1, p2, eq[3], pq[2][3], acc, total;
-  unsigned eq_cap, pq_cap;
+  size_t ctl, off, xs, vox, p0, p1, p2, eq[3], acc, total;
+  unsigned eq_cap;
 };
 static void make_layouts(uint64_t batch, size_t nvox, bool with_acc, Layout out[kMaxPipes]) {
   Layout L; size_t o = 0;
   auto take = [&](size_t b) { size_t at = o; o += align_up(b); return at; };
   L.eq_cap = (unsigned)std::min<uint64_t>(4 * batch, 0x7fffffffu);
   if (const char *e = getenv("PSLMC_TEST_EQ_CAP")) L.eq_cap = (unsigned)std::max(1, atoi(e));   // test hook: exercises MC_E_OVERFLOW (the planes keep their full size)
-  L.pq_cap = (unsigned)std::min<uint64_t>(2 * batch, 0x7fffffffu);   // a photon converts at most once: two annihilation photons each, never more
   L.off = take(sizeof(uint64_t) * 160); L.xs = take(kXsBytes); L.vox = take(4 * nvox);
   L.acc = take(with_acc ? 8 * nvox : 0);
   for (int p = 0; p < kMaxPipes; ++p) {
@@ -64,7 +62,6 @@ static void make_layouts(uint64_t batch, size_t nvox, bool with_acc, Layout out[
     Q.ctl = take(sizeof(Control));
     Q.p0 = take(16 * batch); Q.p1 = take(16 * batch); Q.p2 = take(4 * batch);
     for (int k = 0; k < 3; ++k) Q.eq[k] = take((size_t)16 * L.eq_cap);
-    for (int b = 0; b < 2; ++b) for (int k = 0; k < 3; ++k) Q.pq[b][k] = take((size_t)16 * L.pq_cap);
   }
   for (int p = 0; p < kMaxPipes; ++p) out[p].total = o;
 }
@@ -219,7 +216,7 @@ struct Run {
     a.g = g; a.ctl = ctl; a.seed = seed; a.n_total = n_total; a.perm_a = perm_a;
     round_keys(seed, a.ks);
     a.p0 = (const float4 *)(ws + L.p0); a.p1 = (const float4 *)(ws + L.p1); a.p2 = g.com_index ? (const uint32_t *)(ws + L.p2) : nullptr;
-    a.eq = queue(L.eq, &ctl->n_eq, L.eq_cap); a.pq = queue(L.pq[pq_fill], &ctl->n_pq, L.pq_cap);
+    a.eq = queue(L.eq, &ctl->n_eq, L.eq_cap);
     a.fp = fp; a.fp_base = fp_base;
     a.electrons_local = (flags & MC_FLAG_ELECTRONS_LOCAL) ? 1 : 0;
     a.static_lanes = (flags & MC_FLAG_STATIC_LANES) ? 1 : 0;
@@ -272,13 +269,11 @@ struct Run {
       blocks_electron[0] = persistent_blocks(k_electron<false, false>); blocks_electron[1] = persistent_blocks(k_electron<true, false>);
     }
   }
-  // Folds the finished batch's counters, resets them, and swaps the photon queues (n_pq -> n_pq_prev).
+  // Folds the finished batch's counters into the per-call totals and resets them.
   void next_batch() {
     tm.begin(MC_K_AUX); k_next_batch<<<1, 1, 0, st>>>(ctl); tm.end(MC_K_AUX); ++launches[MC_K_AUX];
-    pq_fill ^= 1;
   }
   const float4 *dbg_p0 = nullptr, *dbg_p1 = nullptr;
-  int pq_fill = 0; bool pq_pending = false;     // photon queues ping-pong: batch i fills pq[i & 1] and consumes pq[(i - 1) & 1]
   // mc_transport_debug: photons of the caller's buffer, then their annihilation photons, then every queued electron
   void transport_photon_debug(uint64_t first, const unsigned *count_ptr) {
     TransportArgs a = base_args();
@@ -296,16 +291,6 @@ struct Run {
     a.src_count = &ctl->n_pb; a.src_head = &ctl->head_pb;
     photon(a);                                 // (annihilation photons are transported inside the launch, by the converting lane)
     drain_electrons();
-  }
-  // Annihilation photons still queued after the last photon batch (call after a k_next_batch).
-  void drain_photon_queue() {
-    if (!pq_pending) return;
-    TransportArgs b = base_args();
-    b.src_kind = SRC_QUEUE; b.src = queue(L.pq[pq_fill ^ 1], &ctl->n_pq_prev, L.pq_cap); b.src_count = &ctl->n_pq_prev; b.src_head = &ctl->head_pq;
-    b.pq.cap = 0;
-    photon(b);
-    drain_electrons();
-    pq_pending = false;
   }
   void drain_electrons() {
     TransportArgs c = base_args();
@@ -329,7 +314,7 @@ static void merge_control(Control &dst, const Control &src) {
       dst.ledger[sl][k][0] = (unsigned long long)a; dst.ledger[sl][k][1] = (unsigned long long)(a >> 64);
     }
   for (int k = 0; k < ST_COUNT; ++k) dst.stat[k] += src.stat[k];
-  dst.hw_eq = std::max(dst.hw_eq, src.hw_eq); dst.hw_pq = std::max(dst.hw_pq, src.hw_pq);
+  dst.hw_eq = std::max(dst.hw_eq, src.hw_eq);
   dst.n_accepted += src.n_accepted; dst.n_missed += src.n_missed; dst.overflow |= src.overflow;
 }
 
@@ -345,7 +330,7 @@ static void fold_stats(const Control &c, const Run &r, mc_stats_t *s) {
   s->n_sec_electrons = c.stat[ST_SEC_E]; s->n_sec_photons = c.stat[ST_SEC_P];
   s->n_electron_tracks = c.stat[ST_ETRACKS]; s->n_electron_steps = c.stat[ST_ESTEPS]; s->n_electron_escape = c.stat[ST_EESC];
   s->n_deposits = c.stat[ST_DEPOSITS];
-  s->queue_high_water[0] = c.hw_eq; s->queue_high_water[1] = c.hw_pq;
+  s->queue_high_water[0] = c.hw_eq; s->queue_high_water[1] = 0;    // no photon queue: annihilation photons stay in their lane
   for (int k = 0; k < 5; ++k) s->launches[k] = r.launches[k];
 }
 
@@ -493,7 +478,6 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
       const uint64_t nb = (hi - lo + batch - 1) / batch, even = std::min(batch, (((hi - lo + nb - 1) / nb) + kThreads - 1) / kThreads * kThreads);
       for (uint64_t first = lo; first < hi; first += even, ++task) {
         const int p = (int)(task % npipe); Run &r = pipes[p];
-        if (P->psr.particle_type[s] != 0 && r.pq_pending) { r.next_batch(); r.drain_photon_queue(); }   // no photon launch ahead to carry them
         sample_batch(p, first, std::min(even, hi - first));
         if (P->psr.particle_type[s] == 0) r.transport_photon_batch(first);
         else r.transport_electron_buffer(first, false, &r.ctl->n_pb, &r.ctl->head_pb);
@@ -512,7 +496,6 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
   for (int p = 0; p < npipe; ++p) {
     Run &r = pipes[p];
     r.next_batch();
-    if (r.pq_pending) { r.drain_photon_queue(); r.next_batch(); }
     if (npipe > 1) {
       CUDA_TRY(cudaEventCreateWithFlags(&ev_join[p], cudaEventDisableTiming));
       CUDA_TRY(cudaEventRecord(ev_join[p], r.st));

@@ -19,13 +19,12 @@ struct Control {
   // per batch
   unsigned n_pb, head_pb;          // particle buffer: entries written by k_sample, consume cursor
   unsigned n_eq, head_eq;          // electron queue
-  unsigned n_pq, head_pq;          // photon queue (annihilation photons)
   unsigned pad0;                   // (mixed order: consume cursor of the electron pass over the particle buffer)
-  unsigned n_pq_prev;              // annihilation photons of the PREVIOUS batch, consumed by this batch's photon launch
+  unsigned pad1, pad2, pad3;
   // per call
   unsigned overflow;               // a queue was full: result invalid → MC_E_OVERFLOW
-  unsigned hw_eq, hw_pq;           // queue high-water marks
-  unsigned pad2;
+  unsigned hw_eq;                  // electron-queue high-water mark
+  unsigned pad4, pad5;
   unsigned long long n_accepted;   // primaries that passed the jaws and entered the phantom
   unsigned long long n_missed;     // primaries that passed the jaws but missed the phantom (k_sample, compact mode)
   unsigned long long ledger[kLedgerSlots][4][2];   // [slot][incident,deposited,escaped,jaw][lo,hi] quanta
@@ -253,9 +252,8 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
 // Folds the finished batch's counters into the per-call totals and resets them.
 __global__ void k_next_batch(Control *c) {
   c->n_accepted += c->n_pb;
-  c->hw_eq = max(c->hw_eq, c->n_eq); c->hw_pq = max(c->hw_pq, c->n_pq);
-  c->n_pq_prev = c->n_pq;           // the photon queues ping-pong: last batch's annihilation photons ride with the next photon launch
-  c->n_pb = c->head_pb = c->n_eq = c->head_eq = c->n_pq = c->head_pq = c->pad0 = 0;
+  c->hw_eq = max(c->hw_eq, c->n_eq);
+  c->n_pb = c->head_pb = c->n_eq = c->head_eq = c->pad0 = 0;
 }
 
 // Packs the caller's phantom into one 32-bit word per voxel (density rounded to nearest on a 22-bit

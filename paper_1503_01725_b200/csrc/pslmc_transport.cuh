@@ -35,11 +35,10 @@ struct TransportArgs {
   const uint32_t *p2;                 // commissioning column per buffer entry, or null
   Queue src;
   const unsigned *src_count;          // entries available (device)
-  const unsigned *src2_count;         // SRC_BUFFER only, or null: `src` holds this many extra tracks, consumed after the buffer
   unsigned *src_head;                 // consume cursor (device)
   unsigned long long first, n_total, perm_a;
   // sinks
-  Queue eq, pq;
+  Queue eq;                           // sink of the charged secondaries
   // options
   unsigned long long *fp; unsigned long long fp_base;
   int electrons_local, static_lanes, stage_scoring;
@@ -224,7 +223,7 @@ struct TrackIn { float x, y, z, u, v, w, E; unsigned long long h; uint32_t track
 
 __device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned idx, unsigned n1) {
   TrackIn t;
-  if (a.src_kind == SRC_BUFFER && idx < n1) {
+  if (a.src_kind == SRC_BUFFER) {
     const float4 A = a.p0[idx], B = a.p1[idx];
     t.x = A.x; t.y = A.y; t.z = A.z; t.E = A.w; t.u = B.x; t.v = B.y; t.w = B.z;
     unsigned long long tt;
@@ -233,7 +232,6 @@ __device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned i
     t.h = history_of(a.first + tt, a.perm_a, a.n_total);
     t.track = 0u; t.blk = 2u; t.col = a.p2 ? a.p2[idx] : 0u;      // blocks 0, 1 were the source draws
   } else {
-    if (a.src_kind == SRC_BUFFER) idx -= n1;
     const float4 A = a.src.a[idx], B = a.src.b[idx]; const uint4 C = a.src.c[idx];
     t.x = A.x; t.y = A.y; t.z = A.z; t.E = A.w; t.u = B.x; t.v = B.y; t.w = B.z;
     t.h = ((unsigned long long)C.y << 32) | C.x; t.track = C.z; t.blk = 0u; t.col = C.w; t.ok = true;
@@ -263,7 +261,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
   ScoreStage<STAGE> stage; stage.init(s_raw + kXsBytes + sizeof(StageRing) * (kThreads / 32) + kAnnihBytes);
   const Grid &g = a.g;
   const unsigned n1 = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
-  const unsigned count = n1 + ((a.src_kind == SRC_BUFFER && a.src2_count) ? min(*a.src2_count, a.src.cap) : 0u);
+  const unsigned count = n1;
   SrcCursor sc; sc.next = sc.end = 0u;
   StageRing &ring = *reinterpret_cast<StageRing *>(s_raw + kXsBytes + sizeof(StageRing) * (threadIdx.x >> 5));
   StageCursor stg; stg.head = stg.n = stg.base_raw = 0u; stg.pending = false;
@@ -452,7 +450,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
   const Grid &g = a.g;
   ScoreStage<STAGE> stage; stage.init(s_raw);
   const unsigned n1 = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
-  const unsigned count = n1 + ((a.src_kind == SRC_BUFFER && a.src2_count) ? min(*a.src2_count, a.src.cap) : 0u);
+  const unsigned count = n1;
   SrcCursor sc; sc.next = sc.end = 0u;
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
