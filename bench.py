@@ -138,7 +138,7 @@ class ClockSampler:
 # Algorithmic work per history of the bench workload, stated in DESIGN.md §Roofline and measured once
 # with ncu (profiles/): SASS thread-instructions the transport kernels retire per C1 primary history,
 # and the bytes k_sample must write per history (32 B per particle that passes the jaws).
-ALG_THREAD_INST_PER_HISTORY = {"C1": {"photon": 675.0, "electron": 856.0, "sample": 507.0},      # profiles/r1c_launches.md
+ALG_THREAD_INST_PER_HISTORY = {"C1": {"photon": 677.0, "electron": 849.0, "sample": 507.0},      # profiles/r1c_launches.md
                                "C4": {"photon": 2575.0, "electron": 2604.0, "sample": 600.0}}    # profiles/r1b_ablation_c4.md (batch 2^22, sorted)
 # DRAM bytes (read + write) per step of each kernel class, from the ncu --set full captures of profiles/r1c_top_kernels.md
 # (the two primary-batch launches; the path's working set is L2-resident, so this is far below any HBM bound)
