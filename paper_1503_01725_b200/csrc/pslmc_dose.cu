@@ -494,8 +494,7 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
     if (hb == 0 && he == N) for (int s = 0; s < 3; ++s) g_stats.n_hist[s] = off[(size_t)(s + 1) * ne] - off[(size_t)s * ne];
   }
   for (int p = 0; p < npipe; ++p) {
-    Run &r = pipes[p];
-    r.next_batch();
+    Run &r = pipes[p];                                // (the last batch's counters are folded on the host, below: no launch)
     if (npipe > 1) {
       CUDA_TRY(cudaEventCreateWithFlags(&ev_join[p], cudaEventDisableTiming));
       CUDA_TRY(cudaEventRecord(ev_join[p], r.st));
@@ -513,6 +512,9 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
   Control hc[kMaxPipes];
   for (int p = 0; p < npipe; ++p) CUDA_TRY(cudaMemcpyAsync(&hc[p], pipes[p].ctl, sizeof(Control), cudaMemcpyDeviceToHost, us));
   CUDA_TRY(cudaStreamSynchronize(us));
+  for (int p = 0; p < npipe; ++p) {                     // what k_next_batch would have folded for the last batch of each pipeline
+    hc[p].n_accepted += hc[p].n_pb; hc[p].hw_eq = std::max(hc[p].hw_eq, hc[p].n_eq);
+  }
   l2w.clear();
   CUDA_TRY(cudaEventElapsedTime(&g_stats.ms_total, ev0, ev1));
   cudaEventDestroy(ev0); cudaEventDestroy(ev1);
