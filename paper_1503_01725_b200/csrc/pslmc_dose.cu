@@ -233,6 +233,7 @@ struct Run {
     k_build_xs<<<(kXsIntervals + 256) / 256, 256, 0, st>>>(ctl, nodes, x0, hh, kXsIntervals);
     xs.data = nodes; xs.x0 = (float)x0; xs.inv_h = (float)(1.0 / hh); xs.n = kXsIntervals;
   }
+  bool started = false;                         // a batch has been launched on this pipeline
   uint64_t batch = 0;                           // upper bound of the entries a photon launch can see
   int photon_blocks(int persistent) const { return (int)std::max<uint64_t>(1, std::min<uint64_t>({(uint64_t)persistent, (batch + kThreads - 1) / kThreads, 4096 / (kThreads / 32)})); }
   void photon(const TransportArgs &a) {
@@ -460,7 +461,8 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
   memset(&g_stats, 0, sizeof g_stats);
   auto sample_batch = [&](int p, uint64_t first, uint64_t count) {
     Run &r = pipes[p];
-    r.next_batch();
+    if (r.started) r.next_batch();                      // (a pipeline's first batch finds the control block freshly zeroed)
+    r.started = true;
     sa[p].first = first; sa[p].count = (unsigned)count;
     r.tm.begin(MC_K_SAMPLE);
     k_sample<<<(unsigned)((count + kThreads - 1) / kThreads), kThreads, 0, r.st>>>(sa[p]);
