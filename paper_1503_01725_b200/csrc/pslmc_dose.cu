@@ -55,11 +55,13 @@ static void make_layouts(uint64_t batch, size_t nvox, bool with_acc, Layout out[
   auto take = [&](size_t b) { size_t at = o; o += align_up(b); return at; };
   L.eq_cap = (unsigned)std::min<uint64_t>(4 * batch, 0x7fffffffu);
   if (const char *e = getenv("PSLMC_TEST_EQ_CAP")) L.eq_cap = (unsigned)std::max(1, atoi(e));   // test hook: exercises MC_E_OVERFLOW (the planes keep their full size)
+  size_t ctl_at[kMaxPipes];
+  for (int p = 0; p < kMaxPipes; ++p) ctl_at[p] = take(sizeof(Control));     // contiguous from offset 0: zeroed by one memset
   L.off = take(sizeof(uint64_t) * 160); L.xs = take(kXsBytes); L.vox = take(4 * nvox);
   L.acc = take(with_acc ? 8 * nvox : 0);
   for (int p = 0; p < kMaxPipes; ++p) {
     Layout &Q = out[p]; Q = L;
-    Q.ctl = take(sizeof(Control));
+    Q.ctl = ctl_at[p];
     Q.p0 = take(16 * batch); Q.p1 = take(16 * batch); Q.p2 = take(4 * batch);
     for (int k = 0; k < 3; ++k) Q.eq[k] = take((size_t)16 * L.eq_cap);
   }
@@ -90,6 +92,13 @@ int upload_tables(psl *P) {
   CUDA_TRY(cudaMemcpy(P->d_table, table.data(), sizeof(AliasEntry) * table.size(), cudaMemcpyHostToDevice));
   CUDA_TRY(cudaMemcpy(P->d_let_off, let_off.data(), sizeof(uint32_t) * G, cudaMemcpyHostToDevice));
   CUDA_TRY(cudaMemcpy(P->d_n_let, n_let.data(), sizeof(uint32_t) * G, cudaMemcpyHostToDevice));
+  // sigma_KN nodes for this model's energy range (the phantom-dependent majorant head is computed per launch)
+  const double e_max = P->psr.e_min + P->psr.e_bin_width * P->n_ebin;
+  P->xs_x0 = std::log2(0.045); P->xs_h = (std::log2(std::max(e_max, 0.1) * 1.001) - P->xs_x0) / kXsIntervals;
+  CUDA_TRY(cudaMalloc(&P->d_xs, kXsBytes));
+  k_build_xs<<<(kXsIntervals + 256) / 256, 256>>>(nullptr, (float *)P->d_xs, P->xs_x0, P->xs_h, kXsIntervals);
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaDeviceSynchronize());
   return MC_OK;
 }
 
@@ -221,10 +230,11 @@ struct Run {
     a.electrons_local = (flags & MC_FLAG_ELECTRONS_LOCAL) ? 1 : 0;
     a.static_lanes = (flags & MC_FLAG_STATIC_LANES) ? 1 : 0;
     a.stage_scoring = (flags & MC_FLAG_STAGE_SCORING) ? 1 : 0;
-    a.xs = xs;
+    a.xs = xs; a.rhomax = rhomax ? rhomax : ctl->rhomax;
     return a;
   }
   XsTable xs{};
+  const float *rhomax = nullptr;                 // where k_pack_phantom left the largest densities (pipeline 0's control block)
   static constexpr size_t kXsSmem = kXsBytes + sizeof(StageRing) * (kThreads / 32) + kAnnihBytes;   // k_photon dynamic shared memory
   // Builds the cross-section table of this call (after k_rhomax) for photon energies up to e_max.
   void build_xs(double e_max) {
@@ -432,16 +442,16 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
   cudaEvent_t ev0, ev1;
   CUDA_TRY(cudaEventCreate(&ev0)); CUDA_TRY(cudaEventCreate(&ev1));
   CUDA_TRY(cudaEventRecord(ev0, us));
-  for (int p = 0; p < npipe; ++p) CUDA_TRY(cudaMemsetAsync(pipes[p].ctl, 0, sizeof(Control), us));
+  CUDA_TRY(cudaMemsetAsync(ws, 0, align_up(sizeof(Control)) * kMaxPipes, us));          // every pipeline's control block
   CUDA_TRY(cudaMemcpyAsync(d_off, off.data(), sizeof(uint64_t) * off.size(), cudaMemcpyHostToDevice, us));
   if (!opts->dose_acc) CUDA_TRY(cudaMemsetAsync(acc, 0, 8 * nvox, us));
   Timer tm_us; tm_us.on = r0.tm.on; tm_us.st = us;
   uint64_t launches_us[5] = {0, 0, 0, 0, 0};
   tm_us.begin(MC_K_AUX);
   k_pack_phantom<<<592, 256, 0, us>>>(ph->density, ph->material, nvox, (uint32_t *)((char *)ws + L.vox), r0.ctl);
-  { cudaStream_t keep = r0.st; r0.st = us; r0.build_xs(P->psr.e_min + P->psr.e_bin_width * P->n_ebin); r0.st = keep; }
-  tm_us.end(MC_K_AUX); launches_us[MC_K_AUX] += 2;
-  for (int p = 1; p < npipe; ++p) pipes[p].xs = r0.xs;
+  r0.xs.data = (const float *)P->d_xs; r0.xs.x0 = (float)P->xs_x0; r0.xs.inv_h = (float)(1.0 / P->xs_h); r0.xs.n = kXsIntervals;
+  tm_us.end(MC_K_AUX); launches_us[MC_K_AUX] += 1;
+  for (int p = 0; p < npipe; ++p) { pipes[p].xs = r0.xs; pipes[p].rhomax = r0.ctl->rhomax; }
   L2Window l2w; l2w.set(us, (char *)ws + L.vox, 4 * nvox);
   cudaEvent_t ev_fork = nullptr, ev_join[kMaxPipes] = {};
   if (npipe > 1) {
@@ -542,6 +552,7 @@ extern "C" void psl_free(psl_t *P) {
   if (P->d_let_off) cudaFree(P->d_let_off);
   if (P->d_n_let) cudaFree(P->d_n_let);
   for (int s = 0; s < 3; ++s) if (P->d_dir[s]) cudaFree(P->d_dir[s]);
+  if (P->d_xs) cudaFree(P->d_xs);
   delete P;
 }
 

@@ -36,6 +36,8 @@ struct psl {
   void *d_table = nullptr;                   // AliasEntry[total lets]
   uint32_t *d_let_off = nullptr, *d_n_let = nullptr;
   size_t total_lets = 0;
+  // sigma_KN nodes in log2 E for photon energies up to the model's top energy (built once; layout: XsTable)
+  void *d_xs = nullptr; double xs_x0 = 0, xs_h = 0;
   // Eq. 6 / Eq. 7 direction models (K = 0: focal geometry): DEVICE float4 {P_cum, mu, sigma_alpha, sigma_beta}[n_ebin][n_ring][K]
   void *d_dir[3] = {nullptr, nullptr, nullptr};
   int dir_K[3] = {0, 0, 0};

@@ -276,10 +276,11 @@ __global__ void k_pack_phantom(const float *density, const uint8_t *material, si
   }
 }
 
-// Photon cross-section data of this call (needs rhomax): layout in pslmc_device.cuh (XsTable), evaluated in double.
+// Photon cross-section data: layout in pslmc_device.cuh (XsTable), evaluated in double.  The sigma_KN nodes depend on
+// the energy range only and are built once per psl_t; the majorant head needs the phantom's rhomax (c, may be null).
 __global__ void k_build_xs(const Control *c, float *data, double x0, double h, int n) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < 3) {
+  if (c && i < 3) {                               // (k_photon recomputes this head per CTA from the call's rhomax; mc_xs_debug reads it here)
     const double rm = (double)c->rhomax[i];
     data[4 * i] = (float)(rm * (double)c_mat.ne[i]); data[4 * i + 1] = (float)(rm * (double)c_mat.cphoto[i]);
     data[4 * i + 2] = (float)(rm * (double)c_mat.ppair[i]); data[4 * i + 3] = 0.0f;

@@ -44,6 +44,7 @@ struct TransportArgs {
   int electrons_local, static_lanes, stage_scoring;
   int want_type;                      // SRC_BUFFER, compact: take only entries of this particle type (bit 31 of p1.w)
   XsTable xs;                         // k_photon: cross-section table (global; copied to shared memory per CTA)
+  const float *rhomax;                // largest density per material of this call's phantom (device; k_pack_phantom)
 };
 
 struct Tally {                         // per-thread running sums, flushed once at kernel exit
@@ -254,7 +255,12 @@ template <bool DBG, bool STAGE>
 __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ TransportArgs a) {
   extern __shared__ __align__(16) unsigned char s_raw[];           // [xs table | one StageRing per warp]
   float *s_xs = reinterpret_cast<float *>(s_raw);
-  for (int i = threadIdx.x; i <= kXsHead + a.xs.n; i += kThreads) s_xs[i] = a.xs.data[i];
+  for (int i = threadIdx.x; i <= a.xs.n; i += kThreads) s_xs[kXsHead + i] = a.xs.data[kXsHead + i];
+  if (threadIdx.x < 3) {                                 // Woodcock majorant coefficients of this phantom (k_pack_phantom's rhomax)
+    const float rm = a.rhomax[threadIdx.x];
+    s_xs[4 * threadIdx.x] = rm * c_mat.ne[threadIdx.x]; s_xs[4 * threadIdx.x + 1] = rm * c_mat.cphoto[threadIdx.x];
+    s_xs[4 * threadIdx.x + 2] = rm * c_mat.ppair[threadIdx.x]; s_xs[4 * threadIdx.x + 3] = 0.0f;
+  }
   __syncthreads();
   // the second annihilation photon of a pair waits here, one slot per lane: (x, y, z, track id), (u, v, w, -)
   float4 *s_annih = reinterpret_cast<float4 *>(s_raw + kXsBytes + sizeof(StageRing) * (kThreads / 32)) + 2 * threadIdx.x;
