@@ -285,7 +285,7 @@ struct Run {
     tm.begin(MC_K_AUX); k_next_batch<<<1, 1, 0, st>>>(ctl); tm.end(MC_K_AUX); ++launches[MC_K_AUX];
   }
   const float4 *dbg_p0 = nullptr, *dbg_p1 = nullptr;
-  // mc_transport_debug: photons of the caller's buffer, then their annihilation photons, then every queued electron
+  // mc_transport_debug: photons of the caller's buffer, then every queued electron
   void transport_photon_debug(uint64_t first, const unsigned *count_ptr) {
     TransportArgs a = base_args();
     a.src_kind = SRC_BUFFER; a.buffer_is_debug = 1; a.first = first; a.want_type = 0;
@@ -293,14 +293,13 @@ struct Run {
     photon(a);
     drain_electrons();
   }
-  // mc_dose: call right after k_next_batch + k_sample.  The photons of the particle buffer and the
-  // annihilation photons the PREVIOUS batch left in the other photon queue go through one launch
-  // (a launch over a few hundred 0.511 MeV photons alone costs the latency of its longest history).
+  // mc_dose: call right after k_sample.  The photons of the particle buffer (annihilation photons are transported
+  // inside the launch by the converting lane), then every electron they queued.
   void transport_photon_batch(uint64_t first) {
     TransportArgs a = base_args();
     a.src_kind = SRC_BUFFER; a.buffer_is_debug = 0; a.first = first; a.want_type = 0;
     a.src_count = &ctl->n_pb; a.src_head = &ctl->head_pb;
-    photon(a);                                 // (annihilation photons are transported inside the launch, by the converting lane)
+    photon(a);
     drain_electrons();
   }
   void drain_electrons() {

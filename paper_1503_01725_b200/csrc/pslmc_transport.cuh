@@ -1,6 +1,6 @@
 // pslmc_transport.cuh — k_photon and k_electron: persistent warps with lane refill, Woodcock photon
-// flights with Klein–Nishina/Kahn Compton, condensed-history electrons, warp-compacted secondary
-// queues, int64 fixed-point scoring.  PAPER.md:118-120 (iterated kernels), :161 (cut-offs);
+// flights with Klein–Nishina/Kahn Compton as a per-lane state machine, condensed-history electrons, a
+// warp-staged electron queue, int64 fixed-point scoring.  PAPER.md:118-120 (iterated kernels), :161 (cut-offs);
 // physics per DESIGN.md P1-P9.
 #pragma once
 #include "pslmc_kernels.cuh"
