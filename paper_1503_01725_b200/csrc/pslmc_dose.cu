@@ -150,13 +150,19 @@ static bool phantom_ok(const phantom_t *ph) {
 }
 
 // Persistent-grid size: every SM filled to the kernel's occupancy.
+// Fraction of the full persistent grid to launch.  When the packed phantom + int64 grid (12 B per voxel) do not fit L2,
+// the kernels are bound by random DRAM sectors and fewer resident warps thrash less: measured on C4 (201 MB) 56.8 ms per
+// 1e8 histories at 1.0, 53.1 at 0.75, 52.6 at 0.5; no effect on C1-C3 at 0.75, losses below (a single batch per pipeline
+// then leaves SMs idle).
+static double g_grid_scale = 1.0;
+
 template <typename K>
 static int persistent_blocks(K kernel, size_t smem = 0) {
   int dev = 0, sms = 0, per = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kernel, kThreads, smem);
-  return std::max(1, sms * std::max(1, per));
+  return std::max(1, (int)(sms * std::max(1, per) * g_grid_scale));
 }
 
 // L2 residency for the packed phantom (north_star (4): "read-only 3D layout that is ... L2-resident").  The random
@@ -428,7 +434,7 @@ static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam
     r.fp = (unsigned long long *)opts->fingerprints; r.fp_base = hb;
     r.dbg = (opts->flags & MC_FLAG_STATS) || opts->fingerprints || opts->com_index;   // the tally lives in the stats variants
     r.tm.on = (opts->flags & MC_FLAG_TIMING) != 0; r.tm.st = r.st;
-    if (p == 0) r.init_blocks();
+    if (p == 0) { g_grid_scale = 12.0 * (double)nvox > 110e6 ? 0.75 : 1.0; r.init_blocks(); }
     else { for (int k = 0; k < 2; ++k) { r.blocks_photon[k] = pipes[0].blocks_photon[k]; r.blocks_electron[k] = pipes[0].blocks_electron[k]; } }
   }
   Run &r0 = pipes[0];
@@ -656,7 +662,7 @@ extern "C" int mc_transport_debug(const phantom_t *ph, int32_t particle_type, co
   r.g = make_grid(*ph, (long long *)opts->dose_acc); r.g.vox = (const uint32_t *)(r.ws + L.vox);
   r.seed = seed; r.n_total = first_history + count; r.perm_a = 0; r.flags = opts->flags; r.batch = count;
   r.fp = (unsigned long long *)opts->fingerprints; r.fp_base = first_history;
-  r.dbg = true; r.tm.on = false; r.init_blocks();
+  r.dbg = true; r.tm.on = false; g_grid_scale = 1.0; r.init_blocks();
   cudaEvent_t ev0, ev1;
   CUDA_TRY(cudaEventCreate(&ev0)); CUDA_TRY(cudaEventCreate(&ev1));
   CUDA_TRY(cudaEventRecord(ev0, r.st));
