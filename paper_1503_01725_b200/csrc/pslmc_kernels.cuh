@@ -225,7 +225,7 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
     if (live && pass) {
       const unsigned dst = base + __popc(keep & ((1u << lane) - 1u));
       o1.w = __uint_as_float(t | ((unsigned)ptype << 31));
-      a.p0[dst] = o0; a.p1[dst] = o1;
+      __stcs(a.p0 + dst, o0); __stcs(a.p1 + dst, o1);         // write-once / read-once: streaming, keeps L2 for the phantom and the grid
       if (a.p2) a.p2[dst] = com_col;
     }
   } else if (live) {

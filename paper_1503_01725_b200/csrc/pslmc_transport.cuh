@@ -149,7 +149,7 @@ __device__ __forceinline__ void stage_complete(const Queue &q, Control *ctl, Sta
   if (base + n_out > q.cap) ctl->overflow = 1u;
   else if (lane < n_out) {
     const unsigned p = (sc.head + lane) & 63u;
-    q.a[base + lane] = r.a[p]; q.b[base + lane] = r.b[p]; q.c[base + lane] = r.c[p];
+    __stcs(q.a + base + lane, r.a[p]); __stcs(q.b + base + lane, r.b[p]); __stcs(q.c + base + lane, r.c[p]);   // write-once / read-once: streaming
   }
   sc.head = (sc.head + n_out) & 63u; sc.n -= n_out; sc.pending = false;
   __syncwarp();
@@ -225,7 +225,7 @@ struct TrackIn { float x, y, z, u, v, w, E; unsigned long long h; uint32_t track
 __device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned idx, unsigned n1) {
   TrackIn t;
   if (a.src_kind == SRC_BUFFER) {
-    const float4 A = a.p0[idx], B = a.p1[idx];
+    const float4 A = __ldcs(a.p0 + idx), B = __ldcs(a.p1 + idx);
     t.x = A.x; t.y = A.y; t.z = A.z; t.E = A.w; t.u = B.x; t.v = B.y; t.w = B.z;
     unsigned long long tt;
     if (a.buffer_is_debug) { tt = idx; t.ok = B.w >= 0.0f; }
@@ -233,7 +233,7 @@ __device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned i
     t.h = history_of(a.first + tt, a.perm_a, a.n_total);
     t.track = 0u; t.blk = 2u; t.col = a.p2 ? a.p2[idx] : 0u;      // blocks 0, 1 were the source draws
   } else {
-    const float4 A = a.src.a[idx], B = a.src.b[idx]; const uint4 C = a.src.c[idx];
+    const float4 A = __ldcs(a.src.a + idx), B = __ldcs(a.src.b + idx); const uint4 C = __ldcs(a.src.c + idx);
     t.x = A.x; t.y = A.y; t.z = A.z; t.E = A.w; t.u = B.x; t.v = B.y; t.w = B.z;
     t.h = ((unsigned long long)C.y << 32) | C.x; t.track = C.z; t.blk = 0u; t.col = C.w; t.ok = true;
   }
