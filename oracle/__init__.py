@@ -53,7 +53,7 @@ class _Result(C.Structure):
                [(k, C.c_uint64) for k in (
                    "n_jaw_rejected", "n_missed", "n_flights", "n_virtual", "n_compton", "n_photo", "n_pair",
                    "n_photon_cutoff", "n_photon_escape", "n_uncollided_escape", "n_sec_electrons", "n_sec_photons",
-                   "n_electron_tracks", "n_electron_steps", "n_electron_escape", "n_deposits")]
+                   "n_electron_tracks", "n_electron_steps", "n_electron_escape", "n_deposits", "n_kahn_trials", "n_deflections")]
 
 
 LEDGERS = ("incident", "deposited", "escaped", "jaw")

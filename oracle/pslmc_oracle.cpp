@@ -22,8 +22,10 @@
 // analytic PSR densities; source back-projection Gaussian; Klein–Nishina angular chi-square and
 // total cross-section vs quadrature of the differential; interaction fractions; exp(-mu x)
 // transmission (homogeneous and layered); CSDA path length vs the closed-form integral; Highland
-// angle moments; energy conservation; permutation invariance; single-history hand trace.
-// No function here is "parity unpinned".
+// angle moments; energy conservation; permutation invariance; single-history hand trace; Compton recoil electron by
+// momentum conservation, pair energy split and annihilation-photon geometry (tests/test_oracle_secondaries.py).
+// No function here is "parity unpinned" (child_track and orc_com_column are [proposed] numberings with nothing
+// external to check against: they are pinned for determinism and by-hand values only).
 //
 // Build: g++ -O2 -std=c++17 -shared -fPIC (no -ffast-math, no -march) — see oracle/__init__.py.
 
@@ -58,6 +60,7 @@ const double FE_DEFAULT = 0.12;                           // energy-loss fractio
 const double FIX = 4294967296.0;                          // 2^32 quanta per MeV
 
 const int FLAG_ELECTRONS_LOCAL = 1;
+const int FLAG_TRACE_BIRTH = 2;       // orc_trace only: log a 'B' event (position, direction, energy) when a track starts
 
 // ---------------------------------------------------------------- R1: Philox4x32-10
 void philox_block(uint64_t seed, uint64_t h, uint32_t track, uint32_t block, uint32_t out[4]) {
@@ -113,6 +116,7 @@ struct Result {
   uint64_t n_sec_electrons, n_sec_photons;
   uint64_t n_electron_tracks, n_electron_steps, n_electron_escape;
   uint64_t n_deposits;
+  uint64_t n_kahn_trials, n_deflections;   // work counters (bench.py's algorithmic-work numerator): Kahn trials, condensed-step deflections
 };
 
 struct Group { int stype, ebin; std::vector<uint16_t> ring, sector; std::vector<uint32_t> thresh, alias; double W = 0; };
@@ -426,9 +430,10 @@ void rotate(double d[3], double ct, double st, double phi) {
 
 // Kahn's rejection for Klein–Nishina; returns eta = E/E'.  One block per trial: words 0, 1, 2 = r1, r2, r3; word 3
 // of the ACCEPTED trial is returned in `w_phi` (the caller's azimuth draw).
-double kahn(double alpha, Stream &st, uint32_t &w_phi) {
+double kahn(double alpha, Stream &st, uint32_t &w_phi, uint64_t *n_trials = nullptr) {
   for (;;) {
     uint32_t w[4]; st.next_block(w);
+    if (n_trials) ++*n_trials;
     double r1 = U_co(w[0]), r2 = U_co(w[1]), r3 = U_co(w[2]);
     w_phi = w[3];
     if (r1 <= (2.0 * alpha + 1.0) / (2.0 * alpha + 9.0)) {
@@ -507,6 +512,7 @@ struct Ctx {
     Fnv f; f.u32(t.track);
     Stream st{seed, t.h, t.track, t.nblk};
     int ijk[3]; bool collided = false;
+    if (flags & FLAG_TRACE_BIRTH) ev(t, 'B');
     if (!locate(t.pos, ijk) && !enter(t, ijk)) { escape(t.E); f.byte('M'); ev(t, 'M'); ++res->n_missed; fp += f.v; return; }
     for (;;) {
       if (t.E < PCUT) { deposit(vox(ijk), t.E); f.byte('A'); ev(t, 'A'); ++res->n_photon_cutoff; break; }
@@ -523,7 +529,7 @@ struct Ctx {
       double tt = U_co(wf[1]) * mmax;
       if (tt < muC) {                                  // Compton, Klein–Nishina by Kahn
         collided = true; ++res->n_compton; f.byte('C');
-        uint32_t w_phi; double alpha = t.E / ME, eta = kahn(alpha, st, w_phi);
+        uint32_t w_phi; double alpha = t.E / ME, eta = kahn(alpha, st, w_phi, &res->n_kahn_trials);
         double k = (eta - 1.0) / alpha, ct = 1.0 - k, sn = std::sqrt(std::fmax(0.0, k * (2.0 - k)));
         double phi = 2.0 * PI * U_co(w_phi);
         double Ep = t.E / eta, T = t.E - Ep, d0[3] = {t.dir[0], t.dir[1], t.dir[2]};
@@ -561,6 +567,7 @@ struct Ctx {
     Stream st{seed, t.h, t.track, t.nblk};
     ++res->n_electron_tracks;
     int ijk[3]; uint32_t steps = 0;
+    if (flags & FLAG_TRACE_BIRTH) ev(t, 'B');
     if (!locate(t.pos, ijk) && !enter(t, ijk)) { escape(t.E); f.u32(0); f.byte('M'); ev(t, 'M'); ++res->n_missed; fp += f.v; return; }
     const double lo[3] = {ph.ox, ph.oy, ph.oz}, dd[3] = {ph.dx, ph.dy, ph.dz};
     // One condensed-history step loses the fraction fE of the energy it starts with (budget); it is cut
@@ -593,7 +600,7 @@ struct Ctx {
         double a1 = U_oc(wd[0]), b1 = U_co(wd[1]);
         double th = std::fmin(PI, th0 * std::sqrt(-2.0 * std::log(a1)));
         rotate(t.dir, std::cos(th), std::sin(th), 2.0 * PI * b1);
-        fresh = true;
+        fresh = true; ++res->n_deflections;
         ev(t, 'T', s);
       } else ev(t, 'S', s);
     }
