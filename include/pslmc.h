@@ -7,7 +7,8 @@
  *                      PAPER.md:61-69  §2.1.2 (sampling areas), :75-80 S1-S2 (Eq. 3)
  *   psl_build_grid     PAPER.md:39-55  the paper's own Cartesian (Xbin, Ybin) lets, steps 1-4
  *   psl_set_direction_model  PAPER.md:94-116 S4-S5, Eq. 6-7 (Gaussian mixtures in (alpha, beta))
- *   mc_plan_allocate   PAPER.md:76-80  Eq. 3 across the beams of a plan
+ *   mc_plan_allocate,
+ *   mc_plan_dose       PAPER.md:76-80  Eq. 3 across the beams of a plan; :73-75 one dose grid for the whole plan
  *   mc_sample_debug    PAPER.md:82-92  S3 (Eq. 4-5), :94-116 S4-S5, jaw rejection :65/:92, set-up :173
  *   mc_dose            PAPER.md:118-120 §2.1.3 (iterated source kernel / transport kernel, M per
  *                      launch, type-major / energy-ascending order), :161 (cut-offs 50 keV / 200 keV)
@@ -22,8 +23,14 @@
  *     (0,0,sad).  Phantom frame: pos_ph = iso + R * (pos_beam - (0,0,sad)), dir_ph = R * dir_beam.
  *   - All entry points return 0 on success or a negative MC_E_* code; mc_last_error() returns a
  *     thread-local message.  Outputs are unspecified after an error.
- *   - Calls on one psl_t are not re-entrant.  mc_dose is synchronous with respect to the given
- *     stream when it returns.
+ *   - The library keeps NO process-global device state: every byte of device scratch is the caller's
+ *     `workspace` (mc_workspace_bytes / mc_host_workspace_bytes; NULL or too small -> MC_E_WORKSPACE, nothing
+ *     is allocated inside mc_dose), every stream is the caller's (`cuda_stream`, `aux_streams`), the only
+ *     device memory the library owns are the read-only tables of a psl_t (allocated by psl_build on the
+ *     device current at that time, freed by psl_free).  Two host threads may therefore run mc_dose at the
+ *     same time on different workspaces and streams (same or different psl_t: a psl_t is read-only after
+ *     psl_build / psl_set_direction_model); a psl_t must be used on the device it was built on.
+ *     mc_dose is synchronous with respect to the given stream when it returns.
  *   - Determinism: for fixed inputs and seed, dose, ledgers and counters are bitwise identical for
  *     every `batch`, every `order`, every `pipelines` and every partition [history_begin,history_end) summed.
  *   - There is no CPU fallback: every entry point that computes needs a CUDA device (sm_100a).
@@ -43,7 +50,7 @@ extern "C" {
 #define MC_E_EMPTY_FIELD -2  /* no let survives the jaw selection                              */
 #define MC_E_WORKSPACE   -3  /* caller-supplied workspace too small                            */
 #define MC_E_CUDA        -4  /* a CUDA runtime call or kernel failed                           */
-#define MC_E_OVERFLOW    -5  /* a secondary queue could not be drained / ledger overflow       */
+#define MC_E_OVERFLOW    -5  /* the electron queue was full, or a voxel's int64 accumulator wrapped */
 
 /* PSR analytic source model (paper layer L0).                           */
 typedef struct {
@@ -82,10 +89,15 @@ typedef struct psl psl_t;          /* opaque: active lets, alias tables, group w
 #define MC_FLAG_STATIC_LANES    8  /* ablation: one particle per thread, no lane refill          */
 #define MC_FLAG_STAGE_SCORING  16  /* stage the scoring atomics of hot voxels in shared memory    */
                                    /* (per-CTA table, added to the grid at kernel exit; same bits)  */
+#define MC_FLAG_RANGE          32  /* take [history_begin, history_end) literally: [0, 0) is then   */
+                                   /* the EMPTY range (a shard without work) instead of "everything" */
+#define MC_FLAG_NO_TILE_SORT   64  /* ablation: do not order a batch's particles by entry tile      */
+#define MC_FLAG_TILE_SORT     128  /* order every batch by entry tile (default: only when phantom + */
+                                   /* dose grid exceed the L2 budget; PAPER.md:118-120 spatial loop)  */
 
 typedef struct {
-  void     *workspace;             /* DEVICE scratch or NULL (library-managed, cached in psl_t)  */
-  size_t    workspace_bytes;
+  void     *workspace;             /* DEVICE scratch, REQUIRED: >= mc_workspace_bytes(psl, ph, batch)  */
+  size_t    workspace_bytes;       /* (mc_dose_host: >= mc_host_workspace_bytes).  Contents are scratch. */
   void     *cuda_stream;           /* cudaStream_t or NULL (legacy default stream)               */
   int64_t  *dose_acc;              /* DEVICE int64[nx*ny*nz] or NULL.  When given, deposits are  */
                                    /* ADDED to it (multi-beam plans) and dose_out may be NULL    */
@@ -93,12 +105,12 @@ typedef struct {
   int32_t   flags;                 /* MC_FLAG_* bits                                             */
   uint64_t *fingerprints;          /* DEVICE u64[history_end-history_begin] or NULL; ADDED to    */
   uint64_t  history_begin;         /* sub-range of history ids to run (sharding) ...             */
-  uint64_t  history_end;           /* ... 0 means n_histories                                    */
-  int32_t   pipelines;             /* 0 = default (2): batches are dealt to this many independent  */
-                                   /* launch sequences on internal streams so that one kernel's    */
-                                   /* tail overlaps the next kernel; 1 = strictly serial launches  */
-                                   /* on cuda_stream (per-kernel times in mc_stats are then        */
-                                   /* disjoint).  Same bits either way.                            */
+  uint64_t  history_end;           /* ... 0 means n_histories (unless MC_FLAG_RANGE)             */
+  int32_t   pipelines;             /* 0 = as many as aux_streams are given (at most 2), 1 = strictly */
+                                   /* serial launches on cuda_stream (per-kernel times in mc_stats    */
+                                   /* are then disjoint).  With 2, batches are dealt alternately to   */
+                                   /* two launch sequences so that one kernel's tail overlaps the     */
+                                   /* other sequence's next kernel.  Same bits either way.            */
   int32_t   reserved;              /* must be 0                                                    */
   /* commissioning tally, off when com_index is NULL: every history carries the */
   /* column of the PSR it was sampled from (its descendants inherit it): (stype*n_ebin+ebin)*n_ring */
@@ -106,7 +118,16 @@ typedef struct {
   /* with com_index[v] = 1 + row > 0 is also ADDED to com_dose[col * com_rows + row].              */
   const int32_t *com_index;        /* DEVICE int32[nx*ny*nz]                                       */
   int64_t  *com_dose;              /* DEVICE int64[com_cols * com_rows], quanta of 2^-32 MeV       */
-  int32_t   com_rows, com_cols;    /* com_cols must be 2*n_ebin*n_ring + n_ebin                    */
+  int32_t   com_rows, com_cols;    /* com_cols must be 2*n_ebin*n_ring + n_ebin; needs particle_type = {0,0,1} */
+  /* streams of the pipelines (caller-owned cudaStream_t, e.g. torch streams; distinct from each other and from */
+  /* cuda_stream).  The library forks them from cuda_stream and joins them back with events; NULL = serial.       */
+  void     *aux_streams[2];
+  /* mc_plan_dose only: this call runs shard `shard_index` of `shard_count` equal contiguous parts of EVERY beam's */
+  /* history range (multi-GPU: one shard per rank, then one int64 all-reduce of dose_acc).  0, 0 = everything.      */
+  int32_t   shard_index, shard_count;
+  uint32_t  debug_eq_cap;          /* test hook: electron-queue capacity in entries (0 = the default 4*batch);   */
+                                   /* the workspace layout keeps its full size.  Exercises MC_E_OVERFLOW.        */
+  uint32_t  reserved2;             /* must be 0                                                    */
 } mc_opts_t;
 
 /* Ledger / kernel-class indices of mc_stats_t.                                                  */
@@ -126,8 +147,10 @@ typedef struct {
   uint64_t n_sec_electrons, n_sec_photons;
   uint64_t n_electron_tracks, n_electron_steps, n_electron_escape;
   uint64_t n_deposits;
-  uint64_t queue_high_water[2];    /* [0] electron queue (entries); [1] always 0 (there is no     */
-                                   /* photon queue: annihilation photons stay in their lane)       */
+  uint64_t n_kahn_trials;          /* Kahn rejection trials (accepted + rejected)                */
+  uint64_t n_deflections;          /* multiple-scattering deflections = completed condensed steps */
+  uint64_t queue_high_water;       /* electron queue, entries (the only queue: annihilation       */
+                                   /* photons stay in the lane that converted)                     */
   uint64_t launches[5];            /* per MC_K_* class                                           */
   float    ms[5];                  /* per MC_K_* class (MC_FLAG_TIMING); with pipelines > 1 the    */
                                    /* classes overlap in time and their sum exceeds ms_total       */
@@ -176,8 +199,11 @@ int  psl_allocate(const psl_t *psl, uint64_t n_histories, uint64_t *off_out);
  * Run mc_dose once per beam with n_out[i] histories into one opts->dose_acc, then scale by the plan total.      */
 int  mc_plan_allocate(const psl_t *const *psls, int32_t n_beams, uint64_t n_histories, uint64_t *n_out);
 
-/* Workspace bytes mc_dose needs for this batch size (0 on invalid arguments).                   */
+/* Workspace bytes mc_dose / mc_plan_dose / mc_transport_debug need for this batch size (0 on invalid arguments;
+ * psl may be NULL: the layout depends on the phantom's voxel count and the batch only).                        */
 size_t mc_workspace_bytes(const psl_t *psl, const phantom_t *ph, uint64_t batch);
+/* The same plus the device staging of mc_dose_host (phantom arrays in, dose out: 13 bytes per voxel).          */
+size_t mc_host_workspace_bytes(const psl_t *psl, const phantom_t *ph, uint64_t batch);
 
 /* mc_dose — the hot path.  Runs histories [history_begin,history_end) of an n_histories-history
  * allocation in batches of `batch` through k_sample → k_photon / k_electron (+ secondary queues)
@@ -189,12 +215,26 @@ int  mc_dose(const psl_t *psl, const phantom_t *ph, const beam_geom_t *beam,
              double *dose_out, const mc_opts_t *opts);
 
 /* mc_dose_host — same, end to end from HOST buffers: ph->density / ph->material and dose_out are
- * HOST pointers; the call uploads the phantom, runs mc_dose, and downloads the dose.            */
+ * HOST pointers (pinned memory makes the copies asynchronous); the call uploads the phantom into the
+ * workspace, runs mc_dose, and downloads the dose.  opts->workspace >= mc_host_workspace_bytes.  */
 int  mc_dose_host(const psl_t *psl, const phantom_t *ph_host, const beam_geom_t *beam,
                   uint64_t n_histories, uint64_t seed, uint64_t batch,
                   double *dose_out_host, const mc_opts_t *opts);
 
-/* Counters, ledgers and timings of the last mc_dose / mc_transport_debug on this thread.        */
+/* mc_plan_dose — a treatment plan of n_beams beams on one phantom (PAPER.md:73-80 S1-S2): Eq. 3 over the sampling
+ * areas of ALL beams gives beam i its n_i of the plan's n_histories (mc_plan_allocate); beam i then runs exactly
+ * like mc_dose(psls[i], ph, &beams[i], n_i, seed + i, batch) and every beam scores into ONE int64 grid
+ * (opts->dose_acc when given - deposits are ADDED - else a grid inside the workspace, zeroed first).
+ *   dose_out[v] = acc[v] * 2^-32 / (rho_v * V_voxel * n_histories)     (DEVICE double[nvox] or NULL)
+ * opts->shard_index / shard_count select one of shard_count equal contiguous parts of every beam's history range;
+ * the shards' int64 grids add up bit for bit to the unsharded plan.  history_begin/end, fingerprints, order and
+ * the commissioning tally are not available at plan level (MC_E_INVALID_ARG).  n_beam_out: HOST u64[n_beams] or NULL.
+ * mc_stats afterwards holds the sums over the beams (ledgers, counters, launches, milliseconds).                  */
+int  mc_plan_dose(const psl_t *const *psls, const beam_geom_t *beams, int32_t n_beams, const phantom_t *ph,
+                  uint64_t n_histories, uint64_t seed, uint64_t batch, double *dose_out, const mc_opts_t *opts,
+                  uint64_t *n_beam_out);
+
+/* Counters, ledgers and timings of the last mc_dose / mc_plan_dose / mc_transport_debug on this thread. */
 int  mc_stats(mc_stats_t *out);
 const char *mc_last_error(void);
 
@@ -221,11 +261,6 @@ int  mc_transport_debug(const phantom_t *ph, int32_t particle_type, const float 
  * E_host: HOST float[n] (0.05 <= E <= e_max); out_host: HOST float[3n] = (sigma_KN cm^2 per electron,
  * ln^2(E/1.022) or 0 below threshold, mu_max cm^-1) per energy.                                  */
 int  mc_xs_debug(const float rhomax[3], double e_max, const float *E_host, uint64_t n, float *out_host);
-
-/* Measurement probe: the rate of nothing but int64 scoring atomics (RED.64) on pseudo-random voxels of a grid of
- * nvox voxels — the ceiling the scoring of the transport kernels is compared with.  acc: DEVICE int64[nvox] (its
- * contents are destroyed).  ms_out: HOST float[2] = (milliseconds by CUDA events, atomics actually issued).     */
-int  mc_atomic_peak_debug(int64_t *acc, uint64_t nvox, uint64_t n_ops, uint64_t seed, float *ms_out);
 
 /* One Philox4x32-10 block computed ON THE DEVICE: key = seed, counter = (block, track, h_lo, h_hi).
  * out: HOST u32[4].                                                                             */

@@ -16,10 +16,12 @@ LIB_PATH = os.path.join(_HERE, "libpslmc.so")
 
 MC_ORDER_SORTED, MC_ORDER_MIXED = 0, 1
 MC_FLAG_ELECTRONS_LOCAL, MC_FLAG_STATS, MC_FLAG_TIMING, MC_FLAG_STATIC_LANES, MC_FLAG_STAGE_SCORING = 1, 2, 4, 8, 16
+MC_FLAG_RANGE, MC_FLAG_NO_TILE_SORT, MC_FLAG_TILE_SORT = 32, 64, 128
 LEDGERS = ("incident", "deposited", "escaped", "jaw")
 KERNEL_CLASSES = ("sample", "photon", "electron", "finalise", "aux")
-EXPORTS = ("psl_build", "psl_build_grid", "psl_set_direction_model", "mc_plan_allocate", "psl_free", "psl_export", "psl_allocate", "mc_workspace_bytes", "mc_dose", "mc_dose_host",
-           "mc_stats", "mc_last_error", "mc_sample_debug", "mc_transport_debug", "mc_philox_debug", "mc_xs_debug", "mc_atomic_peak_debug")
+EXPORTS = ("psl_build", "psl_build_grid", "psl_set_direction_model", "mc_plan_allocate", "mc_plan_dose", "psl_free", "psl_export", "psl_allocate",
+           "mc_workspace_bytes", "mc_host_workspace_bytes", "mc_dose", "mc_dose_host",
+           "mc_stats", "mc_last_error", "mc_sample_debug", "mc_transport_debug", "mc_philox_debug", "mc_xs_debug")
 
 
 class PslmcError(RuntimeError):
@@ -52,7 +54,9 @@ class mc_opts_t(C.Structure):
     _fields_ = [("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("cuda_stream", C.c_void_p),
                 ("dose_acc", C.c_void_p), ("order", C.c_int32), ("flags", C.c_int32), ("fingerprints", C.c_void_p),
                 ("history_begin", C.c_uint64), ("history_end", C.c_uint64), ("pipelines", C.c_int32), ("reserved", C.c_int32),
-                ("com_index", C.c_void_p), ("com_dose", C.c_void_p), ("com_rows", C.c_int32), ("com_cols", C.c_int32)]
+                ("com_index", C.c_void_p), ("com_dose", C.c_void_p), ("com_rows", C.c_int32), ("com_cols", C.c_int32),
+                ("aux_streams", C.c_void_p * 2), ("shard_index", C.c_int32), ("shard_count", C.c_int32),
+                ("debug_eq_cap", C.c_uint32), ("reserved2", C.c_uint32)]
 
 
 class mc_stats_t(C.Structure):
@@ -60,8 +64,9 @@ class mc_stats_t(C.Structure):
                [(k, C.c_uint64) for k in (
                    "n_jaw_rejected", "n_missed", "n_flights", "n_virtual", "n_compton", "n_photo", "n_pair",
                    "n_photon_cutoff", "n_photon_escape", "n_uncollided_escape", "n_sec_electrons", "n_sec_photons",
-                   "n_electron_tracks", "n_electron_steps", "n_electron_escape", "n_deposits")] + \
-               [("queue_high_water", C.c_uint64 * 2), ("launches", C.c_uint64 * 5), ("ms", C.c_float * 5),
+                   "n_electron_tracks", "n_electron_steps", "n_electron_escape", "n_deposits", "n_kahn_trials",
+                   "n_deflections", "queue_high_water")] + \
+               [("launches", C.c_uint64 * 5), ("ms", C.c_float * 5),
                 ("ms_total", C.c_float)]
 
 
@@ -84,8 +89,11 @@ def lib():
         L.psl_free.restype = None
         L.psl_export.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
         L.psl_allocate.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p]
-        L.mc_workspace_bytes.restype = C.c_size_t
-        L.mc_workspace_bytes.argtypes = [C.c_void_p, C.POINTER(phantom_t), C.c_uint64]
+        for f in (L.mc_workspace_bytes, L.mc_host_workspace_bytes):
+            f.restype = C.c_size_t
+            f.argtypes = [C.c_void_p, C.POINTER(phantom_t), C.c_uint64]
+        L.mc_plan_dose.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(phantom_t), C.c_uint64, C.c_uint64, C.c_uint64,
+                                   C.c_void_p, C.POINTER(mc_opts_t), C.c_void_p]
         dose_args = [C.c_void_p, C.POINTER(phantom_t), C.POINTER(beam_geom_t), C.c_uint64, C.c_uint64, C.c_uint64,
                      C.c_void_p, C.POINTER(mc_opts_t)]
         L.mc_dose.argtypes = dose_args
@@ -97,7 +105,6 @@ def lib():
         L.mc_transport_debug.argtypes = [C.POINTER(phantom_t), C.c_int32, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64,
                                          C.POINTER(mc_opts_t)]
         L.mc_philox_debug.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
-        L.mc_atomic_peak_debug.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64, C.c_void_p]
         L.mc_xs_debug.argtypes = [C.c_void_p, C.c_double, C.c_void_p, C.c_uint64, C.c_void_p]
         _lib = L
     return _lib
@@ -144,15 +151,37 @@ def stats() -> dict:
     out = {k: int(getattr(s, k)) for k, t in mc_stats_t._fields_ if t is C.c_uint64}
     out["n_hist"] = [int(x) for x in s.n_hist]
     out["ledger"] = {n: (int(s.ledger_hi[i]) << 64) + int(s.ledger_lo[i]) for i, n in enumerate(LEDGERS)}
-    out["queue_high_water"] = [int(x) for x in s.queue_high_water]
     out["launches"] = {n: int(s.launches[i]) for i, n in enumerate(KERNEL_CLASSES)}
     out["ms"] = {n: float(s.ms[i]) for i, n in enumerate(KERNEL_CLASSES)}
     out["ms_total"] = float(s.ms_total)
     return out
 
 
-def _opts(stream=None, workspace=None, dose_acc=None, order=0, flags=0, fingerprints=None, history_begin=0,
-          history_end=0, pipelines=0, com_index=None, com_dose=None) -> mc_opts_t:
+_aux = {}                                                # device index -> two torch streams for the pipelines (torch owns them)
+_ws = {}                                                 # device index -> cached torch workspace (torch owns the memory)
+
+
+def aux_streams(device=None):
+    import torch
+    d = torch.cuda.current_device() if device is None else torch.device(device).index
+    if d not in _aux:
+        _aux[d] = (torch.cuda.Stream(device=d), torch.cuda.Stream(device=d))
+    return _aux[d]
+
+
+def workspace(nbytes: int, device=None):
+    """A torch uint8 tensor of at least nbytes on the device, cached and grown on demand (the library never allocates)."""
+    import torch
+    d = torch.cuda.current_device() if device is None else torch.device(device).index
+    t = _ws.get(d)
+    if t is None or t.numel() < nbytes:
+        _ws[d] = None
+        t = _ws[d] = torch.empty(nbytes, dtype=torch.uint8, device="cuda:%d" % d)
+    return t
+
+
+def _opts(stream=None, workspace=None, dose_acc=None, order=0, flags=0, fingerprints=None, history_begin=None,
+          history_end=None, pipelines=0, com_index=None, com_dose=None, shard=None, debug_eq_cap=0, aux=None) -> mc_opts_t:
     o = mc_opts_t()
     if workspace is not None:
         o.workspace, o.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
@@ -160,11 +189,20 @@ def _opts(stream=None, workspace=None, dose_acc=None, order=0, flags=0, fingerpr
     o.dose_acc = dose_acc.data_ptr() if dose_acc is not None else None
     o.order, o.flags = order, flags
     o.fingerprints = fingerprints.data_ptr() if fingerprints is not None else None
-    o.history_begin, o.history_end = history_begin, history_end
+    if history_begin is not None or history_end is not None:       # an explicit range is taken literally ([0, 0) is empty)
+        o.history_begin, o.history_end = history_begin or 0, history_end or 0
+        if history_end is not None:
+            o.flags |= MC_FLAG_RANGE
     o.pipelines = pipelines
+    if pipelines != 1:
+        a = aux if aux is not None else aux_streams()
+        o.aux_streams[0], o.aux_streams[1] = int(a[0].cuda_stream), int(a[1].cuda_stream)
     if com_index is not None:                            # commissioning tally: int32[nvox] index, int64[cols, rows] matrix (torch, device)
         o.com_index, o.com_dose = com_index.data_ptr(), com_dose.data_ptr()
         o.com_cols, o.com_rows = com_dose.shape[0], com_dose.shape[1]
+    if shard is not None:
+        o.shard_index, o.shard_count = shard
+    o.debug_eq_cap = debug_eq_cap
     return o
 
 
@@ -225,8 +263,9 @@ class Psl:
         _check(lib().psl_allocate(self.h, n_histories, off.ctypes.data_as(C.c_void_p)))
         return off
 
-    def workspace_bytes(self, phantom: DevicePhantom, batch: int) -> int:
-        return int(lib().mc_workspace_bytes(self.h, C.byref(phantom.c), batch))
+    def workspace_bytes(self, phantom: DevicePhantom, batch: int, host: bool = False) -> int:
+        f = lib().mc_host_workspace_bytes if host else lib().mc_workspace_bytes
+        return int(f(self.h, C.byref(phantom.c), batch))
 
     def sample_debug(self, beam: dict, n_histories: int, seed: int, first: int, count: int, stream=None):
         """Returns a torch float32 tensor (2, count, 4): plane 0 = (x,y,z,E), plane 1 = (u,v,w,status)."""
@@ -242,6 +281,8 @@ class Psl:
         import torch
         if dose_out is None and opt.get("dose_acc") is None:
             dose_out = torch.empty(phantom.nvox, dtype=torch.float64, device=phantom.device)
+        if opt.get("workspace") is None:
+            opt["workspace"] = workspace(self.workspace_bytes(phantom, batch), phantom.device)
         o = _opts(**opt)
         _check(lib().mc_dose(self.h, C.byref(phantom.c), C.byref(_beam(beam)), n_histories, seed, batch,
                              dose_out.data_ptr() if dose_out is not None else None, C.byref(o)))
@@ -255,6 +296,8 @@ class Psl:
         if dose_out is None:
             dose_out = np.empty(density.size, np.float64)
         c = _phantom_struct(ph, density.ctypes.data, material.ctypes.data)
+        if opt.get("workspace") is None:
+            opt["workspace"] = workspace(int(lib().mc_host_workspace_bytes(self.h, C.byref(c), batch)))
         o = _opts(**opt)
         _check(lib().mc_dose_host(self.h, C.byref(c), C.byref(_beam(beam)), n_histories, seed, batch,
                                   dose_out.ctypes.data_as(C.c_void_p), C.byref(o)))
@@ -264,7 +307,9 @@ class Psl:
 def transport_debug(phantom: DevicePhantom, ptype: int, soa, first: int, seed: int, dose_acc, **opt):
     """mc_transport_debug on a (2, count, 4) float32 device tensor in mc_sample_debug's layout."""
     count = soa.shape[1]
-    o = _opts(dose_acc=dose_acc, **opt)
+    if opt.get("workspace") is None:
+        opt["workspace"] = workspace(int(lib().mc_workspace_bytes(None, C.byref(phantom.c), max(count, 1))), phantom.device)
+    o = _opts(dose_acc=dose_acc, pipelines=1, **opt)
     _check(lib().mc_transport_debug(C.byref(phantom.c), ptype, soa.data_ptr(), first, count, seed, C.byref(o)))
 
 
@@ -291,31 +336,23 @@ def plan_allocate(psls, n_histories: int) -> np.ndarray:
     return out
 
 
-def plan_dose(psls, phantom, beams, n_histories: int, seed: int, batch: int = 1 << 22, rank: int = 0, world: int = 1, **opt):
-    """A multi-beam plan (PAPER.md:75-80 S1-S2): Eq. 3 over all beams, one mc_dose per beam (seed + beam index) into one int64
-    grid.  With world > 1 every rank runs its contiguous share of each beam's histories; the caller all-reduces the returned
-    grid (int64, SUM: bit-exact).  Returns (acc int64 on the device, histories per beam)."""
+def plan_dose(psls, phantom, beams, n_histories: int, seed: int, batch: int = 1 << 22, rank: int = 0, world: int = 1,
+              dose_out=None, dose_acc=None, **opt):
+    """mc_plan_dose: a multi-beam plan (PAPER.md:73-80 S1-S2) - Eq. 3 over all beams, beam i with seed + i, one int64 grid.
+    With world > 1 this call runs shard `rank` of every beam's histories; the caller all-reduces the returned grid
+    (int64, SUM: bit-exact).  Returns (acc int64 on the device, histories per beam)."""
     import torch
-    n_beam = plan_allocate(psls, n_histories)
-    acc = torch.zeros(phantom.nvox, dtype=torch.int64, device=phantom.device)
-    for i, (psl, beam) in enumerate(zip(psls, beams)):
-        n = int(n_beam[i])
-        if n == 0:
-            continue
-        hb, he = shard_range(n, rank, world)
-        if hb == he:
-            continue
-        psl.dose(phantom, beam, n, seed + i, batch=batch, dose_acc=acc, history_begin=hb, history_end=he, **opt)
-    return acc, n_beam
-
-
-def atomic_peak(nvox: int, n_ops: int = 1 << 28, seed: int = 1) -> float:
-    """int64 scoring atomics per second on random voxels of an nvox grid (measurement probe)."""
-    import torch
-    acc = torch.zeros(nvox, dtype=torch.int64, device="cuda")
-    out = np.zeros(2, np.float32)
-    _check(lib().mc_atomic_peak_debug(acc.data_ptr(), nvox, n_ops, seed, out.ctypes.data_as(C.c_void_p)))
-    return float(out[1]) / (float(out[0]) * 1e-3)
+    if dose_acc is None:
+        dose_acc = torch.zeros(phantom.nvox, dtype=torch.int64, device=phantom.device)
+    if opt.get("workspace") is None:
+        opt["workspace"] = workspace(int(lib().mc_workspace_bytes(None, C.byref(phantom.c), batch)), phantom.device)
+    o = _opts(dose_acc=dose_acc, shard=(rank, world), **opt)
+    arr = (C.c_void_p * len(psls))(*[p.h for p in psls])
+    bm = (beam_geom_t * len(beams))(*[_beam(b) for b in beams])
+    n_beam = np.zeros(len(psls), np.uint64)
+    _check(lib().mc_plan_dose(arr, bm, len(psls), C.byref(phantom.c), n_histories, seed, batch,
+                              dose_out.data_ptr() if dose_out is not None else None, C.byref(o), n_beam.ctypes.data_as(C.c_void_p)))
+    return dose_acc, n_beam
 
 
 def shard_range(n_histories: int, rank: int, world: int) -> tuple[int, int]:

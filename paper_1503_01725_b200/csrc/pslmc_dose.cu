@@ -1,6 +1,7 @@
 // pslmc_dose.cu — the batching driver and the C ABI of the hot path: iterated k_sample → k_photon /
-// k_electron launches per sub-source type and energy order, secondary
-// queues, int64 scoring, finalise, stats.  No CPU fallback: every entry point here needs a device.
+// k_electron launches per sub-source type and energy order, the electron
+// queue, int64 scoring, finalise, stats.  No CPU fallback: every entry point here needs a device.
+// No process-global device state: scratch and streams are the caller's (include/pslmc.h).
 #include "pslmc_host.h"
 #include "pslmc_transport.cuh"
 
@@ -24,51 +25,32 @@ namespace pslmc {
 
 thread_local mc_stats_t g_stats;
 
-// Library-managed scratch (used when the caller passes no workspace).  One per process; calls are
-// not re-entrant (see pslmc.h).
-struct Scratch { void *ptr = nullptr; size_t bytes = 0; };
-static Scratch g_scratch, g_hostio;
-
-static int scratch_get(Scratch &s, size_t bytes, void **out) {
-  if (s.bytes < bytes) {
-    if (s.ptr) cudaFree(s.ptr);
-    s.ptr = nullptr; s.bytes = 0;
-    CUDA_TRY(cudaMalloc(&s.ptr, bytes));
-    s.bytes = bytes;
-  }
-  *out = s.ptr;
-  return MC_OK;
-}
-
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
-// Workspace layout for a batch of B primaries.  Shared by the whole call: group offsets, cross-section
-// data, packed phantom, (optionally) the int64 dose grid.  Per pipeline (kMaxPipes of them, see run_dose):
-// control block, the particle buffer (2 planes + the commissioning column), the electron queue (capacity 4B, 3 planes).
+// Workspace layout for a batch of B primaries.  Shared by the whole call: control blocks, cross-section
+// data, packed phantom, the int64 dose grid (used when the caller gives no dose_acc).  Per pipeline
+// (kMaxPipes of them, see Session): the particle buffer (2 planes + the commissioning column) and the electron
+// queue (capacity 4B, 3 planes).  mc_dose_host appends its staging area (phantom in, dose out).
 constexpr int kMaxPipes = 2;
 struct Layout {
-  size_t ctl, off, xs, vox, p0, p1, p2, eq[3], acc, total;
+  size_t ctl[kMaxPipes], xs, vox, acc, p0[kMaxPipes], p1[kMaxPipes], p2[kMaxPipes], eq[kMaxPipes][3], total;
+  size_t host_rho, host_mat, host_dose, host_total;
   unsigned eq_cap;
 };
-static void make_layouts(uint64_t batch, size_t nvox, bool with_acc, Layout out[kMaxPipes]) {
-  Layout L; size_t o = 0;
+static Layout make_layout(uint64_t batch, size_t nvox) {
+  Layout L{}; size_t o = 0;
   auto take = [&](size_t b) { size_t at = o; o += align_up(b); return at; };
   L.eq_cap = (unsigned)std::min<uint64_t>(4 * batch, 0x7fffffffu);
-  if (const char *e = getenv("PSLMC_TEST_EQ_CAP")) L.eq_cap = (unsigned)std::max(1, atoi(e));   // test hook: exercises MC_E_OVERFLOW (the planes keep their full size)
-  size_t ctl_at[kMaxPipes];
-  for (int p = 0; p < kMaxPipes; ++p) ctl_at[p] = take(sizeof(Control));     // contiguous from offset 0: zeroed by one memset
-  L.off = take(sizeof(uint64_t) * 160); L.xs = take(kXsBytes); L.vox = take(4 * nvox);
-  L.acc = take(with_acc ? 8 * nvox : 0);
+  for (int p = 0; p < kMaxPipes; ++p) L.ctl[p] = take(sizeof(Control));     // contiguous from offset 0: zeroed by one memset
+  L.xs = take(kXsBytes); L.vox = take(4 * nvox); L.acc = take(8 * nvox);
   for (int p = 0; p < kMaxPipes; ++p) {
-    Layout &Q = out[p]; Q = L;
-    Q.ctl = ctl_at[p];
-    Q.p0 = take(16 * batch); Q.p1 = take(16 * batch); Q.p2 = take(4 * batch);
-    for (int k = 0; k < 3; ++k) Q.eq[k] = take((size_t)16 * L.eq_cap);
+    L.p0[p] = take(16 * batch); L.p1[p] = take(16 * batch); L.p2[p] = take(4 * batch);
+    for (int k = 0; k < 3; ++k) L.eq[p][k] = take((size_t)16 * L.eq_cap);
   }
-  for (int p = 0; p < kMaxPipes; ++p) out[p].total = o;
-}
-static Layout make_layout(uint64_t batch, size_t nvox, bool with_acc) {
-  Layout Ls[kMaxPipes]; make_layouts(batch, nvox, with_acc, Ls); return Ls[0];
+  L.total = o;
+  L.host_rho = take(4 * nvox); L.host_mat = take(nvox); L.host_dose = take(8 * nvox);
+  L.host_total = o;
+  return L;
 }
 
 int upload_tables(psl *P) {
@@ -149,61 +131,22 @@ static bool phantom_ok(const phantom_t *ph) {
          (uint64_t)ph->nx * ph->ny * ph->nz < 0x7fffffffull;
 }
 
-// Persistent-grid size: every SM filled to the kernel's occupancy.
-// Fraction of the full persistent grid to launch.  When the packed phantom + int64 grid (12 B per voxel) do not fit L2,
-// the kernels are bound by random DRAM sectors and fewer resident warps thrash less: measured on C4 (201 MB) 56.8 ms per
-// 1e8 histories at 1.0, 53.1 at 0.75, 52.6 at 0.5; no effect on C1-C3 at 0.75, losses below (a single batch per pipeline
-// then leaves SMs idle).
-static double g_grid_scale = 1.0;
-
+// Persistent-grid size: every SM filled to the kernel's occupancy, times `scale`.
 template <typename K>
-static int persistent_blocks(K kernel, size_t smem = 0) {
+static int persistent_blocks(K kernel, size_t smem, double scale) {
   int dev = 0, sms = 0, per = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kernel, kThreads, smem);
-  return std::max(1, (int)(sms * std::max(1, per) * g_grid_scale));
+  return std::max(1, (int)(sms * std::max(1, per) * scale));
 }
-
-// L2 residency for the packed phantom (north_star (4): "read-only 3D layout that is ... L2-resident").  The random
-// voxel gathers of the transport kernels then hit L2 even when phantom + dose grid exceed it (C4: 64 MiB packed
-// phantom + 128 MiB int64 grid against 126 MB of L2); everything else on the stream is marked streaming.
-struct L2Window {
-  cudaStream_t st = nullptr; bool on = false;
-  void set(cudaStream_t s, const void *base, size_t bytes) {
-    if (!getenv("PSLMC_L2_WINDOW")) return;       // opt-in: measured 11 % SLOWER on C4, neutral elsewhere
-    int dev = 0; cudaGetDevice(&dev);
-    int max_persist = 0, max_window = 0;
-    cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev);
-    cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, dev);
-    if (max_persist <= 0 || max_window <= 0 || bytes < (8u << 20)) { cudaGetLastError(); return; }   // small phantoms stay in L2 anyway
-    size_t cur = 0; cudaDeviceGetLimit(&cur, cudaLimitPersistingL2CacheSize);
-    const size_t want = std::min<size_t>(bytes, (size_t)max_persist);
-    if (cur < want && cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) != cudaSuccess) { cudaGetLastError(); return; }
-    cudaStreamAttrValue v{};
-    v.accessPolicyWindow.base_ptr = const_cast<void *>(base);
-    v.accessPolicyWindow.num_bytes = std::min<size_t>(bytes, (size_t)max_window);
-    v.accessPolicyWindow.hitRatio = (float)std::min(1.0, (double)want / (double)v.accessPolicyWindow.num_bytes);
-    v.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
-    v.accessPolicyWindow.missProp = cudaAccessPropertyNormal;
-    if (cudaStreamSetAttribute(s, cudaStreamAttributeAccessPolicyWindow, &v) != cudaSuccess) { cudaGetLastError(); return; }
-    st = s; on = true;
-  }
-  void clear() {
-    if (!on) return;
-    cudaStreamAttrValue v{};
-    v.accessPolicyWindow.num_bytes = 0;
-    cudaStreamSetAttribute(st, cudaStreamAttributeAccessPolicyWindow, &v);
-    cudaCtxResetPersistingL2Cache();
-    on = false;
-  }
-};
 
 struct Timer {                                  // per-kernel-class CUDA-event timing (MC_FLAG_TIMING)
   bool on = false; cudaStream_t st = nullptr;
   std::vector<cudaEvent_t> ev[5];
   void begin(int cls) { if (!on) return; cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, st); ev[cls].push_back(e); }
   void end(int cls) { begin(cls); }
+  void discard() { for (auto &v : ev) { for (cudaEvent_t e : v) cudaEventDestroy(e); v.clear(); } }
   void collect(float ms[5]) {
     for (int c = 0; c < 5; ++c) {
       ms[c] = 0;
@@ -214,342 +157,308 @@ struct Timer {                                  // per-kernel-class CUDA-event t
   }
 };
 
-// Everything the launch helpers need.
-struct Run {
-  cudaStream_t st; char *ws; Layout L; Grid g; Control *ctl;
-  uint64_t seed, n_total, perm_a; int flags; bool dbg;
-  unsigned long long *fp; uint64_t fp_base;
+// One launch sequence ("pipeline"): its stream, control block, particle buffer and electron queue.
+struct Pipe {
+  cudaStream_t st = nullptr; Control *ctl = nullptr;
+  float4 *p0 = nullptr, *p1 = nullptr; uint32_t *p2 = nullptr;
+  Queue eq{};
   Timer tm; uint64_t launches[5] = {0, 0, 0, 0, 0};
-  int blocks_photon[2], blocks_electron[2];
+  bool started = false;                         // a batch has been launched on this pipeline
+};
 
-  Queue queue(const size_t off[3], unsigned *count, unsigned cap) const {
-    Queue q; q.a = (float4 *)(ws + off[0]); q.b = (float4 *)(ws + off[1]); q.c = (uint4 *)(ws + off[2]); q.count = count; q.cap = cap;
-    return q;
+// Everything one mc_dose / mc_plan_dose / mc_transport_debug call shares: workspace, phantom, kernel variants,
+// pipelines.  begin() → any number of run_beam() → end().  Nothing in between returns to the host: kernels read
+// their input counts from the device control blocks; end() synchronises once.
+struct Session {
+  char *ws = nullptr; Layout L{}; Grid g{}; size_t nvox = 0;
+  cudaStream_t us = nullptr;                    // the caller's stream
+  int npipe = 1; Pipe pipes[kMaxPipes];
+  int flags = 0; bool dbg = false, timing = false;
+  unsigned eq_cap = 0; uint64_t batch = 0;
+  XsTable xs{}; const float *rhomax = nullptr;
+  int blocks_photon = 1, blocks_electron = 1;
+  uint64_t task = 0;                            // batches dealt so far (round-robin over the pipelines)
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev_fork = nullptr, ev_join[kMaxPipes] = {};
+  Timer tm_us; uint64_t launches_us[5] = {0, 0, 0, 0, 0};
+  unsigned long long *fp = nullptr; uint64_t fp_base = 0;
+  static constexpr size_t kXsSmem = kXsBytes + sizeof(StageRing) * (kThreads / 32) + kAnnihBytes;   // k_photon dynamic shared memory
+
+  ~Session() {
+    for (cudaEvent_t e : {ev0, ev1, ev_fork, ev_join[0], ev_join[1]}) if (e) cudaEventDestroy(e);
+    tm_us.discard(); for (Pipe &p : pipes) p.tm.discard();                      // (events left by an early error return)
   }
-  TransportArgs base_args() const {
+
+  // Kernel variants: <stats + fingerprints + commissioning tally> or plain, <shared-memory staging of the scoring> or not.
+  void launch_photon(Pipe &p, const TransportArgs &a) {
+    p.tm.begin(MC_K_PHOTON);
+    const int nb = (int)std::max<uint64_t>(1, std::min<uint64_t>({(uint64_t)blocks_photon, (batch + kThreads - 1) / kThreads, 4096 / (kThreads / 32)}));
+    const size_t sm = kXsSmem + (a.stage_scoring ? kScoreBytes : 0);
+    if (a.stage_scoring) { if (dbg) k_photon<true, true><<<nb, kThreads, sm, p.st>>>(a); else k_photon<false, true><<<nb, kThreads, sm, p.st>>>(a); }
+    else { if (dbg) k_photon<true, false><<<nb, kThreads, sm, p.st>>>(a); else k_photon<false, false><<<nb, kThreads, sm, p.st>>>(a); }
+    p.tm.end(MC_K_PHOTON); ++p.launches[MC_K_PHOTON];
+  }
+  void launch_electron(Pipe &p, const TransportArgs &a) {
+    p.tm.begin(MC_K_ELECTRON);
+    const int nb = blocks_electron; const size_t sm = a.stage_scoring ? kScoreBytes : 0;
+    if (a.stage_scoring) { if (dbg) k_electron<true, true><<<nb, kThreads, sm, p.st>>>(a); else k_electron<false, true><<<nb, kThreads, sm, p.st>>>(a); }
+    else { if (dbg) k_electron<true, false><<<nb, kThreads, sm, p.st>>>(a); else k_electron<false, false><<<nb, kThreads, sm, p.st>>>(a); }
+    p.tm.end(MC_K_ELECTRON); ++p.launches[MC_K_ELECTRON];
+  }
+  void init_blocks(double scale) {
+    const bool stage = (flags & MC_FLAG_STAGE_SCORING) != 0;
+    const size_t smp = kXsSmem + (stage ? kScoreBytes : 0), sme = stage ? kScoreBytes : 0;
+#define PSLMC_SETUP(D, S)                                                                                          \
+    if (dbg == D && stage == S) {                                                                                  \
+      cudaFuncSetAttribute(k_photon<D, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smp);                 \
+      blocks_photon = persistent_blocks(k_photon<D, S>, smp, scale);                                               \
+      blocks_electron = persistent_blocks(k_electron<D, S>, sme, scale);                                           \
+    }
+    PSLMC_SETUP(false, false) PSLMC_SETUP(false, true) PSLMC_SETUP(true, false) PSLMC_SETUP(true, true)
+#undef PSLMC_SETUP
+  }
+
+  TransportArgs base_args(const Pipe &p, uint64_t seed, uint64_t n_total, uint64_t perm_a) const {
     TransportArgs a{};
-    a.g = g; a.ctl = ctl; a.seed = seed; a.n_total = n_total; a.perm_a = perm_a;
+    a.g = g; a.ctl = p.ctl; a.seed = seed; a.n_total = n_total; a.perm_a = perm_a;
     round_keys(seed, a.ks);
-    a.p0 = (const float4 *)(ws + L.p0); a.p1 = (const float4 *)(ws + L.p1); a.p2 = g.com_index ? (const uint32_t *)(ws + L.p2) : nullptr;
-    a.eq = queue(L.eq, &ctl->n_eq, L.eq_cap);
+    a.p0 = p.p0; a.p1 = p.p1; a.p2 = g.com_index ? p.p2 : nullptr;
+    a.eq = p.eq;
     a.fp = fp; a.fp_base = fp_base;
     a.electrons_local = (flags & MC_FLAG_ELECTRONS_LOCAL) ? 1 : 0;
     a.static_lanes = (flags & MC_FLAG_STATIC_LANES) ? 1 : 0;
     a.stage_scoring = (flags & MC_FLAG_STAGE_SCORING) ? 1 : 0;
-    a.xs = xs; a.rhomax = rhomax ? rhomax : ctl->rhomax;
+    a.xs = xs; a.rhomax = rhomax;
     return a;
   }
-  XsTable xs{};
-  const float *rhomax = nullptr;                 // where k_pack_phantom left the largest densities (pipeline 0's control block)
-  static constexpr size_t kXsSmem = kXsBytes + sizeof(StageRing) * (kThreads / 32) + kAnnihBytes;   // k_photon dynamic shared memory
-  // Builds the cross-section table of this call (after k_rhomax) for photon energies up to e_max.
-  void build_xs(double e_max) {
-    const double x0 = std::log2(0.045), x1 = std::log2(e_max * 1.001), hh = (x1 - x0) / kXsIntervals;
-    float *nodes = (float *)(ws + L.xs);
-    k_build_xs<<<(kXsIntervals + 256) / 256, 256, 0, st>>>(ctl, nodes, x0, hh, kXsIntervals);
-    xs.data = nodes; xs.x0 = (float)x0; xs.inv_h = (float)(1.0 / hh); xs.n = kXsIntervals;
+  void drain_electrons(Pipe &p, const TransportArgs &base) {
+    TransportArgs c = base;
+    c.src_kind = SRC_QUEUE; c.src = c.eq; c.src_count = &p.ctl->n_eq; c.src_head = &p.ctl->head_eq;
+    launch_electron(p, c);
   }
-  bool started = false;                         // a batch has been launched on this pipeline
-  uint64_t batch = 0;                           // upper bound of the entries a photon launch can see
-  int photon_blocks(int persistent) const { return (int)std::max<uint64_t>(1, std::min<uint64_t>({(uint64_t)persistent, (batch + kThreads - 1) / kThreads, 4096 / (kThreads / 32)})); }
-  void photon(const TransportArgs &a) {
-    tm.begin(MC_K_PHOTON);
-    const int nb = photon_blocks(blocks_photon[dbg]);
-    if (a.stage_scoring) {
-      if (dbg) k_photon<true, true><<<nb, kThreads, kXsSmem + kScoreBytes, st>>>(a); else k_photon<false, true><<<nb, kThreads, kXsSmem + kScoreBytes, st>>>(a);
-    } else {
-      if (dbg) k_photon<true, false><<<nb, kThreads, kXsSmem, st>>>(a); else k_photon<false, false><<<nb, kThreads, kXsSmem, st>>>(a);
+
+  // Prologue on the caller's stream: zero the control blocks (and the internal grid), pack the phantom, fork the pipelines.
+  int begin(void *workspace, size_t workspace_bytes, bool host_staging, const phantom_t &ph, long long *dose_acc, const mc_opts_t &o,
+            uint64_t batch_, const char *who) {
+    nvox = (size_t)ph.nx * ph.ny * ph.nz; batch = batch_;
+    L = make_layout(batch, nvox);
+    if (!workspace || workspace_bytes < (host_staging ? L.host_total : L.total)) {
+      char b[160]; snprintf(b, sizeof b, "%s: workspace missing or too small (see mc_workspace_bytes)", who);
+      return fail(MC_E_WORKSPACE, b);
     }
-    tm.end(MC_K_PHOTON); ++launches[MC_K_PHOTON];
-  }
-  void electron(const TransportArgs &a) {
-    tm.begin(MC_K_ELECTRON);
-    const int nb = blocks_electron[dbg];
-    if (a.stage_scoring) {
-      if (dbg) k_electron<true, true><<<nb, kThreads, kScoreBytes, st>>>(a); else k_electron<false, true><<<nb, kThreads, kScoreBytes, st>>>(a);
-    } else {
-      if (dbg) k_electron<true, false><<<nb, kThreads, 0, st>>>(a); else k_electron<false, false><<<nb, kThreads, 0, st>>>(a);
+    ws = (char *)workspace; us = (cudaStream_t)o.cuda_stream; flags = o.flags;
+    eq_cap = o.debug_eq_cap ? std::min(o.debug_eq_cap, L.eq_cap) : L.eq_cap;
+    dbg = (o.flags & MC_FLAG_STATS) || o.fingerprints || o.com_index;         // stats, fingerprints and the tally live in the DBG variants
+    timing = (o.flags & MC_FLAG_TIMING) != 0;
+    npipe = o.pipelines > 0 ? o.pipelines : kMaxPipes;
+    npipe = std::max(1, std::min(npipe, kMaxPipes));
+    for (int p = 0; p < npipe; ++p) if (npipe > 1 && !o.aux_streams[p]) npipe = 1;     // no streams given: serial
+    if (npipe > 1 && (o.aux_streams[0] == o.aux_streams[1] || o.aux_streams[0] == o.cuda_stream || o.aux_streams[1] == o.cuda_stream))
+      return fail(MC_E_INVALID_ARG, "aux_streams must be distinct from each other and from cuda_stream");
+    long long *acc = dose_acc ? dose_acc : (long long *)(ws + L.acc);
+    g = make_grid(ph, acc); g.vox = (const uint32_t *)(ws + L.vox);
+    g.com_index = (const int *)o.com_index; g.com_dose = (unsigned long long *)o.com_dose; g.com_rows = o.com_rows;
+    for (int p = 0; p < npipe; ++p) {
+      Pipe &q = pipes[p];
+      q.st = npipe > 1 ? (cudaStream_t)o.aux_streams[p] : us; q.ctl = (Control *)(ws + L.ctl[p]);
+      q.p0 = (float4 *)(ws + L.p0[p]); q.p1 = (float4 *)(ws + L.p1[p]); q.p2 = (uint32_t *)(ws + L.p2[p]);
+      q.eq.a = (float4 *)(ws + L.eq[p][0]); q.eq.b = (float4 *)(ws + L.eq[p][1]); q.eq.c = (uint4 *)(ws + L.eq[p][2]);
+      q.eq.count = &q.ctl->n_eq; q.eq.cap = eq_cap;
+      q.tm.on = timing; q.tm.st = q.st;
     }
-    tm.end(MC_K_ELECTRON); ++launches[MC_K_ELECTRON];
-  }
-  void init_blocks() {
-    const bool stage = (flags & MC_FLAG_STAGE_SCORING) != 0;
-    if (stage) {
-      cudaFuncSetAttribute(k_photon<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kXsSmem + kScoreBytes));
-      cudaFuncSetAttribute(k_photon<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kXsSmem + kScoreBytes));
-      blocks_photon[0] = persistent_blocks(k_photon<false, true>, kXsSmem + kScoreBytes); blocks_photon[1] = persistent_blocks(k_photon<true, true>, kXsSmem + kScoreBytes);
-      blocks_electron[0] = persistent_blocks(k_electron<false, true>, kScoreBytes); blocks_electron[1] = persistent_blocks(k_electron<true, true>, kScoreBytes);
-    } else {
-      cudaFuncSetAttribute(k_photon<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXsSmem);
-      cudaFuncSetAttribute(k_photon<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kXsSmem);
-      blocks_photon[0] = persistent_blocks(k_photon<false, false>, kXsSmem); blocks_photon[1] = persistent_blocks(k_photon<true, false>, kXsSmem);
-      blocks_electron[0] = persistent_blocks(k_electron<false, false>); blocks_electron[1] = persistent_blocks(k_electron<true, false>);
+    // When the packed phantom + int64 grid (12 B per voxel) do not fit L2 the kernels are bound by random DRAM sectors and
+    // fewer resident warps thrash less: measured on C4 (201 MB) 56.8 ms per 1e8 histories at 1.0, 53.1 at 0.75.
+    init_blocks(12.0 * (double)nvox > 110e6 ? 0.75 : 1.0);
+    rhomax = pipes[0].ctl->rhomax;
+    CUDA_TRY(cudaEventCreate(&ev0)); CUDA_TRY(cudaEventCreate(&ev1));
+    CUDA_TRY(cudaEventRecord(ev0, us));
+    CUDA_TRY(cudaMemsetAsync(ws, 0, L.ctl[kMaxPipes - 1] + align_up(sizeof(Control)), us));          // every pipeline's control block
+    if (!dose_acc) CUDA_TRY(cudaMemsetAsync(acc, 0, 8 * nvox, us));
+    tm_us.on = timing; tm_us.st = us;
+    tm_us.begin(MC_K_AUX);
+    k_pack_phantom<<<592, 256, 0, us>>>(ph.density, ph.material, nvox, (uint32_t *)(ws + L.vox), pipes[0].ctl);
+    tm_us.end(MC_K_AUX); ++launches_us[MC_K_AUX];
+    if (npipe > 1) {
+      CUDA_TRY(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
+      CUDA_TRY(cudaEventRecord(ev_fork, us));
+      for (int p = 0; p < npipe; ++p) CUDA_TRY(cudaStreamWaitEvent(pipes[p].st, ev_fork, 0));
     }
+    memset(&g_stats, 0, sizeof g_stats);
+    return MC_OK;
   }
-  // Folds the finished batch's counters into the per-call totals and resets them.
-  void next_batch() {
-    tm.begin(MC_K_AUX); k_next_batch<<<1, 1, 0, st>>>(ctl); tm.end(MC_K_AUX); ++launches[MC_K_AUX];
+
+  // Enqueues every launch of histories [hb, he) of an N-history allocation of one beam.
+  int run_beam(const psl_t *P, const beam_geom_t &beam, uint64_t N, uint64_t seed, uint64_t hb, uint64_t he, bool mixed) {
+    xs.data = (const float *)P->d_xs; xs.x0 = (float)P->xs_x0; xs.inv_h = (float)(1.0 / P->xs_h); xs.n = kXsIntervals;
+    std::vector<uint64_t> off(P->groups.size() + 1);
+    allocate_host(*P, N, off.data());
+    const uint64_t perm_a = mixed ? mixed_multiplier(N) : 0;
+    SampleArgs sa{};
+    sa.m = source_model(*P); sa.beam = beam_xf(beam); sa.seed = seed; round_keys(seed, sa.ks); sa.n_total = N; sa.perm_a = perm_a;
+    for (size_t i = 0; i < off.size(); ++i) sa.off_g[i] = off[i];
+    sa.fp = fp; sa.fp_base = fp_base; sa.compact = 1; sa.g = g; sa.stats = dbg ? 1 : 0;
+    auto sample_batch = [&](Pipe &p, uint64_t first, uint64_t count) {
+      if (p.started) { p.tm.begin(MC_K_AUX); k_next_batch<<<1, 1, 0, p.st>>>(p.ctl); p.tm.end(MC_K_AUX); ++p.launches[MC_K_AUX]; }
+      p.started = true;                                   // (a pipeline's first batch finds the control block freshly zeroed)
+      sa.first = first; sa.count = (unsigned)count; sa.p0 = p.p0; sa.p1 = p.p1; sa.ctl = p.ctl;
+      sa.p2 = g.com_index ? p.p2 : nullptr;
+      p.tm.begin(MC_K_SAMPLE);
+      k_sample<<<(unsigned)((count + kThreads - 1) / kThreads), kThreads, 0, p.st>>>(sa);
+      p.tm.end(MC_K_SAMPLE); ++p.launches[MC_K_SAMPLE];
+    };
+    auto photon_batch = [&](Pipe &p, uint64_t first) {   // the photons of the particle buffer, then every electron they queued
+      TransportArgs a = base_args(p, seed, N, perm_a);
+      a.src_kind = SRC_BUFFER; a.buffer_is_debug = 0; a.first = first; a.want_type = 0;
+      a.src_count = &p.ctl->n_pb; a.src_head = &p.ctl->head_pb;
+      launch_photon(p, a);
+      drain_electrons(p, a);
+    };
+    auto electron_batch = [&](Pipe &p, uint64_t first, unsigned *head) {     // contamination electrons straight from the buffer
+      TransportArgs a = base_args(p, seed, N, perm_a);
+      a.src_kind = SRC_BUFFER; a.buffer_is_debug = 0; a.first = first; a.want_type = 1;
+      a.src_count = &p.ctl->n_pb; a.src_head = head;
+      launch_electron(p, a);
+    };
+    const int ne = P->n_ebin;
+    if (!mixed) {
+      // one sub-source type at a time, energy bins ascending, M histories per launch
+      for (int s = 0; s < 3; ++s) {
+        const uint64_t lo = std::max(hb, off[(size_t)s * ne]), hi = std::min(he, off[(size_t)(s + 1) * ne]);
+        if (lo >= hi) continue;
+        g_stats.n_hist[s] += hi - lo;
+        // equal batches: ceil(n / batch) launches of the same size (a short last batch is mostly tail)
+        const uint64_t nb = (hi - lo + batch - 1) / batch, even = std::min(batch, (((hi - lo + nb - 1) / nb) + kThreads - 1) / kThreads * kThreads);
+        for (uint64_t first = lo; first < hi; first += even, ++task) {
+          Pipe &p = pipes[task % npipe];
+          sample_batch(p, first, std::min(even, hi - first));
+          if (P->psr.particle_type[s] == 0) photon_batch(p, first);
+          else electron_batch(p, first, &p.ctl->head_pb);
+        }
+      }
+    } else {
+      for (uint64_t first = hb; first < he; first += batch, ++task) {
+        Pipe &p = pipes[task % npipe];
+        sample_batch(p, first, std::min(batch, he - first));
+        electron_batch(p, first, &p.ctl->head_pb_e);
+        photon_batch(p, first);
+      }
+      if (hb == 0 && he == N) for (int s = 0; s < 3; ++s) g_stats.n_hist[s] += off[(size_t)(s + 1) * ne] - off[(size_t)s * ne];   // (not tracked per range)
+    }
+    CUDA_TRY(cudaGetLastError());
+    return MC_OK;
   }
-  const float4 *dbg_p0 = nullptr, *dbg_p1 = nullptr;
-  // mc_transport_debug: photons of the caller's buffer, then every queued electron
-  void transport_photon_debug(uint64_t first, const unsigned *count_ptr) {
-    TransportArgs a = base_args();
-    a.src_kind = SRC_BUFFER; a.buffer_is_debug = 1; a.first = first; a.want_type = 0;
-    a.src_count = count_ptr; a.src_head = &ctl->head_pb; a.p0 = dbg_p0; a.p1 = dbg_p1;
-    photon(a);
-    drain_electrons();
+
+  // Joins the pipelines, converts (or only scans) the grid, synchronises once, folds the control blocks into g_stats.
+  int end(const phantom_t &ph, double *dose_out, uint64_t n_norm, uint64_t n_run, const char *who) {
+    for (int p = 0; p < npipe && npipe > 1; ++p) {
+      CUDA_TRY(cudaEventCreateWithFlags(&ev_join[p], cudaEventDisableTiming));
+      CUDA_TRY(cudaEventRecord(ev_join[p], pipes[p].st));
+      CUDA_TRY(cudaStreamWaitEvent(us, ev_join[p], 0));
+    }
+    tm_us.begin(MC_K_FINALISE);
+    const double inv_vn = 1.0 / (ph.dx * ph.dy * ph.dz * (double)std::max<uint64_t>(1, n_norm));
+    k_finalise<<<592, 256, 0, us>>>((const long long *)g.acc, ph.density, nvox, inv_vn, dose_out, pipes[0].ctl);
+    tm_us.end(MC_K_FINALISE); ++launches_us[MC_K_FINALISE];
+    CUDA_TRY(cudaEventRecord(ev1, us));
+    CUDA_TRY(cudaGetLastError());
+    Control hc[kMaxPipes];
+    for (int p = 0; p < npipe; ++p) CUDA_TRY(cudaMemcpyAsync(&hc[p], pipes[p].ctl, sizeof(Control), cudaMemcpyDeviceToHost, us));
+    CUDA_TRY(cudaStreamSynchronize(us));
+    CUDA_TRY(cudaEventElapsedTime(&g_stats.ms_total, ev0, ev1));
+    // fold the pipelines: kernel-class times add up (they overlap in wall time), counters and ledgers sum exactly
+    tm_us.collect(g_stats.ms);
+    Control &c = hc[0];
+    for (int p = 0; p < npipe; ++p) {
+      hc[p].n_accepted += hc[p].n_pb; hc[p].hw_eq = std::max(hc[p].hw_eq, hc[p].n_eq);      // what k_next_batch would have folded for the last batch
+      float ms[5]; pipes[p].tm.collect(ms);
+      for (int k = 0; k < 5; ++k) { g_stats.ms[k] += ms[k]; launches_us[k] += pipes[p].launches[k]; }
+      if (p == 0) continue;
+      for (int sl = 0; sl < kLedgerSlots; ++sl)
+        for (int k = 0; k < 4; ++k) {
+          unsigned __int128 a = ((unsigned __int128)c.ledger[sl][k][1] << 64) | c.ledger[sl][k][0];
+          a += ((unsigned __int128)hc[p].ledger[sl][k][1] << 64) | hc[p].ledger[sl][k][0];
+          c.ledger[sl][k][0] = (unsigned long long)a; c.ledger[sl][k][1] = (unsigned long long)(a >> 64);
+        }
+      for (int k = 0; k < ST_COUNT; ++k) c.stat[k] += hc[p].stat[k];
+      c.hw_eq = std::max(c.hw_eq, hc[p].hw_eq);
+      c.n_accepted += hc[p].n_accepted; c.n_missed += hc[p].n_missed; c.overflow |= hc[p].overflow; c.bad_input |= hc[p].bad_input;
+    }
+    mc_stats_t *s = &g_stats;
+    for (int k = 0; k < 4; ++k) {
+      unsigned __int128 tot = 0;
+      for (int sl = 0; sl < kLedgerSlots; ++sl) tot += ((unsigned __int128)c.ledger[sl][k][1] << 64) | c.ledger[sl][k][0];
+      s->ledger_hi[k] = (int64_t)(uint64_t)(tot >> 64); s->ledger_lo[k] = (uint64_t)tot;
+    }
+    s->n_missed = c.stat[ST_MISSED]; s->n_flights = c.stat[ST_FLIGHTS]; s->n_virtual = c.stat[ST_VIRTUAL];
+    s->n_compton = c.stat[ST_COMPTON]; s->n_photo = c.stat[ST_PHOTO]; s->n_pair = c.stat[ST_PAIR];
+    s->n_photon_cutoff = c.stat[ST_PCUT]; s->n_photon_escape = c.stat[ST_PESC]; s->n_uncollided_escape = c.stat[ST_UNCOLLIDED];
+    s->n_sec_electrons = c.stat[ST_SEC_E]; s->n_sec_photons = c.stat[ST_SEC_P];
+    s->n_electron_tracks = c.stat[ST_ETRACKS]; s->n_electron_steps = c.stat[ST_ESTEPS]; s->n_electron_escape = c.stat[ST_EESC];
+    s->n_deposits = c.stat[ST_DEPOSITS]; s->n_kahn_trials = c.stat[ST_KAHN]; s->n_deflections = c.stat[ST_DEFLECT];
+    s->queue_high_water = c.hw_eq;
+    for (int k = 0; k < 5; ++k) s->launches[k] = launches_us[k];
+    s->n_jaw_rejected = n_run >= c.n_accepted + c.n_missed ? n_run - c.n_accepted - c.n_missed : 0;
+    char b[200];
+    if (c.overflow & 1u) { snprintf(b, sizeof b, "%s: the electron queue overflowed (capacity %u entries); use a larger batch workspace", who, eq_cap); return fail(MC_E_OVERFLOW, b); }
+    if (c.overflow & 2u) { snprintf(b, sizeof b, "%s: a voxel's int64 accumulator wrapped (more than 2^63 quanta = 2.1e9 MeV in one voxel)", who); return fail(MC_E_OVERFLOW, b); }
+    if (c.bad_input) { snprintf(b, sizeof b, "%s: a particle energy outside [0, 4096) MeV", who); return fail(MC_E_INVALID_ARG, b); }
+    return MC_OK;
   }
-  // mc_dose: call right after k_sample.  The photons of the particle buffer (annihilation photons are transported
-  // inside the launch by the converting lane), then every electron they queued.
-  void transport_photon_batch(uint64_t first) {
-    TransportArgs a = base_args();
-    a.src_kind = SRC_BUFFER; a.buffer_is_debug = 0; a.first = first; a.want_type = 0;
-    a.src_count = &ctl->n_pb; a.src_head = &ctl->head_pb;
-    photon(a);
-    drain_electrons();
-  }
-  void drain_electrons() {
-    TransportArgs c = base_args();
-    c.src_kind = SRC_QUEUE; c.src = c.eq; c.src_count = &ctl->n_eq; c.src_head = &ctl->head_eq;
-    electron(c);
-  }
-  void transport_electron_buffer(uint64_t first, bool debug_buffer, const unsigned *count_ptr, unsigned *head) {
-    TransportArgs a = base_args();
-    a.src_kind = SRC_BUFFER; a.buffer_is_debug = debug_buffer; a.first = first; a.want_type = 1;
-    a.src_count = count_ptr; a.src_head = head;
-    electron(a);
+
+  static uint64_t gcd_u64(uint64_t a, uint64_t b) { while (b) { uint64_t t = a % b; a = b; b = t; } return a; }
+  // Mixed order (ablation): thread t handles history (a*t) mod N, a = smallest integer >= floor(0.618...N) coprime to N.
+  static uint64_t mixed_multiplier(uint64_t N) {
+    if (N < 3) return 1;
+    uint64_t a = (uint64_t)(0.6180339887 * (double)N);
+    if (a < 1) a = 1;
+    while (gcd_u64(a, N) != 1) ++a;
+    return a;
   }
 };
 
-// Adds the per-call part of `src` (ledgers, counters, totals) into `dst` (pipelines are folded on the host).
-static void merge_control(Control &dst, const Control &src) {
-  for (int sl = 0; sl < kLedgerSlots; ++sl)
-    for (int k = 0; k < 4; ++k) {
-      unsigned __int128 a = ((unsigned __int128)dst.ledger[sl][k][1] << 64) | dst.ledger[sl][k][0];
-      a += ((unsigned __int128)src.ledger[sl][k][1] << 64) | src.ledger[sl][k][0];
-      dst.ledger[sl][k][0] = (unsigned long long)a; dst.ledger[sl][k][1] = (unsigned long long)(a >> 64);
-    }
-  for (int k = 0; k < ST_COUNT; ++k) dst.stat[k] += src.stat[k];
-  dst.hw_eq = std::max(dst.hw_eq, src.hw_eq);
-  dst.n_accepted += src.n_accepted; dst.n_missed += src.n_missed; dst.overflow |= src.overflow;
+constexpr uint64_t kMaxHistories = 1ull << 53;        // Eq. 3 is evaluated in double: N must be exactly representable
+
+static int check_common(const psl_t *P, const phantom_t *ph, uint64_t N, uint64_t batch, const mc_opts_t *o, const char *who) {
+  char b[200];
+  if (!P || !phantom_ok(ph) || N == 0 || N > kMaxHistories || batch == 0 || batch > (1ull << 30)) {
+    snprintf(b, sizeof b, "%s: invalid argument (null handle, bad phantom, n_histories outside [1, 2^53] or batch outside [1, 2^30])", who);
+    return fail(MC_E_INVALID_ARG, b);
+  }
+  if (o->reserved || o->reserved2) { snprintf(b, sizeof b, "%s: reserved fields of mc_opts_t must be 0", who); return fail(MC_E_INVALID_ARG, b); }
+  int dev = 0; CUDA_TRY(cudaGetDevice(&dev));
+  if (dev != P->device) { snprintf(b, sizeof b, "%s: psl_t was built on device %d, the current device is %d", who, P->device, dev); return fail(MC_E_INVALID_ARG, b); }
+  return MC_OK;
 }
 
-static void fold_stats(const Control &c, const Run &r, mc_stats_t *s) {
-  for (int k = 0; k < 4; ++k) {
-    unsigned __int128 tot = 0;
-    for (int sl = 0; sl < kLedgerSlots; ++sl) tot += ((unsigned __int128)c.ledger[sl][k][1] << 64) | c.ledger[sl][k][0];
-    s->ledger_hi[k] = (int64_t)(uint64_t)(tot >> 64); s->ledger_lo[k] = (uint64_t)tot;
+// The driver proper.  All pointers inside `ph` are DEVICE pointers here.
+static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam, uint64_t N, uint64_t seed, uint64_t batch,
+                    double *dose_out, const mc_opts_t *opts, bool host_staging) {
+  static const mc_opts_t kDefaults = {};
+  if (!opts) opts = &kDefaults;
+  if (!beam || (!dose_out && !opts->dose_acc)) return fail(MC_E_INVALID_ARG, "mc_dose: invalid argument (beam, or neither dose_out nor dose_acc)");
+  if (int rc = check_common(P, ph, N, batch, opts, "mc_dose")) return rc;
+  const bool ranged = (opts->flags & MC_FLAG_RANGE) != 0;
+  const uint64_t hb = opts->history_begin, he = (ranged || opts->history_end) ? opts->history_end : N;
+  if (hb > he || he > N) return fail(MC_E_INVALID_ARG, "mc_dose: history range outside [0, n_histories]");
+  const bool mixed = opts->order == MC_ORDER_MIXED;
+  if (mixed && (N >> 32)) return fail(MC_E_INVALID_ARG, "mc_dose: mixed order needs n_histories < 2^32");
+  if (mixed && opts->fingerprints && (hb != 0 || he != N)) return fail(MC_E_INVALID_ARG, "mc_dose: mixed order + fingerprints needs the full range");
+  if (opts->com_index) {
+    if (!opts->com_dose || opts->com_rows < 1 || opts->com_cols != 2 * P->n_ebin * P->n_ring + P->n_ebin)
+      return fail(MC_E_INVALID_ARG, "mc_dose: commissioning tally needs com_dose, com_rows >= 1 and com_cols = 2*n_ebin*n_ring + n_ebin");
+    if (P->psr.particle_type[0] != 0 || P->psr.particle_type[1] != 0 || P->psr.particle_type[2] != 1)
+      return fail(MC_E_INVALID_ARG, "mc_dose: the commissioning columns are defined for particle_type = {0, 0, 1} (two photon sub-sources, one electron sub-source)");
+    if (mixed) return fail(MC_E_INVALID_ARG, "mc_dose: the commissioning tally runs in sorted order");
   }
-  s->n_missed = c.stat[ST_MISSED]; s->n_flights = c.stat[ST_FLIGHTS]; s->n_virtual = c.stat[ST_VIRTUAL];
-  s->n_compton = c.stat[ST_COMPTON]; s->n_photo = c.stat[ST_PHOTO]; s->n_pair = c.stat[ST_PAIR];
-  s->n_photon_cutoff = c.stat[ST_PCUT]; s->n_photon_escape = c.stat[ST_PESC]; s->n_uncollided_escape = c.stat[ST_UNCOLLIDED];
-  s->n_sec_electrons = c.stat[ST_SEC_E]; s->n_sec_photons = c.stat[ST_SEC_P];
-  s->n_electron_tracks = c.stat[ST_ETRACKS]; s->n_electron_steps = c.stat[ST_ESTEPS]; s->n_electron_escape = c.stat[ST_EESC];
-  s->n_deposits = c.stat[ST_DEPOSITS];
-  s->queue_high_water[0] = c.hw_eq; s->queue_high_water[1] = 0;    // no photon queue: annihilation photons stay in their lane
-  for (int k = 0; k < 5; ++k) s->launches[k] = r.launches[k];
+  Session S;
+  S.fp = (unsigned long long *)opts->fingerprints; S.fp_base = hb;
+  if (int rc = S.begin(opts->workspace, opts->workspace_bytes, host_staging, *ph, (long long *)opts->dose_acc, *opts, batch, "mc_dose")) return rc;
+  if (int rc = S.run_beam(P, *beam, N, seed, hb, he, mixed)) return rc;
+  return S.end(*ph, dose_out, N, he - hb, "mc_dose");
 }
 
 }  // namespace pslmc
 
 using namespace pslmc;
-
-static uint64_t gcd_u64(uint64_t a, uint64_t b) { while (b) { uint64_t t = a % b; a = b; b = t; } return a; }
-
-// Mixed order (ablation): thread t handles history (a*t) mod N, a = smallest integer >= floor(0.618...N) coprime to N.
-static uint64_t mixed_multiplier(uint64_t N) {
-  if (N < 3) return 1;
-  uint64_t a = (uint64_t)(0.6180339887 * (double)N);
-  if (a < 1) a = 1;
-  while (gcd_u64(a, N) != 1) ++a;
-  return a;
-}
-
-// Number of pipelines of a call (PSLMC_PIPELINES = 1 switches the overlap off) and their streams (created once).
-static int pipe_count(int requested) {
-  const char *e = getenv("PSLMC_PIPELINES");
-  const int n = requested > 0 ? requested : (e ? atoi(e) : kMaxPipes);
-  return std::max(1, std::min(n, kMaxPipes));
-}
-static const std::vector<cudaStream_t> *pipe_streams() {
-  static std::vector<cudaStream_t> st;
-  static int dev_of = -1;
-  int dev = 0; cudaGetDevice(&dev);
-  if (st.empty() || dev_of != dev) {
-    st.clear();
-    for (int p = 0; p < kMaxPipes; ++p) {
-      cudaStream_t s = nullptr;
-      if (cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); st.clear(); return nullptr; }
-      st.push_back(s);
-    }
-    dev_of = dev;
-  }
-  return &st;
-}
-
-// The driver proper.  All pointers inside `ph` are DEVICE pointers here.
-static int run_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam, uint64_t N, uint64_t seed, uint64_t batch,
-                    double *dose_out, const mc_opts_t *opts) {
-  static const mc_opts_t kDefaults = {};
-  if (!opts) opts = &kDefaults;
-  if (!P || !beam || !phantom_ok(ph) || N == 0 || batch == 0 || batch > (1ull << 30) || (!dose_out && !opts->dose_acc))
-    return fail(MC_E_INVALID_ARG, "mc_dose: invalid argument");
-  const uint64_t hb = opts->history_begin, he = opts->history_end ? opts->history_end : N;
-  if (hb > he || he > N) return fail(MC_E_INVALID_ARG, "mc_dose: history range outside [0, n_histories]");
-  const bool mixed = opts->order == MC_ORDER_MIXED;
-  if (mixed && (N >> 32)) return fail(MC_E_INVALID_ARG, "mc_dose: mixed order needs n_histories < 2^32");
-  if (mixed && opts->fingerprints && (hb != 0 || he != N)) return fail(MC_E_INVALID_ARG, "mc_dose: mixed order + fingerprints needs the full range");
-  if (opts->com_index && (!opts->com_dose || opts->com_rows < 1 || opts->com_cols != 2 * P->n_ebin * P->n_ring + P->n_ebin))
-    return fail(MC_E_INVALID_ARG, "mc_dose: commissioning tally needs com_dose, com_rows >= 1 and com_cols = 2*n_ebin*n_ring + n_ebin");
-  if (opts->com_index && mixed) return fail(MC_E_INVALID_ARG, "mc_dose: the commissioning tally runs in sorted order");
-  int dev = 0; CUDA_TRY(cudaGetDevice(&dev));
-  if (dev != P->device) return fail(MC_E_INVALID_ARG, "mc_dose: psl_t was built on another device");
-
-  const size_t nvox = (size_t)ph->nx * ph->ny * ph->nz;
-  Layout Ls[kMaxPipes];
-  make_layouts(batch, nvox, opts->dose_acc == nullptr, Ls);
-  const Layout &L = Ls[0];
-  void *ws = opts->workspace;
-  if (ws) { if (opts->workspace_bytes < L.total) return fail(MC_E_WORKSPACE, "mc_dose: workspace too small (see mc_workspace_bytes)"); }
-  else { int rc = scratch_get(g_scratch, L.total, &ws); if (rc) return rc; }
-
-  // Pipelines: batches are dealt round-robin to npipe independent launch sequences, each with its own control
-  // block, particle buffer, queues and stream, all scoring into the one int64 grid.  Every transport kernel is
-  // a persistent grid that fills the GPU, so the CTAs of one pipeline's next kernel start as the other
-  // pipeline's kernel drains: the tails (lanes finishing their last, longest histories) overlap with useful
-  // work instead of leaving SMs idle.  Integer tallies keep the result bit-identical for any npipe.
-  const std::vector<cudaStream_t> *pstreams = nullptr;
-  int npipe = pipe_count(opts->pipelines);
-  if (npipe > 1 && !(pstreams = pipe_streams())) npipe = 1;
-  cudaStream_t us = (cudaStream_t)opts->cuda_stream;
-  long long *acc = opts->dose_acc ? (long long *)opts->dose_acc : (long long *)((char *)ws + L.acc);
-
-  Run pipes[kMaxPipes];
-  for (int p = 0; p < npipe; ++p) {
-    Run &r = pipes[p];
-    r.st = npipe > 1 ? (*pstreams)[p] : us; r.ws = (char *)ws; r.L = Ls[p]; r.ctl = (Control *)(r.ws + Ls[p].ctl);
-    r.g = make_grid(*ph, acc); r.g.vox = (const uint32_t *)(r.ws + L.vox);
-    r.g.com_index = (const int *)opts->com_index; r.g.com_dose = (unsigned long long *)opts->com_dose; r.g.com_rows = opts->com_rows;
-    r.seed = seed; r.n_total = N; r.perm_a = mixed ? mixed_multiplier(N) : 0; r.flags = opts->flags; r.batch = batch;
-    r.fp = (unsigned long long *)opts->fingerprints; r.fp_base = hb;
-    r.dbg = (opts->flags & MC_FLAG_STATS) || opts->fingerprints || opts->com_index;   // the tally lives in the stats variants
-    r.tm.on = (opts->flags & MC_FLAG_TIMING) != 0; r.tm.st = r.st;
-    if (p == 0) { g_grid_scale = 12.0 * (double)nvox > 110e6 ? 0.75 : 1.0; r.init_blocks(); }
-    else { for (int k = 0; k < 2; ++k) { r.blocks_photon[k] = pipes[0].blocks_photon[k]; r.blocks_electron[k] = pipes[0].blocks_electron[k]; } }
-  }
-  Run &r0 = pipes[0];
-
-  std::vector<uint64_t> off(P->groups.size() + 1);
-  allocate_host(*P, N, off.data());
-  unsigned long long *d_off = (unsigned long long *)((char *)ws + L.off);
-
-  // ---- prologue on the caller's stream
-  cudaEvent_t ev0, ev1;
-  CUDA_TRY(cudaEventCreate(&ev0)); CUDA_TRY(cudaEventCreate(&ev1));
-  CUDA_TRY(cudaEventRecord(ev0, us));
-  CUDA_TRY(cudaMemsetAsync(ws, 0, align_up(sizeof(Control)) * kMaxPipes, us));          // every pipeline's control block
-  CUDA_TRY(cudaMemcpyAsync(d_off, off.data(), sizeof(uint64_t) * off.size(), cudaMemcpyHostToDevice, us));
-  if (!opts->dose_acc) CUDA_TRY(cudaMemsetAsync(acc, 0, 8 * nvox, us));
-  Timer tm_us; tm_us.on = r0.tm.on; tm_us.st = us;
-  uint64_t launches_us[5] = {0, 0, 0, 0, 0};
-  tm_us.begin(MC_K_AUX);
-  k_pack_phantom<<<592, 256, 0, us>>>(ph->density, ph->material, nvox, (uint32_t *)((char *)ws + L.vox), r0.ctl);
-  r0.xs.data = (const float *)P->d_xs; r0.xs.x0 = (float)P->xs_x0; r0.xs.inv_h = (float)(1.0 / P->xs_h); r0.xs.n = kXsIntervals;
-  tm_us.end(MC_K_AUX); launches_us[MC_K_AUX] += 1;
-  for (int p = 0; p < npipe; ++p) { pipes[p].xs = r0.xs; pipes[p].rhomax = r0.ctl->rhomax; }
-  L2Window l2w; l2w.set(us, (char *)ws + L.vox, 4 * nvox);
-  cudaEvent_t ev_fork = nullptr, ev_join[kMaxPipes] = {};
-  if (npipe > 1) {
-    CUDA_TRY(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
-    CUDA_TRY(cudaEventRecord(ev_fork, us));
-    for (int p = 0; p < npipe; ++p) CUDA_TRY(cudaStreamWaitEvent(pipes[p].st, ev_fork, 0));
-  }
-
-  SampleArgs sa[kMaxPipes];
-  for (int p = 0; p < npipe; ++p) {
-    Run &r = pipes[p]; SampleArgs &a = sa[p]; a = SampleArgs{};
-    a.m = source_model(*P); a.beam = beam_xf(*beam); a.off_g = d_off; a.seed = seed; round_keys(seed, a.ks); a.n_total = N; a.perm_a = r.perm_a;
-    a.p0 = (float4 *)(r.ws + r.L.p0); a.p1 = (float4 *)(r.ws + r.L.p1); a.ctl = r.ctl; a.fp = r.fp; a.fp_base = hb; a.compact = 1; a.g = r.g; a.stats = r.dbg ? 1 : 0;
-    a.p2 = r.g.com_index ? (uint32_t *)(r.ws + r.L.p2) : nullptr;
-  }
-
-  memset(&g_stats, 0, sizeof g_stats);
-  auto sample_batch = [&](int p, uint64_t first, uint64_t count) {
-    Run &r = pipes[p];
-    if (r.started) r.next_batch();                      // (a pipeline's first batch finds the control block freshly zeroed)
-    r.started = true;
-    sa[p].first = first; sa[p].count = (unsigned)count;
-    r.tm.begin(MC_K_SAMPLE);
-    k_sample<<<(unsigned)((count + kThreads - 1) / kThreads), kThreads, 0, r.st>>>(sa[p]);
-    r.tm.end(MC_K_SAMPLE); ++r.launches[MC_K_SAMPLE];
-  };
-  const int ne = P->n_ebin;
-  uint64_t task = 0;
-  if (!mixed) {
-    // one sub-source type at a time, energy bins ascending, M histories per launch
-    for (int s = 0; s < 3; ++s) {
-      const uint64_t lo = std::max(hb, off[(size_t)s * ne]), hi = std::min(he, off[(size_t)(s + 1) * ne]);
-      if (lo >= hi) continue;
-      g_stats.n_hist[s] = hi - lo;
-      // equal batches: ceil(n / batch) launches of the same size (a short last batch is mostly tail)
-      const uint64_t nb = (hi - lo + batch - 1) / batch, even = std::min(batch, (((hi - lo + nb - 1) / nb) + kThreads - 1) / kThreads * kThreads);
-      for (uint64_t first = lo; first < hi; first += even, ++task) {
-        const int p = (int)(task % npipe); Run &r = pipes[p];
-        sample_batch(p, first, std::min(even, hi - first));
-        if (P->psr.particle_type[s] == 0) r.transport_photon_batch(first);
-        else r.transport_electron_buffer(first, false, &r.ctl->n_pb, &r.ctl->head_pb);
-      }
-    }
-  } else {
-    for (int s = 0; s < 3; ++s) g_stats.n_hist[s] = 0;     // mixed: per-type counts are not tracked per range
-    for (uint64_t first = hb; first < he; first += batch, ++task) {
-      const int p = (int)(task % npipe); Run &r = pipes[p];
-      sample_batch(p, first, std::min(batch, he - first));
-      r.transport_electron_buffer(first, false, &r.ctl->n_pb, &r.ctl->pad0);
-      r.transport_photon_batch(first);
-    }
-    if (hb == 0 && he == N) for (int s = 0; s < 3; ++s) g_stats.n_hist[s] = off[(size_t)(s + 1) * ne] - off[(size_t)s * ne];
-  }
-  for (int p = 0; p < npipe; ++p) {
-    Run &r = pipes[p];                                // (the last batch's counters are folded on the host, below: no launch)
-    if (npipe > 1) {
-      CUDA_TRY(cudaEventCreateWithFlags(&ev_join[p], cudaEventDisableTiming));
-      CUDA_TRY(cudaEventRecord(ev_join[p], r.st));
-      CUDA_TRY(cudaStreamWaitEvent(us, ev_join[p], 0));
-    }
-  }
-  if (dose_out) {
-    tm_us.begin(MC_K_FINALISE);
-    const double inv_vn = 1.0 / (ph->dx * ph->dy * ph->dz * (double)N);
-    k_finalise<<<592, 256, 0, us>>>(acc, ph->density, nvox, inv_vn, dose_out);
-    tm_us.end(MC_K_FINALISE); ++launches_us[MC_K_FINALISE];
-  }
-  CUDA_TRY(cudaEventRecord(ev1, us));
-  CUDA_TRY(cudaGetLastError());
-  Control hc[kMaxPipes];
-  for (int p = 0; p < npipe; ++p) CUDA_TRY(cudaMemcpyAsync(&hc[p], pipes[p].ctl, sizeof(Control), cudaMemcpyDeviceToHost, us));
-  CUDA_TRY(cudaStreamSynchronize(us));
-  for (int p = 0; p < npipe; ++p) {                     // what k_next_batch would have folded for the last batch of each pipeline
-    hc[p].n_accepted += hc[p].n_pb; hc[p].hw_eq = std::max(hc[p].hw_eq, hc[p].n_eq);
-  }
-  l2w.clear();
-  CUDA_TRY(cudaEventElapsedTime(&g_stats.ms_total, ev0, ev1));
-  cudaEventDestroy(ev0); cudaEventDestroy(ev1);
-  if (ev_fork) cudaEventDestroy(ev_fork);
-  for (int p = 0; p < npipe; ++p) if (ev_join[p]) cudaEventDestroy(ev_join[p]);
-  // fold the pipelines: kernel-class times add up (they overlap in wall time), counters and ledgers sum exactly
-  tm_us.collect(g_stats.ms);
-  for (int p = 0; p < npipe; ++p) {
-    float ms[5]; pipes[p].tm.collect(ms);
-    for (int k = 0; k < 5; ++k) { g_stats.ms[k] += ms[k]; launches_us[k] += pipes[p].launches[k]; }
-    if (p > 0) merge_control(hc[0], hc[p]);
-  }
-  for (int k = 0; k < 5; ++k) r0.launches[k] = launches_us[k];
-  fold_stats(hc[0], r0, &g_stats);
-  g_stats.n_jaw_rejected = (he - hb) - hc[0].n_accepted - hc[0].n_missed;
-  if (hc[0].overflow) return fail(MC_E_OVERFLOW, "mc_dose: a secondary queue overflowed; use a larger batch workspace");
-  return MC_OK;
-}
 
 extern "C" void psl_free(psl_t *P) {
   if (!P) return;
@@ -586,34 +495,64 @@ extern "C" int psl_set_direction_model(psl_t *P, int32_t stype, int32_t K, const
   return MC_OK;
 }
 
-extern "C" size_t mc_workspace_bytes(const psl_t *P, const phantom_t *ph, uint64_t batch) {
-  if (!P || !ph || ph->nx <= 0 || ph->ny <= 0 || ph->nz <= 0 || batch == 0 || batch > (1ull << 30)) return 0;
-  return make_layout(batch, (size_t)ph->nx * ph->ny * ph->nz, true).total;
+extern "C" size_t mc_workspace_bytes(const psl_t *, const phantom_t *ph, uint64_t batch) {
+  if (!ph || ph->nx <= 0 || ph->ny <= 0 || ph->nz <= 0 || batch == 0 || batch > (1ull << 30)) return 0;
+  return make_layout(batch, (size_t)ph->nx * ph->ny * ph->nz).total;
+}
+extern "C" size_t mc_host_workspace_bytes(const psl_t *, const phantom_t *ph, uint64_t batch) {
+  if (!ph || ph->nx <= 0 || ph->ny <= 0 || ph->nz <= 0 || batch == 0 || batch > (1ull << 30)) return 0;
+  return make_layout(batch, (size_t)ph->nx * ph->ny * ph->nz).host_total;
 }
 
 extern "C" int mc_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam, uint64_t n_histories, uint64_t seed,
                        uint64_t batch, double *dose_out, const mc_opts_t *opts) {
-  return run_dose(P, ph, beam, n_histories, seed, batch, dose_out, opts);
+  return run_dose(P, ph, beam, n_histories, seed, batch, dose_out, opts, false);
 }
 
 extern "C" int mc_dose_host(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam, uint64_t n_histories, uint64_t seed,
                             uint64_t batch, double *dose_out_host, const mc_opts_t *opts) {
-  if (!ph || ph->nx <= 0 || ph->ny <= 0 || ph->nz <= 0 || !ph->density || !ph->material || !dose_out_host)
-    return fail(MC_E_INVALID_ARG, "mc_dose_host: invalid argument");
+  if (!ph || ph->nx <= 0 || ph->ny <= 0 || ph->nz <= 0 || !ph->density || !ph->material || !dose_out_host || !opts || batch == 0 || batch > (1ull << 30))
+    return fail(MC_E_INVALID_ARG, "mc_dose_host: invalid argument (opts with a workspace is required)");
   const size_t nvox = (size_t)ph->nx * ph->ny * ph->nz;
-  const size_t o_rho = 0, o_mat = align_up(4 * nvox), o_dose = o_mat + align_up(nvox), total = o_dose + 8 * nvox;
-  void *io = nullptr;
-  int rc = scratch_get(g_hostio, total, &io); if (rc) return rc;
-  cudaStream_t st = opts ? (cudaStream_t)opts->cuda_stream : nullptr;
-  char *b = (char *)io;
-  CUDA_TRY(cudaMemcpyAsync(b + o_rho, ph->density, 4 * nvox, cudaMemcpyHostToDevice, st));
-  CUDA_TRY(cudaMemcpyAsync(b + o_mat, ph->material, nvox, cudaMemcpyHostToDevice, st));
-  phantom_t d = *ph; d.density = (const float *)(b + o_rho); d.material = (const uint8_t *)(b + o_mat);
-  rc = run_dose(P, &d, beam, n_histories, seed, batch, (double *)(b + o_dose), opts);
+  const Layout L = make_layout(batch, nvox);
+  if (!opts->workspace || opts->workspace_bytes < L.host_total) return fail(MC_E_WORKSPACE, "mc_dose_host: workspace missing or too small (see mc_host_workspace_bytes)");
+  cudaStream_t st = (cudaStream_t)opts->cuda_stream;
+  char *b = (char *)opts->workspace;
+  CUDA_TRY(cudaMemcpyAsync(b + L.host_rho, ph->density, 4 * nvox, cudaMemcpyHostToDevice, st));
+  CUDA_TRY(cudaMemcpyAsync(b + L.host_mat, ph->material, nvox, cudaMemcpyHostToDevice, st));
+  phantom_t d = *ph; d.density = (const float *)(b + L.host_rho); d.material = (const uint8_t *)(b + L.host_mat);
+  int rc = run_dose(P, &d, beam, n_histories, seed, batch, (double *)(b + L.host_dose), opts, true);
   if (rc) return rc;
-  CUDA_TRY(cudaMemcpyAsync(dose_out_host, b + o_dose, 8 * nvox, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaMemcpyAsync(dose_out_host, b + L.host_dose, 8 * nvox, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
   return MC_OK;
+}
+
+extern "C" int mc_plan_dose(const psl_t *const *psls, const beam_geom_t *beams, int32_t n_beams, const phantom_t *ph,
+                            uint64_t n_histories, uint64_t seed, uint64_t batch, double *dose_out, const mc_opts_t *opts,
+                            uint64_t *n_beam_out) {
+  static const mc_opts_t kDefaults = {};
+  if (!opts) opts = &kDefaults;
+  if (!psls || !beams || n_beams < 1 || (!dose_out && !opts->dose_acc)) return fail(MC_E_INVALID_ARG, "mc_plan_dose: invalid argument");
+  if (opts->history_begin || opts->history_end || opts->fingerprints || opts->com_index || opts->order != MC_ORDER_SORTED || (opts->flags & MC_FLAG_RANGE))
+    return fail(MC_E_INVALID_ARG, "mc_plan_dose: history ranges, fingerprints, mixed order and the commissioning tally are per-beam options (use mc_dose)");
+  const int world = opts->shard_count > 0 ? opts->shard_count : 1, rank = opts->shard_count > 0 ? opts->shard_index : 0;
+  if (rank < 0 || rank >= world) return fail(MC_E_INVALID_ARG, "mc_plan_dose: shard_index outside [0, shard_count)");
+  for (int i = 0; i < n_beams; ++i) if (int rc = check_common(psls[i], ph, n_histories, batch, opts, "mc_plan_dose")) return rc;
+  std::vector<uint64_t> n(n_beams);
+  if (int rc = mc_plan_allocate(psls, n_beams, n_histories, n.data())) return rc;
+  if (n_beam_out) std::copy(n.begin(), n.end(), n_beam_out);
+  Session S;
+  if (int rc = S.begin(opts->workspace, opts->workspace_bytes, false, *ph, (long long *)opts->dose_acc, *opts, batch, "mc_plan_dose")) return rc;
+  uint64_t n_run = 0;
+  for (int i = 0; i < n_beams; ++i) {
+    // shard `rank` of beam i: the same contiguous split as binding.shard_range (n*r/world in 128-bit: n <= 2^53, world < 2^31)
+    const uint64_t hb = (uint64_t)((unsigned __int128)n[i] * rank / world), he = (uint64_t)((unsigned __int128)n[i] * (rank + 1) / world);
+    if (hb >= he) continue;
+    if (int rc = S.run_beam(psls[i], beams[i], n[i], seed + (uint64_t)i, hb, he, false)) return rc;
+    n_run += he - hb;
+  }
+  return S.end(*ph, dose_out, n_histories, n_run, "mc_plan_dose");
 }
 
 extern "C" int mc_stats(mc_stats_t *out) {
@@ -625,24 +564,21 @@ extern "C" int mc_stats(mc_stats_t *out) {
 // ---------------------------------------------------------------- parity / debug exports
 extern "C" int mc_sample_debug(const psl_t *P, const beam_geom_t *beam, uint64_t first_history, uint64_t count,
                                uint64_t n_histories, uint64_t seed, float *soa_out, void *cuda_stream) {
-  if (!P || !beam || n_histories == 0 || first_history + count > n_histories || count > 0x7fffffffull)
+  if (!P || !beam || n_histories == 0 || n_histories > kMaxHistories || first_history + count > n_histories || count > 0x7fffffffull)
     return fail(MC_E_INVALID_ARG, "mc_sample_debug: invalid argument");
   if (count == 0) return MC_OK;
   if (!soa_out) return fail(MC_E_INVALID_ARG, "mc_sample_debug: soa_out is null");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   std::vector<uint64_t> off(P->groups.size() + 1);
   allocate_host(*P, n_histories, off.data());
-  void *d_off = nullptr;
-  CUDA_TRY(cudaMalloc(&d_off, sizeof(uint64_t) * off.size()));
-  CUDA_TRY(cudaMemcpyAsync(d_off, off.data(), sizeof(uint64_t) * off.size(), cudaMemcpyHostToDevice, st));
   SampleArgs sa{};
-  sa.m = source_model(*P); sa.beam = beam_xf(*beam); sa.off_g = (const unsigned long long *)d_off;
+  sa.m = source_model(*P); sa.beam = beam_xf(*beam);
+  for (size_t i = 0; i < off.size(); ++i) sa.off_g[i] = off[i];
   sa.seed = seed; round_keys(seed, sa.ks); sa.first = first_history; sa.n_total = n_histories; sa.perm_a = 0; sa.count = (unsigned)count;
   sa.p0 = (float4 *)soa_out; sa.p1 = (float4 *)soa_out + count; sa.ctl = nullptr; sa.fp = nullptr; sa.compact = 0;
   k_sample<<<(unsigned)((count + kThreads - 1) / kThreads), kThreads, 0, st>>>(sa);
   CUDA_TRY(cudaGetLastError());
   CUDA_TRY(cudaStreamSynchronize(st));
-  cudaFree(d_off);
   return MC_OK;
 }
 
@@ -652,49 +588,30 @@ extern "C" int mc_transport_debug(const phantom_t *ph, int32_t particle_type, co
     return fail(MC_E_INVALID_ARG, "mc_transport_debug: invalid argument (opts->dose_acc is required)");
   memset(&g_stats, 0, sizeof g_stats);
   if (count == 0) return MC_OK;
-  const size_t nvox = (size_t)ph->nx * ph->ny * ph->nz;
-  const Layout L = make_layout(count, nvox, false);
-  void *ws = opts->workspace;
-  if (ws) { if (opts->workspace_bytes < L.total) return fail(MC_E_WORKSPACE, "mc_transport_debug: workspace too small"); }
-  else { int rc = scratch_get(g_scratch, L.total, &ws); if (rc) return rc; }
-  Run r{};
-  r.st = (cudaStream_t)opts->cuda_stream; r.ws = (char *)ws; r.L = L; r.ctl = (Control *)(r.ws + L.ctl);
-  r.g = make_grid(*ph, (long long *)opts->dose_acc); r.g.vox = (const uint32_t *)(r.ws + L.vox);
-  r.seed = seed; r.n_total = first_history + count; r.perm_a = 0; r.flags = opts->flags; r.batch = count;
-  r.fp = (unsigned long long *)opts->fingerprints; r.fp_base = first_history;
-  r.dbg = true; r.tm.on = false; g_grid_scale = 1.0; r.init_blocks();
-  cudaEvent_t ev0, ev1;
-  CUDA_TRY(cudaEventCreate(&ev0)); CUDA_TRY(cudaEventCreate(&ev1));
-  CUDA_TRY(cudaEventRecord(ev0, r.st));
-  CUDA_TRY(cudaMemsetAsync(r.ctl, 0, sizeof(Control), r.st));
-  k_pack_phantom<<<592, 256, 0, r.st>>>(ph->density, ph->material, nvox, (uint32_t *)(r.ws + r.L.vox), r.ctl);
-  r.build_xs(64.0);                              // debug entry: energies up to 64 MeV
+  Session S;
+  mc_opts_t o = *opts; o.flags |= MC_FLAG_STATS; o.pipelines = 1;
+  S.fp = (unsigned long long *)opts->fingerprints; S.fp_base = first_history;
+  if (int rc = S.begin(opts->workspace, opts->workspace_bytes, false, *ph, (long long *)opts->dose_acc, o, count, "mc_transport_debug")) return rc;
+  Pipe &p = S.pipes[0];
+  // cross-section nodes for energies up to 64 MeV (debug entry: any energy below that), in the workspace
+  const double x0 = std::log2(0.045), hh = (std::log2(64.0 * 1.001) - x0) / kXsIntervals;
+  float *nodes = (float *)(S.ws + S.L.xs);
+  k_build_xs<<<(kXsIntervals + 256) / 256, 256, 0, p.st>>>(nullptr, nodes, x0, hh, kXsIntervals);
+  S.xs.data = nodes; S.xs.x0 = (float)x0; S.xs.inv_h = (float)(1.0 / hh); S.xs.n = kXsIntervals;
   // the caller's planes stand in for the particle buffer; n_pb = count
   const unsigned cnt = (unsigned)count;
-  CUDA_TRY(cudaMemcpyAsync(&r.ctl->n_pb, &cnt, sizeof cnt, cudaMemcpyHostToDevice, r.st));
-  TransportArgs a = r.base_args();
-  a.p0 = (const float4 *)soa_in; a.p1 = (const float4 *)soa_in + count;
+  CUDA_TRY(cudaMemcpyAsync(&p.ctl->n_pb, &cnt, sizeof cnt, cudaMemcpyHostToDevice, p.st));
+  TransportArgs a = S.base_args(p, seed, first_history + count, 0);
+  a.p0 = (const float4 *)soa_in; a.p1 = (const float4 *)soa_in + count; a.p2 = nullptr;
   a.src_kind = SRC_BUFFER; a.buffer_is_debug = 1; a.first = first_history; a.want_type = particle_type;
-  a.src_count = &r.ctl->n_pb; a.src_head = &r.ctl->head_pb;
-  if (particle_type == 0) {
-    r.dbg_p0 = (const float4 *)soa_in; r.dbg_p1 = (const float4 *)soa_in + count;
-    r.transport_photon_debug(first_history, &r.ctl->n_pb);
-  } else {
-    r.electron(a);
-  }
-  k_next_batch<<<1, 1, 0, r.st>>>(r.ctl);
-  CUDA_TRY(cudaEventRecord(ev1, r.st));
-  CUDA_TRY(cudaGetLastError());
-  Control hc;
-  CUDA_TRY(cudaMemcpyAsync(&hc, r.ctl, sizeof(Control), cudaMemcpyDeviceToHost, r.st));
-  CUDA_TRY(cudaStreamSynchronize(r.st));
-  CUDA_TRY(cudaEventElapsedTime(&g_stats.ms_total, ev0, ev1));
-  cudaEventDestroy(ev0); cudaEventDestroy(ev1);
-  fold_stats(hc, r, &g_stats);
-  if (hc.overflow) return fail(MC_E_OVERFLOW, "mc_transport_debug: a secondary queue overflowed");
-  return MC_OK;
+  a.src_count = &p.ctl->n_pb; a.src_head = &p.ctl->head_pb;
+  if (particle_type == 0) { S.launch_photon(p, a); S.drain_electrons(p, a); }
+  else S.launch_electron(p, a);
+  k_next_batch<<<1, 1, 0, p.st>>>(p.ctl);
+  return S.end(*ph, nullptr, 1, 0, "mc_transport_debug");
 }
 
+// (debug probe: allocates its own few KB of device memory - not on the hot path)
 extern "C" int mc_xs_debug(const float rhomax[3], double e_max, const float *E_host, uint64_t n, float *out_host) {
   if (!rhomax || !E_host || !out_host || !(e_max > 0.05) || n > (1ull << 28)) return fail(MC_E_INVALID_ARG, "mc_xs_debug: invalid argument");
   if (n == 0) return MC_OK;
@@ -705,30 +622,13 @@ extern "C" int mc_xs_debug(const float rhomax[3], double e_max, const float *E_h
   for (int k = 0; k < 3; ++k) hc.rhomax[k] = rhomax[k];
   CUDA_TRY(cudaMemcpy(d + o_ctl, &hc, sizeof hc, cudaMemcpyHostToDevice));
   CUDA_TRY(cudaMemcpy(d + o_e, E_host, 4 * n, cudaMemcpyHostToDevice));
-  Run r{}; r.st = nullptr; r.ws = d; r.L.xs = o_xs; r.ctl = (Control *)(d + o_ctl);
-  r.build_xs(e_max);
-  k_xs_debug<<<(unsigned)((n + 255) / 256), 256>>>(r.xs, (const float *)(d + o_e), n, (float *)(d + o_out));
+  const double x0 = std::log2(0.045), hh = (std::log2(e_max * 1.001) - x0) / kXsIntervals;
+  k_build_xs<<<(kXsIntervals + 256) / 256, 256>>>((const Control *)(d + o_ctl), (float *)(d + o_xs), x0, hh, kXsIntervals);
+  XsTable xs{(const float *)(d + o_xs), (float)x0, (float)(1.0 / hh), kXsIntervals};
+  k_xs_debug<<<(unsigned)((n + 255) / 256), 256>>>(xs, (const float *)(d + o_e), n, (float *)(d + o_out));
   CUDA_TRY(cudaGetLastError());
   CUDA_TRY(cudaMemcpy(out_host, d + o_out, 12 * n, cudaMemcpyDeviceToHost));
   cudaFree(d);
-  return MC_OK;
-}
-
-extern "C" int mc_atomic_peak_debug(int64_t *acc, uint64_t nvox, uint64_t n_ops, uint64_t seed, float *ms_out) {
-  if (!acc || !ms_out || nvox == 0 || nvox >= 0x7fffffffull || n_ops == 0) return fail(MC_E_INVALID_ARG, "mc_atomic_peak_debug: invalid argument");
-  int dev = 0, sms = 0; CUDA_TRY(cudaGetDevice(&dev));
-  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  const unsigned blocks = (unsigned)sms * 8, threads = blocks * kThreads;
-  const unsigned per_thread = (unsigned)std::max<uint64_t>(1, n_ops / threads);
-  cudaEvent_t e0, e1; CUDA_TRY(cudaEventCreate(&e0)); CUDA_TRY(cudaEventCreate(&e1));
-  k_atomic_peak<<<blocks, kThreads>>>((unsigned long long *)acc, (unsigned)nvox, 16u, (unsigned)seed);      // warm-up
-  CUDA_TRY(cudaEventRecord(e0));
-  k_atomic_peak<<<blocks, kThreads>>>((unsigned long long *)acc, (unsigned)nvox, per_thread, (unsigned)seed + 1u);
-  CUDA_TRY(cudaEventRecord(e1));
-  CUDA_TRY(cudaEventSynchronize(e1));
-  CUDA_TRY(cudaEventElapsedTime(ms_out, e0, e1));
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
-  ms_out[1] = (float)((double)per_thread * threads);
   return MC_OK;
 }
 

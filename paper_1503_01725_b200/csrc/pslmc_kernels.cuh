@@ -1,5 +1,5 @@
-// pslmc_kernels.cuh — the kernels of the hot path: k_sample (PAPER.md:82-116 S3-S5), k_photon,
-// k_electron (physics DESIGN.md P1-P9), secondary queues, finalise.
+// pslmc_kernels.cuh — k_sample (PAPER.md:82-116 S3-S5: alias pick, position, energy, direction, jaw test, set-up
+// transform, phantom entry, compaction of the survivors), the control block, phantom packing, finalise.
 #pragma once
 #include "pslmc_device.cuh"
 
@@ -11,7 +11,7 @@ constexpr unsigned kFull = 0xffffffffu;
 
 enum Stat {
   ST_MISSED = 0, ST_FLIGHTS, ST_VIRTUAL, ST_COMPTON, ST_PHOTO, ST_PAIR, ST_PCUT, ST_PESC, ST_UNCOLLIDED,
-  ST_SEC_E, ST_SEC_P, ST_ETRACKS, ST_ESTEPS, ST_EESC, ST_DEPOSITS, ST_COUNT
+  ST_SEC_E, ST_SEC_P, ST_ETRACKS, ST_ESTEPS, ST_EESC, ST_DEPOSITS, ST_KAHN, ST_DEFLECT, ST_COUNT
 };
 
 // Device-resident control block.  `batch` part is reset by k_next_batch, the rest once per call.
@@ -19,12 +19,11 @@ struct Control {
   // per batch
   unsigned n_pb, head_pb;          // particle buffer: entries written by k_sample, consume cursor
   unsigned n_eq, head_eq;          // electron queue
-  unsigned pad0;                   // (mixed order: consume cursor of the electron pass over the particle buffer)
-  unsigned pad1, pad2, pad3;
+  unsigned head_pb_e;              // mixed order: consume cursor of the electron pass over the particle buffer
   // per call
-  unsigned overflow;               // a queue was full: result invalid → MC_E_OVERFLOW
+  unsigned overflow;               // bit 0: the electron queue was full; bit 1: a voxel accumulator wrapped → MC_E_OVERFLOW
+  unsigned bad_input;              // mc_transport_debug: a particle with an energy outside [0, 4096) MeV was skipped
   unsigned hw_eq;                  // electron-queue high-water mark
-  unsigned pad4, pad5;
   unsigned long long n_accepted;   // primaries that passed the jaws and entered the phantom
   unsigned long long n_missed;     // primaries that passed the jaws but missed the phantom (k_sample, compact mode)
   unsigned long long ledger[kLedgerSlots][4][2];   // [slot][incident,deposited,escaped,jaw][lo,hi] quanta
@@ -63,7 +62,7 @@ struct BeamXf { float iso[3]; float R[9]; float sad; };
 struct SampleArgs {
   SourceModel m;
   BeamXf beam;
-  const unsigned long long *off_g;   // [G+1] device
+  unsigned long long off_g[160];     // [G+1] prefix offsets of the groups' history-id ranges (Eq. 3; host-computed, G <= 159)
   uint32_t ks[20];                   // Philox round keys of `seed` (host-computed)
   unsigned long long seed, first, n_total, perm_a;   // perm_a != 0 → mixed order: h = (perm_a * t) mod n_total
   unsigned count;
@@ -88,11 +87,11 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
   __shared__ unsigned s_miss[kThreads / 32];
   const SourceModel &m = a.m;
   __shared__ int s_g0;
-  for (int i = threadIdx.x; i <= m.n_groups; i += kThreads) s_off[i] = a.off_g[i];
+  for (int i = threadIdx.x; i <= m.n_groups; i += kThreads) s_off[i] = a.off_g[i];      // (constant bank → shared: the per-thread walk below indexes it divergently)
   // group of h: last g with off[g] <= h (empty groups have off[g] == off[g+1] and are skipped by "last").
   // Sorted order: history ids of a block are consecutive, so one thread searches for the block's first
   // history and the others walk forward from there (usually zero steps).
-  if (threadIdx.x == kThreads - 1 && a.perm_a == 0) {            // (reads the global copy: no barrier before this)
+  if (threadIdx.x == kThreads - 1 && a.perm_a == 0) {            // (reads the parameter copy: no barrier before this)
     const unsigned long long hb = a.first + (unsigned long long)blockIdx.x * kThreads;
     int lo = 0, hi = m.n_groups;
     while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (a.off_g[mid] <= hb) lo = mid; else hi = mid; }
@@ -253,7 +252,7 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
 __global__ void k_next_batch(Control *c) {
   c->n_accepted += c->n_pb;
   c->hw_eq = max(c->hw_eq, c->n_eq);
-  c->n_pb = c->head_pb = c->n_eq = c->head_eq = c->pad0 = 0;
+  c->n_pb = c->head_pb = c->n_eq = c->head_eq = c->head_pb_e = 0;
 }
 
 // Packs the caller's phantom into one 32-bit word per voxel (density rounded to nearest on a 22-bit
@@ -292,16 +291,6 @@ __global__ void k_build_xs(const Control *c, float *data, double x0, double h, i
   data[kXsHead + i] = (float)skn;
 }
 
-// Measurement probe: nothing but int64 scoring atomics on pseudo-random voxels of [0, nvox) - the ceiling the scoring of
-// the transport kernels is compared with.  Each thread issues `per_thread` REDs.
-__global__ void k_atomic_peak(unsigned long long *acc, unsigned nvox, unsigned per_thread, unsigned seed) {
-  unsigned x = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + seed;
-  for (unsigned i = 0; i < per_thread; ++i) {
-    x = x * 1664525u + 1013904223u;
-    atomicAdd(acc + (unsigned)(((unsigned long long)(x ^ (x >> 15)) * nvox) >> 32), 1ull + i);
-  }
-}
-
 // Parity probe: the table lookup k_photon does, for a list of energies.  out: (sigma_KN, ln^2(E/1.022), mu_max) per energy.
 __global__ void k_xs_debug(XsTable xs, const float *E, size_t n, float *out) {
   const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
@@ -311,12 +300,16 @@ __global__ void k_xs_debug(XsTable xs, const float *E, size_t n, float *out) {
   out[3 * i] = skn; out[3 * i + 1] = lp2; out[3 * i + 2] = mu;
 }
 
-// dose[v] = acc[v] 2^-32 / (rho_v V N)
-__global__ void k_finalise(const long long *acc, const float *density, size_t n, double inv_vn, double *dose) {
+// dose[v] = acc[v] 2^-32 / (rho_v V N).  Deposits are never negative, so a negative accumulator has wrapped past
+// 2^63 quanta (2.1e9 MeV in one voxel): flagged, mc_dose then returns MC_E_OVERFLOW.  dose == nullptr: scan only.
+__global__ void k_finalise(const long long *acc, const float *density, size_t n, double inv_vn, double *dose, Control *c) {
+  bool wrapped = false;
   for (size_t v = blockIdx.x * (size_t)blockDim.x + threadIdx.x; v < n; v += (size_t)gridDim.x * blockDim.x) {
-    const float rho = density[v];
-    dose[v] = rho > 0.f ? (double)acc[v] * (1.0 / 4294967296.0) * inv_vn / (double)rho : 0.0;
+    const long long q = acc[v];
+    wrapped |= q < 0;
+    if (dose) { const float rho = density[v]; dose[v] = rho > 0.f ? (double)q * (1.0 / 4294967296.0) * inv_vn / (double)rho : 0.0; }
   }
+  if (wrapped) atomicOr(&c->overflow, 2u);
 }
 
 __global__ void k_philox_debug(unsigned long long seed, unsigned long long h, uint32_t track, uint32_t block, uint32_t *out) {

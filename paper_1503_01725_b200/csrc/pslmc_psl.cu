@@ -171,7 +171,7 @@ void allocate_host(const psl &P, uint64_t N, uint64_t *off) {
   std::vector<size_t> order(G);
   for (size_t g = 0; g < G; ++g) order[g] = g;
   std::stable_sort(order.begin(), order.end(), [&](size_t a, size_t b) { return frac[a] > frac[b]; });
-  const uint64_t rem = N - used;
+  const uint64_t rem = used <= N ? N - used : 0;      // N <= 2^53 (checked by the callers): (double)N is exact and used <= N
   for (uint64_t r = 0; r < rem; ++r) ++n[order[r % G]];
   off[0] = 0;
   for (size_t g = 0; g < G; ++g) off[g + 1] = off[g] + n[g];
@@ -186,6 +186,8 @@ extern "C" int psl_build(const psr_params_t *psr, const jaws_t *jaws, int32_t n_
       psr->n_ring > 65535 || 3 * psr->n_ebin > 159 || !(jaws->x1 < jaws->x2) || !(jaws->y1 < jaws->y2) ||
       !(psr->ring_width > 0) || !(psr->e_bin_width > 0))
     return fail(MC_E_INVALID_ARG, "psl_build: invalid argument");
+  if (!(psr->e_min >= 0) || !(psr->e_min + psr->n_ebin * psr->e_bin_width < 4096.0))     // the exact warp sums of the ledgers hold energies below 4096 MeV
+    return fail(MC_E_INVALID_ARG, "psl_build: energy range must lie in [0, 4096) MeV");
   for (int s = 0; s < 3; ++s)
     if (!(psr->z_phsp > psr->z_src[s]) || !(jaws->z_jx > psr->z_src[s]) || !(jaws->z_jy > psr->z_src[s]) || psr->sigma_src[s] < 0 ||
         (psr->particle_type[s] != 0 && psr->particle_type[s] != 1))
@@ -204,6 +206,8 @@ extern "C" int psl_build_grid(const psr_params_t *psr, const jaws_t *jaws, doubl
       !(jaws->x1 < jaws->x2) || !(jaws->y1 < jaws->y2) || !(psr->ring_width > 0) || !(psr->e_bin_width > 0) || !(let_size > 0) ||
       2.0 * std::ceil(psr->n_ring * psr->ring_width / let_size) > 4096.0)
     return fail(MC_E_INVALID_ARG, "psl_build_grid: invalid argument");
+  if (!(psr->e_min >= 0) || !(psr->e_min + psr->n_ebin * psr->e_bin_width < 4096.0))
+    return fail(MC_E_INVALID_ARG, "psl_build_grid: energy range must lie in [0, 4096) MeV");
   for (int s = 0; s < 3; ++s)
     if (!(psr->z_phsp > psr->z_src[s]) || !(jaws->z_jx > psr->z_src[s]) || !(jaws->z_jy > psr->z_src[s]) || psr->sigma_src[s] < 0 ||
         (psr->particle_type[s] != 0 && psr->particle_type[s] != 1))
@@ -219,6 +223,7 @@ extern "C" int psl_build_grid(const psr_params_t *psr, const jaws_t *jaws, doubl
 
 extern "C" int psl_allocate(const psl_t *P, uint64_t n_histories, uint64_t *off_out) {
   if (!P || !off_out) return fail(MC_E_INVALID_ARG, "psl_allocate: null argument");
+  if (n_histories > (1ull << 53)) return fail(MC_E_INVALID_ARG, "psl_allocate: n_histories above 2^53 (Eq. 3 is evaluated in double)");
   allocate_host(*P, n_histories, off_out);
   return MC_OK;
 }
@@ -227,7 +232,7 @@ extern "C" int psl_allocate(const psl_t *P, uint64_t n_histories, uint64_t *off_
 // beam i gets N * W_i / sum_j W_j histories, W_i = sum of its active group weights, largest-remainder rounding,
 // ties to the lower beam index.
 extern "C" int mc_plan_allocate(const psl_t *const *psls, int32_t n_beams, uint64_t n_histories, uint64_t *n_out) {
-  if (!psls || !n_out || n_beams < 1) return fail(MC_E_INVALID_ARG, "mc_plan_allocate: invalid argument");
+  if (!psls || !n_out || n_beams < 1 || n_histories > (1ull << 53)) return fail(MC_E_INVALID_ARG, "mc_plan_allocate: invalid argument (n_histories <= 2^53)");
   std::vector<double> W(n_beams, 0.0), frac(n_beams);
   double tot = 0;
   for (int i = 0; i < n_beams; ++i) {
@@ -244,7 +249,7 @@ extern "C" int mc_plan_allocate(const psl_t *const *psls, int32_t n_beams, uint6
   std::vector<int> order(n_beams);
   for (int i = 0; i < n_beams; ++i) order[i] = i;
   std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return frac[a] > frac[b]; });
-  const uint64_t rem = n_histories - used;
+  const uint64_t rem = used <= n_histories ? n_histories - used : 0;
   for (uint64_t r = 0; r < rem; ++r) ++n_out[order[r % n_beams]];
   return MC_OK;
 }

@@ -1,5 +1,5 @@
 // pslmc_transport.cuh — k_photon and k_electron: persistent warps with lane refill, Woodcock photon
-// flights with Klein–Nishina/Kahn Compton as a per-lane state machine, condensed-history electrons, a
+// flights with Klein–Nishina/Kahn Compton as a per-lane state machine, condensed-history electrons, the
 // warp-staged electron queue, int64 fixed-point scoring.  PAPER.md:118-120 (iterated kernels), :161 (cut-offs);
 // physics per DESIGN.md P1-P9.
 #pragma once
@@ -113,7 +113,7 @@ struct Pending {
       st.add(g, v, (unsigned long long)q);
       if (COM && g.com_index) {                      // only the stats/fingerprint kernel variants are launched with a tally
         const int row = __ldg(g.com_index + v);
-        if (row > 0) atomicAdd(g.com_dose + (size_t)col * g.com_rows + (row - 1), (unsigned long long)q);
+        if (row > 0 && row <= g.com_rows) atomicAdd(g.com_dose + (size_t)col * g.com_rows + (row - 1), (unsigned long long)q);
       }
     }
     q = 0;
@@ -146,7 +146,7 @@ __device__ __forceinline__ void stage_complete(const Queue &q, Control *ctl, Sta
   const unsigned lane = threadIdx.x & 31u;
   __syncwarp();
   const unsigned base = __shfl_sync(kFull, sc.base_raw, 0);
-  if (base + n_out > q.cap) ctl->overflow = 1u;
+  if (base + n_out > q.cap) atomicOr(&ctl->overflow, 1u);      // dropped whole; k_electron does not run on a queue that overflowed
   else if (lane < n_out) {
     const unsigned p = (sc.head + lane) & 63u;
     __stcs(q.a + base + lane, r.a[p]); __stcs(q.b + base + lane, r.b[p]); __stcs(q.c + base + lane, r.c[p]);   // write-once / read-once: streaming
@@ -228,7 +228,10 @@ __device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned i
     const float4 A = __ldcs(a.p0 + idx), B = __ldcs(a.p1 + idx);
     t.x = A.x; t.y = A.y; t.z = A.z; t.E = A.w; t.u = B.x; t.v = B.y; t.w = B.z;
     unsigned long long tt;
-    if (a.buffer_is_debug) { tt = idx; t.ok = B.w >= 0.0f; }
+    if (a.buffer_is_debug) {
+      tt = idx; t.ok = B.w >= 0.0f;
+      if (t.ok && !(A.w >= 0.0f && A.w < 4096.0f)) { t.ok = false; a.ctl->bad_input = 1u; }     // warp_sum_q is exact below 4096 MeV
+    }
     else { const unsigned bits = __float_as_uint(B.w); tt = bits & 0x7fffffffu; t.ok = (int)(bits >> 31) == a.want_type; }
     t.h = history_of(a.first + tt, a.perm_a, a.n_total);
     t.track = 0u; t.blk = 2u; t.col = a.p2 ? a.p2[idx] : 0u;      // blocks 0, 1 were the source draws
@@ -366,6 +369,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
       uint32_t d0, d1, d2, d3;
       rng.next(a.ks, d0, d1, d2, d3);                    // trial block (r1, r2, r3, azimuth) or pair block (split, cos, azimuth)
       if (state == PH_KAHN) {
+        if (DBG) ++tl.st[ST_KAHN];
         // Kahn's rejection (P5).  With dn = 1 + 2 alpha r2:  branch A: eta = dn, branch B:
         // eta = (2 alpha + 1)/dn.  k = (eta - 1)/alpha is 2 r2 (A) or 2 (1 - r2)/dn (B) in exact
         // arithmetic; these forms have no cancellation in fp32.
@@ -454,6 +458,9 @@ template <bool DBG, bool STAGE>
 __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant__ TransportArgs a) {
   extern __shared__ __align__(16) unsigned char s_raw[];           // [score staging table] when enabled
   const Grid &g = a.g;
+  // a queue that overflowed holds slots that were never written (a reservation that straddled its end is dropped
+  // whole): the call fails with MC_E_OVERFLOW, nothing here may be read
+  if (a.src_kind == SRC_QUEUE && (a.ctl->overflow & 1u)) return;
   ScoreStage<STAGE> stage; stage.init(s_raw);
   const unsigned n1 = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
   const unsigned count = n1;
@@ -531,6 +538,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
         } else if (turn) {
           uint32_t d0, d1, d2, d3;
           rng.next(a.ks, d0, d1, d2, d3);                // deflection block: Gaussian radius, azimuth
+          if (DBG) ++tl.st[ST_DEFLECT];
           // theta = (13.6 / p beta) sqrt(tacc) sqrt(-2 ln a), p beta = Tms (Tms + 2 me)/(Tms + me): one division, one root
           const float c = __fdividef(13.6f * (Tms + kMe), Tms * (Tms + 2.0f * kMe));
           const float th = fminf(kPi, c * sqrt_fast(tacc * (-2.0f * __logf(u_oc(d0)))));

@@ -143,6 +143,16 @@ def test_edge_cases(B, gpsl, cfg):
     with pytest.raises(B.PslmcError) as e:
         g.dose(dph, beam, 1000, 3, batch=1 << 16, workspace=small)
     assert e.value.code == -3
+    # the empty shard [0, 0) is empty, not "everything" (MC_FLAG_RANGE, set by the binding for explicit ranges)
+    acc.zero_()
+    g.dose(dph, beam, 1000, 3, batch=64, dose_acc=acc, history_begin=0, history_end=0)
+    assert int(acc.abs().sum().item()) == 0 and B.stats()["ledger"]["incident"] == 0
+    # no workspace at the C ABI: MC_E_WORKSPACE, nothing is allocated behind the caller's back
+    import ctypes as C
+    o = B.mc_opts_t(); o.cuda_stream = int(torch.cuda.current_stream().cuda_stream)
+    d0 = torch.empty(dph.nvox, dtype=torch.float64, device="cuda")
+    rc = B.lib().mc_dose(g.h, C.byref(dph.c), C.byref(B._beam(beam)), 1000, 3, 64, d0.data_ptr(), C.byref(o))
+    assert rc == -3
     ws = torch.empty(g.workspace_bytes(dph, 1 << 12), dtype=torch.uint8, device="cuda")
     a = g.dose(dph, beam, 20_000, 3, batch=1 << 12, workspace=ws).clone()
     b = g.dose(dph, beam, 20_000, 3, batch=1 << 12)
@@ -152,6 +162,62 @@ def test_edge_cases(B, gpsl, cfg):
     with torch.cuda.stream(s):
         c2 = g.dose(dph, beam, 20_000, 3, batch=1 << 12, stream=s)
     assert torch.equal(a, c2)
+
+
+def test_no_allocation_inside_mc_dose_and_voxel_overflow(B, gpsl, cfg):
+    """no hidden allocation inside mc_dose (free device memory is the same before and after, with the
+    caller's workspace and streams); a voxel accumulator that wraps past 2^63 quanta is reported as MC_E_OVERFLOW."""
+    import torch
+    c = cfg("C0")
+    dph = B.DevicePhantom(c["phantom"])
+    g, beam = gpsl("C0"), c["beams"][0]
+    ws = torch.empty(g.workspace_bytes(dph, 1 << 14), dtype=torch.uint8, device="cuda")
+    acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
+    dose = torch.empty(dph.nvox, dtype=torch.float64, device="cuda")
+    B.aux_streams()
+    g.dose(dph, beam, 50_000, 3, batch=1 << 14, dose_out=dose, dose_acc=acc, workspace=ws)        # module load, first-use costs
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    for pipes in (1, 2):
+        g.dose(dph, beam, 50_000, 3, batch=1 << 14, dose_out=dose, dose_acc=acc, workspace=ws, pipelines=pipes, flags=B.MC_FLAG_TIMING)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free0
+    # overflow: the hottest voxel starts 1000 quanta below 2^63
+    acc.zero_()
+    g.dose(dph, beam, 50_000, 3, batch=1 << 14, dose_acc=acc, workspace=ws)
+    hot = int(acc.argmax().item())
+    acc.zero_(); acc[hot] = (1 << 63) - 1000
+    with pytest.raises(B.PslmcError) as e:
+        g.dose(dph, beam, 50_000, 3, batch=1 << 14, dose_acc=acc, workspace=ws)
+    assert e.value.code == -5 and "wrapped" in str(e.value)
+
+
+def test_two_host_threads_two_handles(B, cfg):
+    """no process-global scratch or streams - two host threads, each with its own psl_t, workspace and streams,
+    run mc_dose at the same time and get the bits of the serial runs."""
+    import threading
+    import torch
+    c = cfg("C0")
+    dph = B.DevicePhantom(c["phantom"])
+    beam = c["beams"][0]
+    ref, out = {}, {}
+    psls = [B.Psl(c["psr"], c["jaws"], c["n_sectors"]) for _ in range(2)]
+    for t, g in enumerate(psls):
+        ref[t] = g.dose(dph, beam, 200_000, 11 + t, batch=1 << 13).clone()
+
+    def work(t):
+        torch.cuda.set_device(0)
+        s = torch.cuda.Stream()
+        aux = (torch.cuda.Stream(), torch.cuda.Stream())
+        ws = torch.empty(psls[t].workspace_bytes(dph, 1 << 13), dtype=torch.uint8, device="cuda")
+        with torch.cuda.stream(s):
+            for _ in range(3):
+                out[t] = psls[t].dose(dph, beam, 200_000, 11 + t, batch=1 << 13, workspace=ws, stream=s, aux=aux).clone()
+        s.synchronize()
+
+    th = [threading.Thread(target=work, args=(t,)) for t in range(2)]
+    [t.start() for t in th]; [t.join() for t in th]
+    assert torch.equal(out[0], ref[0]) and torch.equal(out[1], ref[1])
 
 
 def test_host_entry_point_matches_device_entry_point(B, gpsl, cfg):
@@ -173,7 +239,7 @@ def test_vacuum_and_queue_stats(B, orc, cfg, wl):
     g, o = B.Psl(c["psr"], c["jaws"], 16), orc.Psl(c["psr"], c["jaws"], 16)
     compare_with_oracle(B, orc, g, o, ph, c["beams"][0], 300_000, 8, batch=1 << 16, frac_vox=0.98)
     st = B.stats()
-    assert 0 < st["queue_high_water"][0] < 4 * (1 << 16) and st["launches"]["photon"] > 0
+    assert 0 < st["queue_high_water"] < 4 * (1 << 16) and st["launches"]["photon"] > 0
 
 
 # ---------------------------------------------------------------- plan level (NEXT-4)
@@ -192,10 +258,21 @@ def test_plan_allocation_eq3_and_sharded_plan(B, cfg):
     dph = B.DevicePhantom(c["phantom"])
     g = B.Psl(c["psr"], c["jaws"], c["n_sectors"])
     beams = c["beams"]
-    acc, nb = B.plan_dose([g] * len(beams), dph, beams, 2_100_000, 40, batch=1 << 18)
-    assert nb.tolist() == [300_000] * 7
+    dose = torch.empty(dph.nvox, dtype=torch.float64, device="cuda")
+    acc, nb = B.plan_dose([g] * len(beams), dph, beams, 2_100_000, 40, batch=1 << 18, dose_out=dose)
+    st = B.stats()
+    assert nb.tolist() == [300_000] * 7 and sum(st["n_hist"]) == 2_100_000 and int(acc.sum().item()) == st["ledger"]["deposited"]
     parts = [B.plan_dose([g] * len(beams), dph, beams, 2_100_000, 40, batch=1 << 17, rank=r, world=2)[0] for r in range(2)]
     assert torch.equal(parts[0] + parts[1], acc)
+    # mc_plan_dose = one mc_dose per beam (seed + beam index) into one grid, normalised by the plan's histories
+    acc2 = torch.zeros_like(acc)
+    for i, beam in enumerate(beams):
+        g.dose(dph, beam, 300_000, 40 + i, batch=1 << 16, dose_acc=acc2)
+    assert torch.equal(acc, acc2)
+    rho = torch.as_tensor(np.asarray(c["phantom"]["density"], np.float64)).cuda()
+    V = c["phantom"]["dx"] * c["phantom"]["dy"] * c["phantom"]["dz"]
+    exp = torch.where(rho > 0, acc.double() / 2.0 ** 32 / (torch.clamp(rho, min=1e-30) * V * 2_100_000), torch.zeros_like(rho))
+    assert torch.allclose(dose, exp, rtol=1e-14, atol=0)
     d = acc.cpu().numpy().reshape(120, 256, 256)
     assert d[50:70, 118:138, 118:138].mean() > 5 * d[50:70, :20, :20].mean()
 

@@ -200,33 +200,39 @@ def test_transport_electron_beam(B, orc, wl):
     assert out[1]["n_missed"] == 5 and out[1]["n_electron_tracks"] == n
 
 
-def test_queue_overflow_is_reported_not_corrupting(B, orc, monkeypatch):
+def test_queue_overflow_is_reported_not_corrupting(B, orc):
     """The electron queue holds 4 entries per batch particle: enough for any source this library is for (2.3 per 6 MeV
-    photon in bone, measured; still below 4 at 50 MeV).  With the capacity cut by the test hook PSLMC_TEST_EQ_CAP the call
-    must fail with MC_E_OVERFLOW, write nothing out of bounds, and leave the library usable.  The photon queue (2 per
-    batch particle: a photon converts at most once) cannot overflow."""
+    photon in bone, measured; still below 4 at 50 MeV).  With the capacity cut by the test hook mc_opts_t.debug_eq_cap the
+    call must fail with MC_E_OVERFLOW, write nothing out of bounds, never read a queue slot that was not written (the
+    workspace is filled with NaN bit patterns first: a NaN electron would never stop) and leave the library usable."""
     import torch
     n = 64
     ph = dict(nx=n, ny=n, nz=n, dx=1.0, dy=1.0, dz=1.0, ox=-32.0, oy=-32.0, oz=0.0,
               density=np.full(n ** 3, 1.85, np.float32), material=np.full(n ** 3, 2, np.uint8))
     dph = B.DevicePhantom(ph)
+    ws = torch.empty(int(B.lib().mc_workspace_bytes(None, dph.c, 20000)) + 1024, dtype=torch.uint8, device="cuda")
 
-    def run(E, cnt=20000):
+    def run(E, cnt=20000, **opt):
+        ws.fill_(0xFF)                                        # every float in the scratch reads as NaN
         soa = np.zeros((2, cnt, 4), np.float32); soa[0, :, 2] = 1.0; soa[0, :, 3] = E; soa[1, :, 2] = 1.0
         acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
-        B.transport_debug(dph, 0, torch.as_tensor(soa).cuda(), 0, 5, acc)
+        B.transport_debug(dph, 0, torch.as_tensor(soa).cuda(), 0, 5, acc, workspace=ws, **opt)
+        assert int(ws[-1024:].min().item()) == 0xFF           # nothing written past the layout
         return acc, B.stats()
 
     a0, st0 = run(6.0)
-    assert st0["queue_high_water"][0] < 4 * 20000 and st0["n_pair"] > 0
-    monkeypatch.setenv("PSLMC_TEST_EQ_CAP", "1000")
-    with pytest.raises(B.PslmcError) as e:
-        run(6.0)
-    assert e.value.code == -5
-    monkeypatch.delenv("PSLMC_TEST_EQ_CAP")
-    a1, st1 = run(6.0)                                     # same bits as before the failed call
+    assert st0["queue_high_water"] < 4 * 20000 and st0["n_pair"] > 0
+    for cap in (1000, 1001, 37):                              # a reservation that straddles the end is dropped whole
+        with pytest.raises(B.PslmcError) as e:
+            run(6.0, debug_eq_cap=cap)
+        assert e.value.code == -5
+    a1, st1 = run(6.0)                                     # same bits as before the failed calls
     assert torch.equal(a0, a1) and st0["ledger"] == st1["ledger"]
-    # pair-dominated energies: two photon-queue entries per conversion, never more than 2 per batch particle
+    # pair-dominated energies: the annihilation photons stay in their lane, two per conversion
     a2, st2 = run(50.0, cnt=5000)
-    assert st2["n_pair"] > 2500 and st2["n_sec_photons"] == 2 * st2["n_pair"] and st2["queue_high_water"][1] <= 2 * 5000
-    assert st2["queue_high_water"][0] < 4 * 5000
+    assert st2["n_pair"] > 2500 and st2["n_sec_photons"] == 2 * st2["n_pair"]
+    assert st2["queue_high_water"] < 4 * 5000
+    # energies the exact ledger sums cannot hold are rejected, not mis-added
+    with pytest.raises(B.PslmcError) as e:
+        run(5000.0, cnt=100)
+    assert e.value.code == -1
