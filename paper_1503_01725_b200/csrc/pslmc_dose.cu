@@ -233,6 +233,7 @@ struct Session {
   void drain_electrons(Pipe &p, const TransportArgs &base) {
     TransportArgs c = base;
     c.src_kind = SRC_QUEUE; c.src = c.eq; c.src_count = &p.ctl->n_eq; c.src_head = &p.ctl->head_eq;
+    c.buffer_is_debug = 0;                        // queued secondaries are not incident energy (mc_transport_debug's buffer is)
     launch_electron(p, c);
   }
 
