@@ -91,9 +91,12 @@ typedef struct psl psl_t;          /* opaque: active lets, alias tables, group w
                                    /* (per-CTA table, added to the grid at kernel exit; same bits)  */
 #define MC_FLAG_RANGE          32  /* take [history_begin, history_end) literally: [0, 0) is then   */
                                    /* the EMPTY range (a shard without work) instead of "everything" */
-#define MC_FLAG_NO_TILE_SORT   64  /* ablation: do not order a batch's particles by entry tile      */
-#define MC_FLAG_TILE_SORT     128  /* order every batch by entry tile (default: only when phantom + */
-                                   /* dose grid exceed the L2 budget; PAPER.md:118-120 spatial loop)  */
+#define MC_FLAG_NO_TILE_SORT   64  /* overrides MC_FLAG_TILE_SORT                                   */
+#define MC_FLAG_TILE_SORT     128  /* ablation: order every batch's particles by the tile of the     */
+                                   /* phantom they enter (PAPER.md:118-120 spatial loop); same bits   */
+#define MC_FLAG_FP_VOXELS     256  /* strict fingerprints: also the voxel of every deposit, the stream  */
+                                   /* position after every accepted Kahn sampling and whether an electron */
+                                   /* sub-step ended its condensed step (equal = same draws in the same roles) */
 
 typedef struct {
   void     *workspace;             /* DEVICE scratch, REQUIRED: >= mc_workspace_bytes(psl, ph, batch)  */

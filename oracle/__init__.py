@@ -57,6 +57,7 @@ class _Result(C.Structure):
 
 
 LEDGERS = ("incident", "deposited", "escaped", "jaw")
+FLAG_ELECTRONS_LOCAL, FLAG_TRACE_BIRTH, FLAG_FP_VOXELS = 1, 2, 4      # orc_dose / orc_transport / orc_trace flags
 _lib = None
 
 
@@ -84,6 +85,8 @@ def lib():
         L.orc_sample.argtypes = [C.c_void_p, C.POINTER(_Beam), C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint64, C.c_void_p]
         L.orc_dose.argtypes = [C.c_void_p, C.POINTER(_Phantom), C.POINTER(_Beam), C.c_uint64, C.c_uint64, C.c_uint64,
                                C.c_uint64, C.c_int32, C.c_void_p, C.POINTER(_Result), C.c_void_p]
+        L.orc_dose_list.argtypes = [C.c_void_p, C.POINTER(_Phantom), C.POINTER(_Beam), C.c_uint64, C.c_uint64, C.c_void_p,
+                                    C.c_uint64, C.c_int32, C.c_void_p, C.POINTER(_Result), C.c_void_p]
         L.orc_dose_com.argtypes = [C.c_void_p, C.POINTER(_Phantom), C.POINTER(_Beam), C.c_uint64, C.c_uint64, C.c_uint64,
                                    C.c_uint64, C.c_void_p, C.POINTER(_Result), C.c_void_p, C.c_void_p, C.c_int64]
         L.orc_com_column.restype = C.c_uint32
@@ -203,6 +206,19 @@ class Psl:
         lib().orc_dose(self.h, C.byref(phantom.c), C.byref(_beam(beam)), n_histories, seed, h_begin, h_end, flags,
                        _ptr(acc), C.byref(res), _ptr(fp) if fp is not None else None)
         return acc, _result(res), fp
+
+
+def dose_list(psl: "Psl", phantom: Phantom, beam: dict, n_histories: int, seed: int, ids, flags: int = 0,
+              acc: np.ndarray | None = None, fingerprints: bool = False):
+    """The tally of a list of history ids of an n_histories allocation.  Returns (acc, result dict, fingerprints or None)."""
+    ids = np.ascontiguousarray(ids, np.uint64)
+    if acc is None:
+        acc = np.zeros(phantom.nvox, np.int64)
+    fp = np.zeros(ids.size, np.uint64) if fingerprints else None
+    res = _Result()
+    lib().orc_dose_list(psl.h, C.byref(phantom.c), C.byref(_beam(beam)), n_histories, seed, _ptr(ids), ids.size, flags,
+                        _ptr(acc), C.byref(res), _ptr(fp) if fp is not None else None)
+    return acc, _result(res), fp
 
 
 def dose_com(psl: "Psl", phantom: Phantom, beam: dict, n_histories: int, seed: int, com_index: np.ndarray, n_rows: int,

@@ -61,6 +61,8 @@ const double FIX = 4294967296.0;                          // 2^32 quanta per MeV
 
 const int FLAG_ELECTRONS_LOCAL = 1;
 const int FLAG_TRACE_BIRTH = 2;       // orc_trace only: log a 'B' event (position, direction, energy) when a track starts
+const int FLAG_FP_VOXELS = 4;         // strict fingerprints (F1): also the voxel of every deposit, the stream position after every
+                                      // accepted Kahn sampling (= which trial was accepted) and whether an electron sub-step ended its condensed step
 
 // ---------------------------------------------------------------- R1: Philox4x32-10
 void philox_block(uint64_t seed, uint64_t h, uint32_t track, uint32_t block, uint32_t out[4]) {
@@ -454,6 +456,7 @@ struct Ctx {
   Phantom ph; uint64_t seed; int flags; double fE;
   int64_t *acc; Result *res; i128 ledger[4]; double rhomax[3];
   std::vector<Track> stack; uint64_t fp; std::vector<Event> *trace;
+  Fnv *cur = nullptr;                 // fingerprint of the track being transported (FLAG_FP_VOXELS: deposits hash their voxel into it)
 
   void init(const Phantom &p) {
     ph = p; ledger[0] = ledger[1] = ledger[2] = ledger[3] = 0; trace = nullptr; fE = FE_DEFAULT;
@@ -474,8 +477,9 @@ struct Ctx {
   // Commissioning tally: com_index[v] = 0 (voxel not needed) or 1 + row; com_dose[col * com_rows + row]
   // with col = the PSR unit of the history (all descendants inherit it).
   const int32_t *com_index = nullptr; int64_t *com_dose = nullptr; int64_t com_rows = 0; uint32_t com_col = 0;
-  void deposit(size_t v, double dE) {
+  void deposit(size_t v, double dE, uint32_t tag = 0) {
     int64_t q = quanta(dE); acc[v] += q; ledger[1] += q; ++res->n_deposits;
+    if ((flags & FLAG_FP_VOXELS) && cur) cur->u32((uint32_t)v | tag);
     if (com_index && com_index[v] > 0) com_dose[(size_t)com_col * com_rows + (com_index[v] - 1)] += q;
   }
   void escape(double E) { ledger[2] += quanta(E); }
@@ -509,7 +513,7 @@ struct Ctx {
   }
 
   void photon(Track t) {
-    Fnv f; f.u32(t.track);
+    Fnv f; f.u32(t.track); cur = &f;
     Stream st{seed, t.h, t.track, t.nblk};
     int ijk[3]; bool collided = false;
     if (flags & FLAG_TRACE_BIRTH) ev(t, 'B');
@@ -530,6 +534,7 @@ struct Ctx {
       if (tt < muC) {                                  // Compton, Klein–Nishina by Kahn
         collided = true; ++res->n_compton; f.byte('C');
         uint32_t w_phi; double alpha = t.E / ME, eta = kahn(alpha, st, w_phi, &res->n_kahn_trials);
+        if (flags & FLAG_FP_VOXELS) f.u32(st.j);
         double k = (eta - 1.0) / alpha, ct = 1.0 - k, sn = std::sqrt(std::fmax(0.0, k * (2.0 - k)));
         double phi = 2.0 * PI * U_co(w_phi);
         double Ep = t.E / eta, T = t.E - Ep, d0[3] = {t.dir[0], t.dir[1], t.dir[2]};
@@ -563,7 +568,7 @@ struct Ctx {
   }
 
   void electron(Track t) {
-    Fnv f; f.u32(t.track);
+    Fnv f; f.u32(t.track); cur = &f;
     Stream st{seed, t.h, t.track, t.nblk};
     ++res->n_electron_tracks;
     int ijk[3]; uint32_t steps = 0;
@@ -588,8 +593,9 @@ struct Ctx {
       bool turn = sE <= sv + EPS_B;                       // the sub-step ends the condensed step
       double s = turn ? sE : sv + EPS_B, dT = turn ? budget : D * s;
       ++steps; ++res->n_electron_steps;
-      if (t.E - dT <= ECUT) { deposit(v, t.E); ev(t, 'A', s); f.u32(steps); f.byte('A'); break; }
-      deposit(v, dT);
+      const uint32_t tag = turn ? 0x80000000u : 0u;
+      if (t.E - dT <= ECUT) { deposit(v, t.E, tag); ev(t, 'A', s); f.u32(steps); f.byte('A'); break; }
+      deposit(v, dT, tag);
       for (int a = 0; a < 3; ++a) t.pos[a] += s * t.dir[a];
       t.E -= dT; budget -= dT; tacc += rho * s / X0[m];
       if (!locate(t.pos, ijk)) { escape(t.E); ev(t, 'E', s); ++res->n_electron_escape; f.u32(steps); f.byte('E'); break; }
@@ -660,6 +666,24 @@ void orc_sample(const void *h, const Beam *beam, uint64_t N, uint64_t seed, uint
   }
 }
 
+// One history of an N-history allocation: source sampling, then its whole shower.  Returns the history's fingerprint.
+static uint64_t run_one_history(const Psl &psl, const Beam &beam, const uint64_t *off, uint64_t seed, uint64_t hh, Ctx &c, Result *res) {
+  Sampled s = sample_history(psl, beam, off, seed, hh);
+  int stype = psl.groups[s.group].stype;
+  ++res->n_hist[stype];
+  c.ledger[0] += Ctx::quanta(s.E);
+  c.fp = 0;
+  if (s.rejected) {
+    c.ledger[3] += Ctx::quanta(s.E); ++res->n_jaw_rejected;
+    Fnv f; f.u32(0); f.byte('J'); c.fp += f.v;
+  } else {
+    Track t; t.pos[0] = s.x; t.pos[1] = s.y; t.pos[2] = s.z; t.dir[0] = s.u; t.dir[1] = s.v; t.dir[2] = s.w; t.E = s.E;
+    t.type = psl.p.particle_type[stype]; t.h = hh; t.track = 0; t.nblk = 2; t.nchild = 0;
+    c.stack.push_back(t); c.run_history();
+  }
+  return c.fp;
+}
+
 // Full path for histories [h_begin, h_end) of an N-history allocation.  acc: int64[nvox], ADDED to.
 // fingerprints: u64[h_end-h_begin] or NULL, ADDED to.
 int32_t orc_dose(const void *h, const Phantom *ph, const Beam *beam, uint64_t N, uint64_t seed, uint64_t h_begin,
@@ -669,20 +693,23 @@ int32_t orc_dose(const void *h, const Phantom *ph, const Beam *beam, uint64_t N,
   Ctx c; c.init(*ph); c.seed = seed; c.flags = flags; c.acc = acc; c.res = res;
   std::vector<uint64_t> off(psl.groups.size() + 1); allocate(psl, N, off.data());
   for (uint64_t hh = h_begin; hh < h_end; ++hh) {
-    Sampled s = sample_history(psl, *beam, off.data(), seed, hh);
-    int stype = psl.groups[s.group].stype;
-    ++res->n_hist[stype];
-    c.ledger[0] += Ctx::quanta(s.E);
-    c.fp = 0;
-    if (s.rejected) {
-      c.ledger[3] += Ctx::quanta(s.E); ++res->n_jaw_rejected;
-      Fnv f; f.u32(0); f.byte('J'); c.fp += f.v;
-    } else {
-      Track t; t.pos[0] = s.x; t.pos[1] = s.y; t.pos[2] = s.z; t.dir[0] = s.u; t.dir[1] = s.v; t.dir[2] = s.w; t.E = s.E;
-      t.type = psl.p.particle_type[stype]; t.h = hh; t.track = 0; t.nblk = 2; t.nchild = 0;
-      c.stack.push_back(t); c.run_history();
-    }
-    if (fingerprints) fingerprints[hh - h_begin] += c.fp;
+    uint64_t fp = run_one_history(psl, *beam, off.data(), seed, hh, c, res);
+    if (fingerprints) fingerprints[hh - h_begin] += fp;
+  }
+  c.store_ledgers();
+  return 0;
+}
+
+// The same for a LIST of history ids (tests: the tally of a chosen set of histories).  fingerprints: u64[count] or NULL.
+int32_t orc_dose_list(const void *h, const Phantom *ph, const Beam *beam, uint64_t N, uint64_t seed, const uint64_t *ids,
+                      uint64_t count, int32_t flags, int64_t *acc, Result *res, uint64_t *fingerprints) {
+  const Psl &psl = *(const Psl *)h;
+  std::memset(res, 0, sizeof(Result));
+  Ctx c; c.init(*ph); c.seed = seed; c.flags = flags; c.acc = acc; c.res = res;
+  std::vector<uint64_t> off(psl.groups.size() + 1); allocate(psl, N, off.data());
+  for (uint64_t i = 0; i < count; ++i) {
+    uint64_t fp = run_one_history(psl, *beam, off.data(), seed, ids[i], c, res);
+    if (fingerprints) fingerprints[i] += fp;
   }
   c.store_ledgers();
   return 0;

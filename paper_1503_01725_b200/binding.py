@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libpslmc.so")
 
 MC_ORDER_SORTED, MC_ORDER_MIXED = 0, 1
 MC_FLAG_ELECTRONS_LOCAL, MC_FLAG_STATS, MC_FLAG_TIMING, MC_FLAG_STATIC_LANES, MC_FLAG_STAGE_SCORING = 1, 2, 4, 8, 16
-MC_FLAG_RANGE, MC_FLAG_NO_TILE_SORT, MC_FLAG_TILE_SORT = 32, 64, 128
+MC_FLAG_RANGE, MC_FLAG_NO_TILE_SORT, MC_FLAG_TILE_SORT, MC_FLAG_FP_VOXELS = 32, 64, 128, 256
 LEDGERS = ("incident", "deposited", "escaped", "jaw")
 KERNEL_CLASSES = ("sample", "photon", "electron", "finalise", "aux")
 EXPORTS = ("psl_build", "psl_build_grid", "psl_set_direction_model", "mc_plan_allocate", "mc_plan_dose", "psl_free", "psl_export", "psl_allocate",

@@ -82,6 +82,11 @@ struct Grid {
   const uint8_t *material;
   const uint32_t *vox;                               // packed phantom, one gather per voxel: density bits rounded to a
                                                      // 22-bit mantissa | material index in the two low bits
+  // Two-level phantom: one word per brick of 4x4x4 voxels = the brick's common voxel word | 0x80000000 when all its
+  // voxels are equal (densities are >= 0, so bit 31 of a voxel word is free), else 0.  A phantom that is mostly
+  // uniform bricks (water tanks, slabs: n_uniform >= 90 % of the bricks, decided per call on the device) is then read
+  // through this table, which stays in L1/L2, and only the mixed bricks go to the 4-byte-per-voxel array.
+  const uint32_t *brick; const unsigned *n_uniform; int nbx, nby; unsigned nbricks;
   unsigned long long *acc;                           // int64 fixed-point dose accumulator (2^-32 MeV)
   // commissioning tally, off when com_index is null: com_index[v] = 0 or 1 + row,
   // com_dose[col * com_rows + row], col = the PSR unit the history was sampled from
@@ -96,8 +101,11 @@ __device__ __forceinline__ bool locate(const Grid &g, float x, float y, float z,
   i = (int)fi; j = (int)fj; k = (int)fk;
   return in;
 }
-__device__ __forceinline__ void fetch_voxel(const Grid &g, int v, float &rho, int &mt) {
-  const uint32_t p = __ldg(g.vox + v);
+__device__ __forceinline__ bool use_bricks(const Grid &g) { return g.brick != nullptr && *g.n_uniform * 10ull >= g.nbricks * 9ull; }
+__device__ __forceinline__ void fetch_voxel(const Grid &g, bool bricks, int i, int j, int k, int v, float &rho, int &mt) {
+  uint32_t p = 0u;
+  if (bricks) p = __ldg(g.brick + ((i >> 2) + g.nbx * ((j >> 2) + g.nby * (k >> 2))));
+  if (p & 0x80000000u) p &= 0x7fffffffu; else p = __ldg(g.vox + v);
   rho = __uint_as_float(p & ~3u); mt = (int)(p & 3u);
 }
 __device__ __forceinline__ int vox_index(const Grid &g, int i, int j, int k) { return (k * g.ny + j) * g.nx + i; }

@@ -29,22 +29,27 @@ static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 // Workspace layout for a batch of B primaries.  Shared by the whole call: control blocks, cross-section
 // data, packed phantom, the int64 dose grid (used when the caller gives no dose_acc).  Per pipeline
-// (kMaxPipes of them, see Session): the particle buffer (2 planes + the commissioning column) and the electron
-// queue (capacity 4B, 3 planes).  mc_dose_host appends its staging area (phantom in, dose out).
+// (kMaxPipes of them, see Session): the particle buffer (2 planes + the commissioning column) twice - as packed by
+// k_sample and ordered by entry tile -, the entry-tile counters, and the electron queue (capacity 4B, 3 planes).  mc_dose_host appends its staging area (phantom in, dose out).
 constexpr int kMaxPipes = 2;
 struct Layout {
-  size_t ctl[kMaxPipes], xs, vox, acc, p0[kMaxPipes], p1[kMaxPipes], p2[kMaxPipes], eq[kMaxPipes][3], total;
+  size_t ctl[kMaxPipes], tile[kMaxPipes], xs, vox, brick, acc, p0[kMaxPipes], p1[kMaxPipes], p2[kMaxPipes], q0[kMaxPipes], q1[kMaxPipes], q2[kMaxPipes],
+      eq[kMaxPipes][3], total, zero_bytes;
   size_t host_rho, host_mat, host_dose, host_total;
   unsigned eq_cap;
 };
-static Layout make_layout(uint64_t batch, size_t nvox) {
+static size_t brick_count(int nx, int ny, int nz) { return (size_t)((nx + 3) / 4) * ((ny + 3) / 4) * ((nz + 3) / 4); }
+static Layout make_layout(uint64_t batch, size_t nvox, size_t nbricks) {
   Layout L{}; size_t o = 0;
   auto take = [&](size_t b) { size_t at = o; o += align_up(b); return at; };
   L.eq_cap = (unsigned)std::min<uint64_t>(4 * batch, 0x7fffffffu);
-  for (int p = 0; p < kMaxPipes; ++p) L.ctl[p] = take(sizeof(Control));     // contiguous from offset 0: zeroed by one memset
-  L.xs = take(kXsBytes); L.vox = take(4 * nvox); L.acc = take(8 * nvox);
+  for (int p = 0; p < kMaxPipes; ++p) L.ctl[p] = take(sizeof(Control));     // contiguous from offset 0: zeroed by one memset,
+  for (int p = 0; p < kMaxPipes; ++p) L.tile[p] = take(2 * sizeof(unsigned) * kTileBinsMax);   // with the entry-tile counts and cursors
+  L.zero_bytes = o;
+  L.xs = take(kXsBytes); L.vox = take(4 * nvox); L.brick = take(4 * nbricks); L.acc = take(8 * nvox);
   for (int p = 0; p < kMaxPipes; ++p) {
     L.p0[p] = take(16 * batch); L.p1[p] = take(16 * batch); L.p2[p] = take(4 * batch);
+    L.q0[p] = take(16 * batch); L.q1[p] = take(16 * batch); L.q2[p] = take(4 * batch);     // the same, ordered by entry tile
     for (int k = 0; k < 3; ++k) L.eq[p][k] = take((size_t)16 * L.eq_cap);
   }
   L.total = o;
@@ -160,7 +165,9 @@ struct Timer {                                  // per-kernel-class CUDA-event t
 // One launch sequence ("pipeline"): its stream, control block, particle buffer and electron queue.
 struct Pipe {
   cudaStream_t st = nullptr; Control *ctl = nullptr;
-  float4 *p0 = nullptr, *p1 = nullptr; uint32_t *p2 = nullptr;
+  float4 *p0 = nullptr, *p1 = nullptr; uint32_t *p2 = nullptr;      // packed by k_sample
+  float4 *q0 = nullptr, *q1 = nullptr; uint32_t *q2 = nullptr;      // ordered by entry tile (what the transport kernels read when tiles are on)
+  unsigned *tile_count = nullptr, *tile_cursor = nullptr;
   Queue eq{};
   Timer tm; uint64_t launches[5] = {0, 0, 0, 0, 0};
   bool started = false;                         // a batch has been launched on this pipeline
@@ -176,7 +183,8 @@ struct Session {
   int flags = 0; bool dbg = false, timing = false;
   unsigned eq_cap = 0; uint64_t batch = 0;
   XsTable xs{}; const float *rhomax = nullptr;
-  int blocks_photon = 1, blocks_electron = 1;
+  int blocks_photon = 1, blocks_electron = 1, sms = 1;
+  TileMap tm{};                                 // nbins = 0: batches are not ordered by entry tile
   uint64_t task = 0;                            // batches dealt so far (round-robin over the pipelines)
   cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev_fork = nullptr, ev_join[kMaxPipes] = {};
   Timer tm_us; uint64_t launches_us[5] = {0, 0, 0, 0, 0};
@@ -221,12 +229,14 @@ struct Session {
     TransportArgs a{};
     a.g = g; a.ctl = p.ctl; a.seed = seed; a.n_total = n_total; a.perm_a = perm_a;
     round_keys(seed, a.ks);
-    a.p0 = p.p0; a.p1 = p.p1; a.p2 = g.com_index ? p.p2 : nullptr;
+    const bool tiles = tm.nbins > 0;
+    a.p0 = tiles ? p.q0 : p.p0; a.p1 = tiles ? p.q1 : p.p1; a.p2 = g.com_index ? (tiles ? p.q2 : p.p2) : nullptr;
     a.eq = p.eq;
     a.fp = fp; a.fp_base = fp_base;
     a.electrons_local = (flags & MC_FLAG_ELECTRONS_LOCAL) ? 1 : 0;
     a.static_lanes = (flags & MC_FLAG_STATIC_LANES) ? 1 : 0;
     a.stage_scoring = (flags & MC_FLAG_STAGE_SCORING) ? 1 : 0;
+    a.fp_voxels = (flags & MC_FLAG_FP_VOXELS) ? 1 : 0;
     a.xs = xs; a.rhomax = rhomax;
     return a;
   }
@@ -241,7 +251,7 @@ struct Session {
   int begin(void *workspace, size_t workspace_bytes, bool host_staging, const phantom_t &ph, long long *dose_acc, const mc_opts_t &o,
             uint64_t batch_, const char *who) {
     nvox = (size_t)ph.nx * ph.ny * ph.nz; batch = batch_;
-    L = make_layout(batch, nvox);
+    L = make_layout(batch, nvox, brick_count(ph.nx, ph.ny, ph.nz));
     if (!workspace || workspace_bytes < (host_staging ? L.host_total : L.total)) {
       char b[160]; snprintf(b, sizeof b, "%s: workspace missing or too small (see mc_workspace_bytes)", who);
       return fail(MC_E_WORKSPACE, b);
@@ -257,27 +267,44 @@ struct Session {
       return fail(MC_E_INVALID_ARG, "aux_streams must be distinct from each other and from cuda_stream");
     long long *acc = dose_acc ? dose_acc : (long long *)(ws + L.acc);
     g = make_grid(ph, acc); g.vox = (const uint32_t *)(ws + L.vox);
+    g.nbx = (ph.nx + 3) / 4; g.nby = (ph.ny + 3) / 4; g.nbricks = (unsigned)((size_t)g.nbx * g.nby * ((ph.nz + 3) / 4));
+    g.brick = (const uint32_t *)(ws + L.brick); g.n_uniform = &((Control *)(ws + L.ctl[0]))->n_uniform_bricks;
     g.com_index = (const int *)o.com_index; g.com_dose = (unsigned long long *)o.com_dose; g.com_rows = o.com_rows;
     for (int p = 0; p < npipe; ++p) {
       Pipe &q = pipes[p];
       q.st = npipe > 1 ? (cudaStream_t)o.aux_streams[p] : us; q.ctl = (Control *)(ws + L.ctl[p]);
       q.p0 = (float4 *)(ws + L.p0[p]); q.p1 = (float4 *)(ws + L.p1[p]); q.p2 = (uint32_t *)(ws + L.p2[p]);
+      q.q0 = (float4 *)(ws + L.q0[p]); q.q1 = (float4 *)(ws + L.q1[p]); q.q2 = (uint32_t *)(ws + L.q2[p]);
+      q.tile_count = (unsigned *)(ws + L.tile[p]); q.tile_cursor = q.tile_count + kTileBinsMax;
       q.eq.a = (float4 *)(ws + L.eq[p][0]); q.eq.b = (float4 *)(ws + L.eq[p][1]); q.eq.c = (uint4 *)(ws + L.eq[p][2]);
       q.eq.count = &q.ctl->n_eq; q.eq.cap = eq_cap;
       q.tm.on = timing; q.tm.st = q.st;
     }
     // When the packed phantom + int64 grid (12 B per voxel) do not fit L2 the kernels are bound by random DRAM sectors and
     // fewer resident warps thrash less: measured on C4 (201 MB) 56.8 ms per 1e8 histories at 1.0, 53.1 at 0.75.
-    init_blocks(12.0 * (double)nvox > 110e6 ? 0.75 : 1.0);
+    const bool big = 12.0 * (double)nvox > 110e6;
+    init_blocks(big ? 0.75 : 1.0);
+    { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+    // Entry-tile ordering of every batch (the spatial inner loop): MC_FLAG_TILE_SORT.  Off by default:
+    // measured on C4 it takes 10 % off the transport kernels' time and costs as much in the sort - photons
+    // scatter 10-20 cm away from their entry tile.  Cubic tiles of 2^shift voxels, at most kTileBinsMax bins.
+    tm = TileMap{};
+    if ((o.flags & MC_FLAG_TILE_SORT) && !(o.flags & MC_FLAG_NO_TILE_SORT)) {
+      int sh = 3;
+      auto nt = [&](int n) { return ((n - 1) >> sh) + 1; };
+      while ((long long)nt(ph.nx) * nt(ph.ny) * nt(ph.nz) > kTileBinsMax) ++sh;
+      tm.shift = sh; tm.ntx = nt(ph.nx); tm.nty = nt(ph.ny); tm.nbins = tm.ntx * tm.nty * nt(ph.nz);
+    }
     rhomax = pipes[0].ctl->rhomax;
     CUDA_TRY(cudaEventCreate(&ev0)); CUDA_TRY(cudaEventCreate(&ev1));
     CUDA_TRY(cudaEventRecord(ev0, us));
-    CUDA_TRY(cudaMemsetAsync(ws, 0, L.ctl[kMaxPipes - 1] + align_up(sizeof(Control)), us));          // every pipeline's control block
+    CUDA_TRY(cudaMemsetAsync(ws, 0, L.zero_bytes, us));          // every pipeline's control block and entry-tile counters
     if (!dose_acc) CUDA_TRY(cudaMemsetAsync(acc, 0, 8 * nvox, us));
     tm_us.on = timing; tm_us.st = us;
     tm_us.begin(MC_K_AUX);
     k_pack_phantom<<<592, 256, 0, us>>>(ph.density, ph.material, nvox, (uint32_t *)(ws + L.vox), pipes[0].ctl);
-    tm_us.end(MC_K_AUX); ++launches_us[MC_K_AUX];
+    k_bricks<<<(g.nbricks + 255) / 256, 256, 0, us>>>(g.vox, g.nx, g.ny, g.nz, g.nbx, g.nby, g.nbricks, (uint32_t *)(ws + L.brick), pipes[0].ctl);
+    tm_us.end(MC_K_AUX); launches_us[MC_K_AUX] += 2;
     if (npipe > 1) {
       CUDA_TRY(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
       CUDA_TRY(cudaEventRecord(ev_fork, us));
@@ -302,8 +329,19 @@ struct Session {
       p.started = true;                                   // (a pipeline's first batch finds the control block freshly zeroed)
       sa.first = first; sa.count = (unsigned)count; sa.p0 = p.p0; sa.p1 = p.p1; sa.ctl = p.ctl;
       sa.p2 = g.com_index ? p.p2 : nullptr;
+      sa.tm = tm; sa.tile_count = tm.nbins ? p.tile_count : nullptr;
       p.tm.begin(MC_K_SAMPLE);
-      k_sample<<<(unsigned)((count + kThreads - 1) / kThreads), kThreads, 0, p.st>>>(sa);
+      const unsigned nblk = (unsigned)std::min<uint64_t>((count + kThreads - 1) / kThreads, (uint64_t)sms * 8);      // persistent: 8 CTAs of 256 per SM
+      k_sample<<<nblk, kThreads, sizeof(unsigned) * tm.nbins, p.st>>>(sa);
+      if (tm.nbins) {                                     // counting sort of the survivors by entry tile: counts -> cursors -> moves
+        k_tile_scan<<<1, 1024, 0, p.st>>>(p.tile_count, p.tile_cursor, tm.nbins);
+        ScatterArgs sc{};
+        sc.g = g; sc.tm = tm; sc.p0 = p.p0; sc.p1 = p.p1; sc.p2 = sa.p2; sc.q0 = p.q0; sc.q1 = p.q1; sc.q2 = p.q2;
+        sc.n_pb = &p.ctl->n_pb; sc.cursor = p.tile_cursor;
+        const unsigned nsc = (unsigned)std::min<uint64_t>((count + kTileChunk - 1) / kTileChunk, (uint64_t)sms * 4);
+        k_tile_scatter<<<nsc, kThreads, 2 * sizeof(unsigned) * tm.nbins, p.st>>>(sc);
+        p.launches[MC_K_SAMPLE] += 2;
+      }
       p.tm.end(MC_K_SAMPLE); ++p.launches[MC_K_SAMPLE];
     };
     auto photon_batch = [&](Pipe &p, uint64_t first) {   // the photons of the particle buffer, then every electron they queued
@@ -498,11 +536,11 @@ extern "C" int psl_set_direction_model(psl_t *P, int32_t stype, int32_t K, const
 
 extern "C" size_t mc_workspace_bytes(const psl_t *, const phantom_t *ph, uint64_t batch) {
   if (!ph || ph->nx <= 0 || ph->ny <= 0 || ph->nz <= 0 || batch == 0 || batch > (1ull << 30)) return 0;
-  return make_layout(batch, (size_t)ph->nx * ph->ny * ph->nz).total;
+  return make_layout(batch, (size_t)ph->nx * ph->ny * ph->nz, brick_count(ph->nx, ph->ny, ph->nz)).total;
 }
 extern "C" size_t mc_host_workspace_bytes(const psl_t *, const phantom_t *ph, uint64_t batch) {
   if (!ph || ph->nx <= 0 || ph->ny <= 0 || ph->nz <= 0 || batch == 0 || batch > (1ull << 30)) return 0;
-  return make_layout(batch, (size_t)ph->nx * ph->ny * ph->nz).host_total;
+  return make_layout(batch, (size_t)ph->nx * ph->ny * ph->nz, brick_count(ph->nx, ph->ny, ph->nz)).host_total;
 }
 
 extern "C" int mc_dose(const psl_t *P, const phantom_t *ph, const beam_geom_t *beam, uint64_t n_histories, uint64_t seed,
@@ -515,7 +553,7 @@ extern "C" int mc_dose_host(const psl_t *P, const phantom_t *ph, const beam_geom
   if (!ph || ph->nx <= 0 || ph->ny <= 0 || ph->nz <= 0 || !ph->density || !ph->material || !dose_out_host || !opts || batch == 0 || batch > (1ull << 30))
     return fail(MC_E_INVALID_ARG, "mc_dose_host: invalid argument (opts with a workspace is required)");
   const size_t nvox = (size_t)ph->nx * ph->ny * ph->nz;
-  const Layout L = make_layout(batch, nvox);
+  const Layout L = make_layout(batch, nvox, brick_count(ph->nx, ph->ny, ph->nz));
   if (!opts->workspace || opts->workspace_bytes < L.host_total) return fail(MC_E_WORKSPACE, "mc_dose_host: workspace missing or too small (see mc_host_workspace_bytes)");
   cudaStream_t st = (cudaStream_t)opts->cuda_stream;
   char *b = (char *)opts->workspace;
@@ -577,7 +615,8 @@ extern "C" int mc_sample_debug(const psl_t *P, const beam_geom_t *beam, uint64_t
   for (size_t i = 0; i < off.size(); ++i) sa.off_g[i] = off[i];
   sa.seed = seed; round_keys(seed, sa.ks); sa.first = first_history; sa.n_total = n_histories; sa.perm_a = 0; sa.count = (unsigned)count;
   sa.p0 = (float4 *)soa_out; sa.p1 = (float4 *)soa_out + count; sa.ctl = nullptr; sa.fp = nullptr; sa.compact = 0;
-  k_sample<<<(unsigned)((count + kThreads - 1) / kThreads), kThreads, 0, st>>>(sa);
+  int sms = 1; cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P->device);
+  k_sample<<<(unsigned)std::min<uint64_t>((count + kThreads - 1) / kThreads, (uint64_t)sms * 8), kThreads, 0, st>>>(sa);
   CUDA_TRY(cudaGetLastError());
   CUDA_TRY(cudaStreamSynchronize(st));
   return MC_OK;

@@ -29,6 +29,7 @@ struct Control {
   unsigned long long ledger[kLedgerSlots][4][2];   // [slot][incident,deposited,escaped,jaw][lo,hi] quanta
   unsigned long long stat[ST_COUNT];
   float rhomax[4];                 // largest density per material (as float, written via atomicMax on bits)
+  unsigned n_uniform_bricks;       // bricks of 4x4x4 voxels whose voxels are all equal (k_bricks; two-level phantom)
 };
 
 // One alias-table entry, 16 B: everything k_sample needs after picking a column.
@@ -58,6 +59,7 @@ struct SourceModel {               // read-only, uploaded once by psl_build
 };
 
 struct BeamXf { float iso[3]; float R[9]; float sad; };
+struct TileMap { int shift, ntx, nty, nbins; };      // entry tiles (below); nbins = 0: no ordering
 
 struct SampleArgs {
   SourceModel m;
@@ -74,42 +76,56 @@ struct SampleArgs {
   int compact;                       // 1: survivors packed, p1.w = local index bits; 0: indexed by t, p1.w = status
   Grid g;                            // compact mode: survivors are moved to their phantom entry point here (P4),
   int stats;                         //   with every lane of the warp busy, instead of in the transport kernels' refill
+  TileMap tm; unsigned *tile_count;  // compact mode, tile ordering: entry-tile histogram of the batch (device), or null
 };
 
 __device__ __forceinline__ unsigned long long history_of(unsigned long long t, unsigned long long perm_a, unsigned long long n_total) {
   return perm_a ? (perm_a * t) % n_total : t;
 }
 
+// ------------------------------------------------------------------ entry tiles (the spatial inner loop)
+// A batch's survivors can be ordered by the tile of the phantom their entry voxel lies in, so that the lanes resident at
+// any time work under a few neighbouring tiles and their voxel gathers and scoring atomics stay in L2.
+// Tiles are cubes of 2^shift voxels; bins run in snake order (x reversed on odd rows, y reversed on odd slabs) so that
+// consecutive bins are always face neighbours.  Counting sort: k_sample counts, k_tile_scan turns counts into
+// cursors, k_tile_scatter moves the particles.  The order inside a bin is arbitrary: results do not depend on it.
+constexpr int kTileBinsMax = 4096;
+__device__ __forceinline__ unsigned tile_bin(const TileMap &tm, int vi, int vj, int vk) {
+  int tx = vi >> tm.shift, ty = vj >> tm.shift; const int tz = vk >> tm.shift;
+  if (tz & 1) ty = tm.nty - 1 - ty;
+  const int row = ty + tm.nty * tz;
+  if (row & 1) tx = tm.ntx - 1 - tx;
+  return (unsigned)(tx + tm.ntx * row);
+}
+
 // ------------------------------------------------------------------ k_sample
+// Persistent grid: a thread samples histories t = blockIdx.x*kThreads + threadIdx.x + i*gridDim.x*kThreads.  The
+// (sub-source, energy bin) group of a history is found once per thread and then walked forward (sorted order:
+// history ids only grow), ledgers are summed in registers and flushed once per warp at the end: no barrier in the loop.
 __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ SampleArgs a) {
   __shared__ unsigned long long s_off[160];
-  __shared__ unsigned long long s_led[kThreads / 32][3];
-  __shared__ unsigned s_miss[kThreads / 32];
+  extern __shared__ unsigned s_hist[];                     // [tm.nbins] entry-tile histogram of this CTA (tile ordering only)
   const SourceModel &m = a.m;
-  __shared__ int s_g0;
-  for (int i = threadIdx.x; i <= m.n_groups; i += kThreads) s_off[i] = a.off_g[i];      // (constant bank → shared: the per-thread walk below indexes it divergently)
-  // group of h: last g with off[g] <= h (empty groups have off[g] == off[g+1] and are skipped by "last").
-  // Sorted order: history ids of a block are consecutive, so one thread searches for the block's first
-  // history and the others walk forward from there (usually zero steps).
-  if (threadIdx.x == kThreads - 1 && a.perm_a == 0) {            // (reads the parameter copy: no barrier before this)
-    const unsigned long long hb = a.first + (unsigned long long)blockIdx.x * kThreads;
-    int lo = 0, hi = m.n_groups;
-    while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (a.off_g[mid] <= hb) lo = mid; else hi = mid; }
-    s_g0 = lo;
-  }
+  for (int i = threadIdx.x; i <= m.n_groups; i += kThreads) s_off[i] = a.off_g[i];      // (constant bank → shared: indexed divergently below)
+  const bool tiles = a.tm.nbins > 0 && a.tile_count != nullptr;
+  if (tiles) for (int i = threadIdx.x; i < a.tm.nbins; i += kThreads) s_hist[i] = 0u;
   __syncthreads();
-  const unsigned t = blockIdx.x * kThreads + threadIdx.x;
   const unsigned lane = threadIdx.x & 31u;
-  const bool live = t < a.count;
   unsigned long long q_inc = 0, q_jaw = 0, q_esc = 0;
-  bool pass = false, missed = false;
+  unsigned n_miss = 0;
+  int g = -1;                                              // group of the thread's previous history (sorted order)
+  for (unsigned t0 = blockIdx.x * kThreads; t0 < a.count; t0 += gridDim.x * kThreads) {
+  const unsigned t = t0 + threadIdx.x;
+  const bool live = t < a.count;
+  bool pass = false;
   float4 o0 = make_float4(0.f, 0.f, 0.f, 0.f), o1 = o0;
-  int g = 0, ptype = 0;
+  int ptype = 0;
+  unsigned bin = 0u;
   uint32_t com_col = 0u;
   if (live) {
     const unsigned long long h = history_of(a.first + t, a.perm_a, a.n_total);
-    if (a.perm_a == 0) {
-      g = s_g0;
+    // group of h: last g with off[g] <= h (empty groups have off[g] == off[g+1] and are skipped by "last")
+    if (a.perm_a == 0 && g >= 0) {
       while (g + 1 < m.n_groups && s_off[g + 1] <= h) ++g;
     } else {
       int lo = 0, hi = m.n_groups;         // invariant: off[lo] <= h < off[hi]
@@ -154,10 +170,10 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
       // ring of the position: for sector lets it is the let's own ring (an integer: no fp32 floor decision)
       const int i = m.let_mode == 0 ? (int)ring : min((int)(r / m.ring_width), m.n_ring - 1);
       const float4 *tab = m.dir_tab[stype] + ((size_t)ebin * m.n_ring + i) * K;
-      const float t = u_co(y0);
+      const float tq = u_co(y0);
       int k = 0;
       float4 c = __ldg(tab);
-      while (k < K - 1 && t >= c.x) { ++k; c = __ldg(tab + k); }              // sequential search of P_{i,k}
+      while (k < K - 1 && tq >= c.x) { ++k; c = __ldg(tab + k); }             // sequential search of P_{i,k}
       const float rho_n = sqrtf(-2.0f * logf(u_oc(y1)));
       sincospif(2.0f * u_co(y2), &sn, &cs);
       const float alpha = fminf(1.5f, fmaxf(-1.5f, __fmaf_rn(c.z * rho_n, cs, c.y)));
@@ -194,9 +210,10 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
     o1.x = __fmaf_rn(R[0], dx, __fmaf_rn(R[1], dy, R[2] * dz));
     o1.y = __fmaf_rn(R[3], dx, __fmaf_rn(R[4], dy, R[5] * dz));
     o1.z = __fmaf_rn(R[6], dx, __fmaf_rn(R[7], dy, R[8] * dz));
-    q_inc = (unsigned long long)quanta(E);
+    const unsigned long long qE = (unsigned long long)quanta(E);
+    q_inc += qE;
     if (!pass) {
-      q_jaw = q_inc;
+      q_jaw += qE;
       if (a.fp) {
         Fnv f; f.init(0u); f.byte('J');
         atomicAdd(a.fp + (h - a.fp_base), f.v);
@@ -205,14 +222,14 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
       // P4 entry: a particle that starts outside the grid is moved to its entry point (+ eps); a miss ends here
       int vi, vj, vk;
       if (!locate(a.g, o0.x, o0.y, o0.z, vi, vj, vk) && !enter(a.g, o0.x, o0.y, o0.z, o1.x, o1.y, o1.z, vi, vj, vk)) {
-        missed = true; pass = false; q_esc = q_inc;
+        ++n_miss; pass = false; q_esc += qE;
         if (a.fp) {
           Fnv f; f.init(0u);
           if (ptype) f.u32(0u);           // an electron track records its (zero) step count first
           f.byte('M');
           atomicAdd(a.fp + (h - a.fp_base), f.v);
         }
-      }
+      } else if (tiles) bin = tile_bin(a.tm, vi, vj, vk);
     }
   }
   if (a.compact) {
@@ -226,24 +243,94 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
       o1.w = __uint_as_float(t | ((unsigned)ptype << 31));
       __stcs(a.p0 + dst, o0); __stcs(a.p1 + dst, o1);         // write-once / read-once: streaming, keeps L2 for the phantom and the grid
       if (a.p2) a.p2[dst] = com_col;
+      if (tiles) atomicAdd(&s_hist[bin], 1u);
     }
   } else if (live) {
     o1.w = pass ? (float)g : -(float)g - 1.0f;
     a.p0[t] = o0; a.p1[t] = o1;
   }
-  // ledgers: incident and jaw-rejected energy, block-reduced, spread over slots
+  }
+  // ledgers: incident, jaw-rejected and escaped (missed) energy, one 128-bit add per warp and ledger, spread over slots
   if (a.ctl) {
-    q_inc = warp_sum_q(q_inc); q_jaw = warp_sum_q(q_jaw); q_esc = warp_sum_q(q_esc);
-    const unsigned nmiss = __popc(__ballot_sync(kFull, missed));
-    if (lane == 0) { s_led[threadIdx.x >> 5][0] = q_inc; s_led[threadIdx.x >> 5][1] = q_jaw; s_led[threadIdx.x >> 5][2] = q_esc; s_miss[threadIdx.x >> 5] = nmiss; }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      unsigned long long si = 0, sj = 0, se = 0; unsigned nm = 0;
-      for (int w = 0; w < kThreads / 32; ++w) { si += s_led[w][0]; sj += s_led[w][1]; se += s_led[w][2]; nm += s_miss[w]; }
-      unsigned long long (*L)[2] = a.ctl->ledger[blockIdx.x % kLedgerSlots];
-      add128(L[0], si); add128(L[3], sj); add128(L[2], se);
+    q_inc = warp_sum_u64(q_inc); q_jaw = warp_sum_u64(q_jaw); q_esc = warp_sum_u64(q_esc);
+    const unsigned nm = __reduce_add_sync(kFull, n_miss);
+    if (lane == 0) {
+      unsigned long long (*L)[2] = a.ctl->ledger[(blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5)) % kLedgerSlots];
+      add128(L[0], q_inc); add128(L[3], q_jaw); add128(L[2], q_esc);
       if (nm) { atomicAdd(&a.ctl->n_missed, (unsigned long long)nm); if (a.stats) atomicAdd(&a.ctl->stat[ST_MISSED], (unsigned long long)nm); }
     }
+  }
+  if (tiles) {
+    __syncthreads();
+    for (int i = threadIdx.x; i < a.tm.nbins; i += kThreads) { const unsigned c = s_hist[i]; if (c) atomicAdd(a.tile_count + i, c); }
+  }
+}
+
+// Counts → cursors (exclusive prefix sum over the bins, one CTA of 1024 threads), counts zeroed for the next batch.
+__global__ void __launch_bounds__(1024) k_tile_scan(unsigned *count, unsigned *cursor, int nbins) {
+  __shared__ unsigned s_w[32];
+  const int per = (nbins + 1023) / 1024, b0 = threadIdx.x * per;
+  unsigned loc[4], sum = 0;                                  // per <= 4 (kTileBinsMax / 1024)
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { loc[k] = (k < per && b0 + k < nbins) ? count[b0 + k] : 0u; sum += loc[k]; }
+  unsigned inc = sum;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const unsigned v = __shfl_up_sync(kFull, inc, o); if ((threadIdx.x & 31) >= o) inc += v; }
+  if ((threadIdx.x & 31) == 31) s_w[threadIdx.x >> 5] = inc;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    unsigned w = s_w[threadIdx.x], wi = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const unsigned v = __shfl_up_sync(kFull, wi, o); if (threadIdx.x >= o) wi += v; }
+    s_w[threadIdx.x] = wi - w;
+  }
+  __syncthreads();
+  unsigned run = s_w[threadIdx.x >> 5] + inc - sum;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) if (k < per && b0 + k < nbins) { cursor[b0 + k] = run; run += loc[k]; count[b0 + k] = 0u; }
+}
+
+// Moves the packed survivors (p planes) to their tile-ordered places (q planes).  A CTA takes chunks of kTileChunk
+// particles: local histogram in shared memory, one global reservation per non-empty bin, then the moves.
+constexpr int kTileChunk = 4096;
+struct ScatterArgs {
+  Grid g; TileMap tm;
+  const float4 *p0, *p1; const uint32_t *p2;
+  float4 *q0, *q1; uint32_t *q2;
+  const unsigned *n_pb; unsigned *cursor;
+};
+__global__ void __launch_bounds__(kThreads) k_tile_scatter(const __grid_constant__ ScatterArgs a) {
+  extern __shared__ unsigned s_t[];                          // [nbins] counts, then [nbins] bases
+  unsigned *s_cnt = s_t, *s_base = s_t + a.tm.nbins;
+  const unsigned n = *a.n_pb;
+  for (unsigned c0 = blockIdx.x * kTileChunk; c0 < n; c0 += gridDim.x * kTileChunk) {
+    for (int i = threadIdx.x; i < a.tm.nbins; i += kThreads) s_cnt[i] = 0u;
+    __syncthreads();
+    unsigned bins[kTileChunk / kThreads];
+#pragma unroll
+    for (int k = 0; k < kTileChunk / kThreads; ++k) {
+      const unsigned i = c0 + k * kThreads + threadIdx.x;
+      bins[k] = 0xffffffffu;
+      if (i < n) {
+        const float4 A = __ldcs(a.p0 + i);
+        int vi, vj, vk; locate(a.g, A.x, A.y, A.z, vi, vj, vk);     // inside the grid: k_sample moved it to its entry point
+        bins[k] = tile_bin(a.tm, vi, vj, vk);
+        atomicAdd(&s_cnt[bins[k]], 1u);
+      }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < a.tm.nbins; i += kThreads) { const unsigned c = s_cnt[i]; if (c) s_base[i] = atomicAdd(a.cursor + i, c); s_cnt[i] = 0u; }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < kTileChunk / kThreads; ++k) {
+      const unsigned i = c0 + k * kThreads + threadIdx.x;
+      if (bins[k] != 0xffffffffu) {
+        const unsigned dst = s_base[bins[k]] + atomicAdd(&s_cnt[bins[k]], 1u);
+        __stcs(a.q0 + dst, __ldcs(a.p0 + i)); __stcs(a.q1 + dst, __ldcs(a.p1 + i));
+        if (a.p2) a.q2[dst] = a.p2[i];
+      }
+    }
+    __syncthreads();
   }
 }
 
@@ -273,6 +360,23 @@ __global__ void k_pack_phantom(const float *density, const uint8_t *material, si
     for (int o = 16; o > 0; o >>= 1) b = fmaxf(b, __shfl_xor_sync(kFull, b, o));
     if ((threadIdx.x & 31) == 0 && b > 0.f) atomicMax((unsigned *)&c->rhomax[k], __float_as_uint(b));
   }
+}
+
+// The brick table of the two-level phantom (Grid::brick): one thread per brick of 4x4x4 voxels (clipped at the grid's edge).
+__global__ void k_bricks(const uint32_t *vox, int nx, int ny, int nz, int nbx, int nby, unsigned nbricks, uint32_t *brick, Control *c) {
+  const unsigned b = blockIdx.x * blockDim.x + threadIdx.x;
+  bool uni = false;
+  if (b < nbricks) {
+    const int bi = (int)(b % (unsigned)nbx), bj = (int)((b / (unsigned)nbx) % (unsigned)nby), bk = (int)(b / ((unsigned)nbx * (unsigned)nby));
+    const uint32_t w0 = vox[((size_t)(bk * 4) * ny + bj * 4) * nx + bi * 4];
+    uni = true;
+    for (int k = bk * 4; k < min(bk * 4 + 4, nz); ++k)
+      for (int j = bj * 4; j < min(bj * 4 + 4, ny); ++j)
+        for (int i = bi * 4; i < min(bi * 4 + 4, nx); ++i) uni &= vox[((size_t)k * ny + j) * nx + i] == w0;
+    brick[b] = uni ? (w0 | 0x80000000u) : 0u;
+  }
+  const unsigned n = __popc(__ballot_sync(kFull, uni));
+  if ((threadIdx.x & 31) == 0 && n) atomicAdd(&c->n_uniform_bricks, n);
 }
 
 // Photon cross-section data: layout in pslmc_device.cuh (XsTable), evaluated in double.  The sigma_KN nodes depend on

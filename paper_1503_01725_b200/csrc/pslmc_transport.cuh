@@ -42,6 +42,7 @@ struct TransportArgs {
   // options
   unsigned long long *fp; unsigned long long fp_base;
   int electrons_local, static_lanes, stage_scoring;
+  int fp_voxels;                      // DBG variants: strict fingerprints (MC_FLAG_FP_VOXELS)
   int want_type;                      // SRC_BUFFER, compact: take only entries of this particle type (bit 31 of p1.w)
   XsTable xs;                         // k_photon: cross-section table (global; copied to shared memory per CTA)
   const float *rhomax;                // largest density per material of this call's phantom (device; k_pack_phantom)
@@ -269,6 +270,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
   float4 *s_annih = reinterpret_cast<float4 *>(s_raw + kXsBytes + sizeof(StageRing) * (kThreads / 32)) + 2 * threadIdx.x;
   ScoreStage<STAGE> stage; stage.init(s_raw + kXsBytes + sizeof(StageRing) * (kThreads / 32) + kAnnihBytes);
   const Grid &g = a.g;
+  const bool bricks = use_bricks(g);
   const unsigned n1 = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
   const unsigned count = n1;
   SrcCursor sc; sc.next = sc.end = 0u;
@@ -324,7 +326,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
       if (E >= kPcut) xs_lookup(s_xs, a.xs.x0, a.xs.inv_h, a.xs.n, E, skn, inv_e3, lp2, mu_max);
       if (E < kPcut) {                                   // below cut-off: absorbed on the spot
         const long long q = quanta(E); pend.add(g, stage, cvox, q); tl.dep += (unsigned long long)q;
-        if (DBG) { fnv.byte('A'); ++tl.st[ST_PCUT]; ++tl.st[ST_DEPOSITS]; }
+        if (DBG) { if (a.fp_voxels) fnv.u32((uint32_t)cvox); fnv.byte('A'); ++tl.st[ST_PCUT]; ++tl.st[ST_DEPOSITS]; }
         done = true;
       } else if (!(mu_max > 0.0f)) {
         tl.esc += (unsigned long long)quanta(E);
@@ -343,7 +345,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
           done = true;
         } else {
           cvox = vox_index(g, vi, vj, vk);
-          float rho; int mt; fetch_voxel(g, cvox, rho, mt);
+          float rho; int mt; fetch_voxel(g, bricks, vi, vj, vk, cvox, rho, mt);
           const float muC = rho * (c_mat.ne[mt] * skn), muT = rho * (c_mat.cphoto[mt] * inv_e3), muK = rho * (c_mat.ppair[mt] * lp2);
           const float tt = u_co(d1) * mu_max;
           if (tt < muC) {                                // Compton: Kahn trials are event 2
@@ -351,7 +353,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
             if (DBG) { fnv.byte('C'); ++tl.st[ST_COMPTON]; }
           } else if (tt < muC + muT) {                   // photo-electric: local absorption
             const long long q = quanta(E); pend.add(g, stage, cvox, q); tl.dep += (unsigned long long)q;
-            if (DBG) { fnv.byte('P'); ++tl.st[ST_PHOTO]; ++tl.st[ST_DEPOSITS]; }
+            if (DBG) { fnv.byte('P'); if (a.fp_voxels) fnv.u32((uint32_t)cvox); ++tl.st[ST_PHOTO]; ++tl.st[ST_DEPOSITS]; }
             done = true;
           } else if (tt < muC + muT + muK) {             // pair production: event 2
             state = PH_PAIR;
@@ -382,6 +384,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
         const float ct = 1.0f - k;
         const bool accept = brA ? (r3 <= 4.0f * (ie - ie * ie)) : (r3 <= 0.5f * (ct * ct + ie));
         if (accept) {
+          if (DBG && a.fp_voxels) fnv.u32(rng.blk);                // strict fingerprint: which trial was accepted
           const float sn = sqrt_fast(fmaxf(0.0f, k * (2.0f - k)));
           const float Ep = E * ie, T = E - Ep, u0 = u, v0 = v, w0 = w;
           rotate(u, v, w, ct, sn, u_co(d3));
@@ -394,7 +397,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
             if (DBG) ++tl.st[ST_SEC_E];
           } else {
             const long long q = quanta(T); pend.add(g, stage, cvox, q); tl.dep += (unsigned long long)q;
-            if (DBG) ++tl.st[ST_DEPOSITS];
+            if (DBG) { if (a.fp_voxels) fnv.u32((uint32_t)cvox); ++tl.st[ST_DEPOSITS]; }
           }
           ++nchild; E = Ep; state = PH_FLIGHT;
         }
@@ -408,7 +411,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
             if (DBG) ++tl.st[ST_SEC_E];
           } else {
             const long long q = quanta(Tc[sl]); pend.add(g, stage, cvox, q); tl.dep += (unsigned long long)q;
-            if (DBG) ++tl.st[ST_DEPOSITS];
+            if (DBG) { if (a.fp_voxels) fnv.u32((uint32_t)cvox); ++tl.st[ST_DEPOSITS]; }
           }
         }
         const float cz = 2.0f * u_co(d1) - 1.0f, sz = sqrtf(fmaxf(0.0f, 1.0f - cz * cz));
@@ -462,6 +465,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
   // whole): the call fails with MC_E_OVERFLOW, nothing here may be read
   if (a.src_kind == SRC_QUEUE && (a.ctl->overflow & 1u)) return;
   ScoreStage<STAGE> stage; stage.init(s_raw);
+  const bool bricks = use_bricks(g);
   const unsigned n1 = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
   const unsigned count = n1;
   SrcCursor sc; sc.next = sc.end = 0u;
@@ -506,7 +510,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
 
     if (active) {                                        // one sub-step
       const int vox = vox_index(g, vi, vj, vk);
-      float rho; int mt; fetch_voxel(g, vox, rho, mt);
+      float rho; int mt; fetch_voxel(g, bricks, vi, vj, vk, vox, rho, mt);
       if (fresh) { budget = kFe * T; Tms = T; tacc = 0.0f; fresh = false; }
       const float D = (c_mat.sscale[mt] * rho) * __fmaf_rn(0.078f, T, __fmaf_rn(0.25f, rcp_fast(T), 1.52f));
       const float sE = D > 0.0f ? __fdividef(budget, D) : INFINITY;
@@ -517,7 +521,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
       const bool turn = sE <= sv + kEpsB;              // this sub-step ends the condensed step
       const float s = turn ? sE : sv + kEpsB, dT = turn ? budget : D * s;
       ++steps;
-      if (DBG) { ++tl.st[ST_ESTEPS]; ++tl.st[ST_DEPOSITS]; }
+      if (DBG) { ++tl.st[ST_ESTEPS]; ++tl.st[ST_DEPOSITS]; if (a.fp_voxels) fnv.u32((uint32_t)vox | (turn ? 0x80000000u : 0u)); }
       bool done = false;
       const bool stop = T - dT <= kEcut;               // below the cut-off after this sub-step: everything left is deposited here
       const long long q = quanta(stop ? T : dT); pend.add(g, stage, vox, q); tl.dep += (unsigned long long)q;

@@ -5,11 +5,14 @@ import numpy as np
 from scipy import ndimage
 
 
-def gamma_pass_rate(ref, ev, voxel_cm, dose_frac=0.01, dta_cm=0.1, threshold=0.10, step_cm=0.025):
-    """ref, ev: 3-D arrays (z, y, x).  Returns (pass rate over voxels with ref >= threshold * max, gamma array)."""
+def gamma_pass_rate(ref, ev, voxel_cm, dose_frac=0.01, dta_cm=0.1, threshold=0.10, step_cm=0.025, max_points=0, seed=0):
+    """ref, ev: 3-D arrays (z, y, x).  Returns (pass rate over voxels with ref >= threshold * max, gamma array).
+    max_points > 0: evaluate a seeded random sample of that many of those voxels (large grids)."""
     ref = np.asarray(ref, np.float64); ev = np.asarray(ev, np.float64)
     dmax = ref.max()
     idx = np.argwhere(ref >= threshold * dmax)
+    if max_points and len(idx) > max_points:
+        idx = idx[np.sort(np.random.default_rng(seed).choice(len(idx), max_points, replace=False))]
     dd = dose_frac * dmax
     n = int(np.floor(dta_cm * 1.0001 / step_cm))
     offs = np.arange(-n, n + 1) * step_cm

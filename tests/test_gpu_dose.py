@@ -83,7 +83,8 @@ def test_bitwise_identity_under_batch_order_partition(B, gpsl, cfg):
     for batch, opt in ((1000, {}), (33_333, {}), (1 << 20, {}), (1 << 13, dict(order=B.MC_ORDER_MIXED)),
                        (1 << 15, dict(flags=B.MC_FLAG_STATIC_LANES)), (1 << 15, dict(flags=B.MC_FLAG_STATS | B.MC_FLAG_TIMING)),
                        (1 << 14, dict(pipelines=1)), (1 << 12, dict(pipelines=2, flags=B.MC_FLAG_TIMING)),
-                       (1 << 16, dict(flags=B.MC_FLAG_STAGE_SCORING)), (1 << 12, dict(flags=B.MC_FLAG_STAGE_SCORING | B.MC_FLAG_STATS, order=B.MC_ORDER_MIXED))):
+                       (1 << 16, dict(flags=B.MC_FLAG_STAGE_SCORING)), (1 << 12, dict(flags=B.MC_FLAG_STAGE_SCORING | B.MC_FLAG_STATS, order=B.MC_ORDER_MIXED)),
+                       (1 << 14, dict(flags=B.MC_FLAG_TILE_SORT)), (1 << 13, dict(flags=B.MC_FLAG_TILE_SORT | B.MC_FLAG_STATS, order=B.MC_ORDER_MIXED, pipelines=1))):
         acc, dose, st, fp = gpu_dose(B, g, dph, beam, N, seed, batch, **opt)
         assert np.array_equal(acc, ref_acc), (batch, opt)
         assert np.array_equal(dose, ref_dose) and np.array_equal(fp, ref_fp)
