@@ -62,7 +62,7 @@ const double FIX = 4294967296.0;                          // 2^32 quanta per MeV
 const int FLAG_ELECTRONS_LOCAL = 1;
 const int FLAG_TRACE_BIRTH = 2;       // orc_trace only: log a 'B' event (position, direction, energy) when a track starts
 const int FLAG_FP_VOXELS = 4;         // strict fingerprints (F1): also the voxel of every deposit, the stream position after every
-                                      // accepted Kahn sampling (= which trial was accepted) and whether an electron sub-step ended its condensed step
+                                      // accepted Kahn sampling (= which trial was accepted) with the branch it took, and whether an electron sub-step ended its condensed step
 
 // ---------------------------------------------------------------- R1: Philox4x32-10
 void philox_block(uint64_t seed, uint64_t h, uint32_t track, uint32_t block, uint32_t out[4]) {
@@ -432,7 +432,7 @@ void rotate(double d[3], double ct, double st, double phi) {
 
 // Kahn's rejection for Klein–Nishina; returns eta = E/E'.  One block per trial: words 0, 1, 2 = r1, r2, r3; word 3
 // of the ACCEPTED trial is returned in `w_phi` (the caller's azimuth draw).
-double kahn(double alpha, Stream &st, uint32_t &w_phi, uint64_t *n_trials = nullptr) {
+double kahn(double alpha, Stream &st, uint32_t &w_phi, uint64_t *n_trials = nullptr, int *branch = nullptr) {
   for (;;) {
     uint32_t w[4]; st.next_block(w);
     if (n_trials) ++*n_trials;
@@ -440,11 +440,11 @@ double kahn(double alpha, Stream &st, uint32_t &w_phi, uint64_t *n_trials = null
     w_phi = w[3];
     if (r1 <= (2.0 * alpha + 1.0) / (2.0 * alpha + 9.0)) {
       double eta = 1.0 + 2.0 * alpha * r2;
-      if (r3 <= 4.0 * (1.0 / eta - 1.0 / (eta * eta))) return eta;
+      if (r3 <= 4.0 * (1.0 / eta - 1.0 / (eta * eta))) { if (branch) *branch = 0; return eta; }
     } else {
       double eta = (2.0 * alpha + 1.0) / (1.0 + 2.0 * alpha * r2);
       double ct = 1.0 - (eta - 1.0) / alpha;
-      if (r3 <= 0.5 * (ct * ct + 1.0 / eta)) return eta;
+      if (r3 <= 0.5 * (ct * ct + 1.0 / eta)) { if (branch) *branch = 1; return eta; }
     }
   }
 }
@@ -533,8 +533,8 @@ struct Ctx {
       double tt = U_co(wf[1]) * mmax;
       if (tt < muC) {                                  // Compton, Klein–Nishina by Kahn
         collided = true; ++res->n_compton; f.byte('C');
-        uint32_t w_phi; double alpha = t.E / ME, eta = kahn(alpha, st, w_phi, &res->n_kahn_trials);
-        if (flags & FLAG_FP_VOXELS) f.u32(st.j);
+        uint32_t w_phi; int branch = 0; double alpha = t.E / ME, eta = kahn(alpha, st, w_phi, &res->n_kahn_trials, &branch);
+        if (flags & FLAG_FP_VOXELS) f.u32(st.j | (branch ? 0x80000000u : 0u));
         double k = (eta - 1.0) / alpha, ct = 1.0 - k, sn = std::sqrt(std::fmax(0.0, k * (2.0 - k)));
         double phi = 2.0 * PI * U_co(w_phi);
         double Ep = t.E / eta, T = t.E - Ep, d0[3] = {t.dir[0], t.dir[1], t.dir[2]};

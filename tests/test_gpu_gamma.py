@@ -69,7 +69,7 @@ GG = [("C1", 0, 4_000_000_000), ("C2", 0, 4_000_000_000), ("C3", 0, 4_000_000_00
 @pytest.mark.parametrize("name,beam,n", GG)
 def test_gamma_gpu_vs_gpu_two_seeds(name, beam, n, cfg):
     """Consistency of the GPU path with itself under a change of seed, on the real geometries: gamma 1 %/1 mm (global)
-    between two seeds, with the per-voxel statistical sigma printed beside it (measured from the two halves of one run).
+    between two seeds, with the per-voxel statistical sigma printed beside it (measured with a third seed).
     Where sigma <= 0.35 % the north_star bar (>= 99 %) is asserted as it stands; where the statistics a test run can
     afford leave more noise than that, the pass rate is compared with what pure noise of the measured sigma gives
     (dose criterion alone, no distance-to-agreement: a lower bound) - a bias between seeds would show as a deficit."""
@@ -87,11 +87,11 @@ def test_gamma_gpu_vs_gpu_two_seeds(name, beam, n, cfg):
         g.dose(dph, c["beams"][beam], n, seed, batch=1 << 22, dose_acc=acc, history_begin=hb, history_end=he)
         return acc.cpu().numpy().astype(np.float64)
 
-    a1, a2 = run(1001, 0, n // 2), run(1001, n // 2, n)
-    d_a, d_b = (a1 + a2).reshape(shape), run(2002, 0, n).reshape(shape)
+    d_a, d_b, d_c = (run(s, 0, n).reshape(shape) for s in (1001, 2002, 3003))
+    rho = np.asarray(ph["density"], np.float64).reshape(shape)
+    d_a, d_b, d_c = (np.where(rho >= 0.1, d / np.maximum(rho, 1e-30), 0.0) for d in (d_a, d_b, d_c))     # dose in tissue (the air around C3's body would define Dmax)
     big = d_a > 0.1 * d_a.max()
-    half = ((a1 - a2).reshape(shape)[big] / d_a[big])                     # difference of the halves / full tally: std = sigma_full... x 1
-    sigma = float(half.std())                                             # (a1-a2)/(a1+a2) has the relative sigma of the full run
+    sigma = float(((d_b[big] - d_c[big]) / d_a[big]).std() / np.sqrt(2.0))    # from the two seeds the gamma does not use twice
     rate, gam = gamma_pass_rate(d_a, d_b, (ph["dx"], ph["dy"], ph["dz"]), dose_frac=0.01, dta_cm=0.1, threshold=0.10,
                                 max_points=60_000, seed=7)
     # noise-only expectation without DTA: |N(0, sqrt(2) sigma D_v)| <= 0.01 Dmax, averaged over the evaluated voxels
