@@ -160,8 +160,8 @@ class Psl:
         self.grid_x0 = lib().orc_psl_grid_x0(self.h) if n_sectors == 0 else 0.0
 
     def __del__(self):
-        if getattr(self, "h", None):
-            lib().orc_psl_free(self.h)
+        if getattr(self, "h", None) and _lib is not None:        # (at interpreter shutdown the module globals may be gone)
+            _lib.orc_psl_free(self.h)
             self.h = None
 
     def set_direction_model(self, stype: int, c, mu, sigma_a, sigma_b):

@@ -91,6 +91,7 @@ struct Grid {
   // commissioning tally, off when com_index is null: com_index[v] = 0 or 1 + row,
   // com_dose[col * com_rows + row], col = the PSR unit the history was sampled from
   const int *com_index; unsigned long long *com_dose; int com_rows;
+  const uint32_t *com_mask;                          // one bit per voxel: com_index[v] != 0 (built per call; the index array itself is read only for those)
 };
 
 __device__ __forceinline__ long long quanta(float e) { return __float2ll_rn(e * 4294967296.0f); }

@@ -33,7 +33,7 @@ static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 // k_sample and ordered by entry tile -, the entry-tile counters, and the electron queue (capacity 4B, 3 planes).  mc_dose_host appends its staging area (phantom in, dose out).
 constexpr int kMaxPipes = 2;
 struct Layout {
-  size_t ctl[kMaxPipes], tile[kMaxPipes], xs, vox, brick, acc, p0[kMaxPipes], p1[kMaxPipes], p2[kMaxPipes], q0[kMaxPipes], q1[kMaxPipes], q2[kMaxPipes],
+  size_t ctl[kMaxPipes], tile[kMaxPipes], xs, vox, brick, com_mask, acc, p0[kMaxPipes], p1[kMaxPipes], p2[kMaxPipes], q0[kMaxPipes], q1[kMaxPipes], q2[kMaxPipes],
       eq[kMaxPipes][3], total, zero_bytes;
   size_t host_rho, host_mat, host_dose, host_total;
   unsigned eq_cap;
@@ -46,7 +46,7 @@ static Layout make_layout(uint64_t batch, size_t nvox, size_t nbricks) {
   for (int p = 0; p < kMaxPipes; ++p) L.ctl[p] = take(sizeof(Control));     // contiguous from offset 0: zeroed by one memset,
   for (int p = 0; p < kMaxPipes; ++p) L.tile[p] = take(2 * sizeof(unsigned) * kTileBinsMax);   // with the entry-tile counts and cursors
   L.zero_bytes = o;
-  L.xs = take(kXsBytes); L.vox = take(4 * nvox); L.brick = take(4 * nbricks); L.acc = take(8 * nvox);
+  L.xs = take(kXsBytes); L.vox = take(4 * nvox); L.brick = take(4 * nbricks); L.com_mask = take(4 * ((nvox + 31) / 32)); L.acc = take(8 * nvox);
   for (int p = 0; p < kMaxPipes; ++p) {
     L.p0[p] = take(16 * batch); L.p1[p] = take(16 * batch); L.p2[p] = take(4 * batch);
     L.q0[p] = take(16 * batch); L.q1[p] = take(16 * batch); L.q2[p] = take(4 * batch);     // the same, ordered by entry tile
@@ -180,10 +180,10 @@ struct Session {
   char *ws = nullptr; Layout L{}; Grid g{}; size_t nvox = 0;
   cudaStream_t us = nullptr;                    // the caller's stream
   int npipe = 1; Pipe pipes[kMaxPipes];
-  int flags = 0; bool dbg = false, timing = false;
+  int flags = 0, mode = MODE_PLAIN; bool dbg = false, timing = false;
   unsigned eq_cap = 0; uint64_t batch = 0;
   XsTable xs{}; const float *rhomax = nullptr;
-  int blocks_photon = 1, blocks_electron = 1, sms = 1;
+  int blocks_photon = 1, blocks_electron = 1, blocks_sample = 1, sms = 1;
   TileMap tm{};                                 // nbins = 0: batches are not ordered by entry tile
   uint64_t task = 0;                            // batches dealt so far (round-robin over the pipelines)
   cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev_fork = nullptr, ev_join[kMaxPipes] = {};
@@ -197,33 +197,40 @@ struct Session {
   }
 
   // Kernel variants: <stats + fingerprints + commissioning tally> or plain, <shared-memory staging of the scoring> or not.
+  // Kernel variants: mode (plain / + commissioning tally / + stats and fingerprints) x shared-memory staging of the scoring.
+  template <int M, bool S> void launch_photon_v(Pipe &p, const TransportArgs &a, int nb, size_t sm) { k_photon<M, S><<<nb, kThreads, sm, p.st>>>(a); }
+  template <int M, bool S> void launch_electron_v(Pipe &p, const TransportArgs &a, int nb, size_t sm) { k_electron<M, S><<<nb, kThreads, sm, p.st>>>(a); }
+#define PSLMC_DISPATCH(fn, ...)                                                                                     \
+  do {                                                                                                              \
+    const bool st_ = (flags & MC_FLAG_STAGE_SCORING) != 0;                                                          \
+    if (mode == MODE_PLAIN) { if (st_) fn<MODE_PLAIN, true>(__VA_ARGS__); else fn<MODE_PLAIN, false>(__VA_ARGS__); } \
+    else if (mode == MODE_COM) { if (st_) fn<MODE_COM, true>(__VA_ARGS__); else fn<MODE_COM, false>(__VA_ARGS__); }  \
+    else { if (st_) fn<MODE_DBG, true>(__VA_ARGS__); else fn<MODE_DBG, false>(__VA_ARGS__); }                        \
+  } while (0)
   void launch_photon(Pipe &p, const TransportArgs &a) {
     p.tm.begin(MC_K_PHOTON);
     const int nb = (int)std::max<uint64_t>(1, std::min<uint64_t>({(uint64_t)blocks_photon, (batch + kThreads - 1) / kThreads, 4096 / (kThreads / 32)}));
     const size_t sm = kXsSmem + (a.stage_scoring ? kScoreBytes : 0);
-    if (a.stage_scoring) { if (dbg) k_photon<true, true><<<nb, kThreads, sm, p.st>>>(a); else k_photon<false, true><<<nb, kThreads, sm, p.st>>>(a); }
-    else { if (dbg) k_photon<true, false><<<nb, kThreads, sm, p.st>>>(a); else k_photon<false, false><<<nb, kThreads, sm, p.st>>>(a); }
+    PSLMC_DISPATCH(launch_photon_v, p, a, nb, sm);
     p.tm.end(MC_K_PHOTON); ++p.launches[MC_K_PHOTON];
   }
   void launch_electron(Pipe &p, const TransportArgs &a) {
     p.tm.begin(MC_K_ELECTRON);
     const int nb = blocks_electron; const size_t sm = a.stage_scoring ? kScoreBytes : 0;
-    if (a.stage_scoring) { if (dbg) k_electron<true, true><<<nb, kThreads, sm, p.st>>>(a); else k_electron<false, true><<<nb, kThreads, sm, p.st>>>(a); }
-    else { if (dbg) k_electron<true, false><<<nb, kThreads, sm, p.st>>>(a); else k_electron<false, false><<<nb, kThreads, sm, p.st>>>(a); }
+    PSLMC_DISPATCH(launch_electron_v, p, a, nb, sm);
     p.tm.end(MC_K_ELECTRON); ++p.launches[MC_K_ELECTRON];
+  }
+  template <int M, bool S> void setup_v(size_t smp, size_t sme, double scale) {
+    cudaFuncSetAttribute(k_photon<M, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smp);
+    blocks_photon = persistent_blocks(k_photon<M, S>, smp, scale);
+    blocks_electron = persistent_blocks(k_electron<M, S>, sme, scale);
   }
   void init_blocks(double scale) {
     const bool stage = (flags & MC_FLAG_STAGE_SCORING) != 0;
     const size_t smp = kXsSmem + (stage ? kScoreBytes : 0), sme = stage ? kScoreBytes : 0;
-#define PSLMC_SETUP(D, S)                                                                                          \
-    if (dbg == D && stage == S) {                                                                                  \
-      cudaFuncSetAttribute(k_photon<D, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smp);                 \
-      blocks_photon = persistent_blocks(k_photon<D, S>, smp, scale);                                               \
-      blocks_electron = persistent_blocks(k_electron<D, S>, sme, scale);                                           \
-    }
-    PSLMC_SETUP(false, false) PSLMC_SETUP(false, true) PSLMC_SETUP(true, false) PSLMC_SETUP(true, true)
-#undef PSLMC_SETUP
+    PSLMC_DISPATCH(setup_v, smp, sme, scale);
   }
+#undef PSLMC_DISPATCH
 
   TransportArgs base_args(const Pipe &p, uint64_t seed, uint64_t n_total, uint64_t perm_a) const {
     TransportArgs a{};
@@ -258,7 +265,8 @@ struct Session {
     }
     ws = (char *)workspace; us = (cudaStream_t)o.cuda_stream; flags = o.flags;
     eq_cap = o.debug_eq_cap ? std::min(o.debug_eq_cap, L.eq_cap) : L.eq_cap;
-    dbg = (o.flags & MC_FLAG_STATS) || o.fingerprints || o.com_index;         // stats, fingerprints and the tally live in the DBG variants
+    dbg = (o.flags & MC_FLAG_STATS) || o.fingerprints;                        // stats and fingerprints live in the DBG variants,
+    mode = dbg ? MODE_DBG : (o.com_index ? MODE_COM : MODE_PLAIN);            // the commissioning tally has its own
     timing = (o.flags & MC_FLAG_TIMING) != 0;
     npipe = o.pipelines > 0 ? o.pipelines : kMaxPipes;
     npipe = std::max(1, std::min(npipe, kMaxPipes));
@@ -270,6 +278,7 @@ struct Session {
     g.nbx = (ph.nx + 3) / 4; g.nby = (ph.ny + 3) / 4; g.nbricks = (unsigned)((size_t)g.nbx * g.nby * ((ph.nz + 3) / 4));
     g.brick = (const uint32_t *)(ws + L.brick); g.n_uniform = &((Control *)(ws + L.ctl[0]))->n_uniform_bricks;
     g.com_index = (const int *)o.com_index; g.com_dose = (unsigned long long *)o.com_dose; g.com_rows = o.com_rows;
+    g.com_mask = (const uint32_t *)(ws + L.com_mask);
     for (int p = 0; p < npipe; ++p) {
       Pipe &q = pipes[p];
       q.st = npipe > 1 ? (cudaStream_t)o.aux_streams[p] : us; q.ctl = (Control *)(ws + L.ctl[p]);
@@ -292,12 +301,14 @@ struct Session {
     // measured on C4 it takes 10 % off the transport kernels' time and costs as much in the sort - photons
     // scatter 10-20 cm away from their entry tile.  Cubic tiles of 2^shift voxels, at most kTileBinsMax bins.
     tm = TileMap{};
+    blocks_sample = 0;
     if ((o.flags & MC_FLAG_TILE_SORT) && !(o.flags & MC_FLAG_NO_TILE_SORT)) {
       int sh = 3;
       auto nt = [&](int n) { return ((n - 1) >> sh) + 1; };
       while ((long long)nt(ph.nx) * nt(ph.ny) * nt(ph.nz) > kTileBinsMax) ++sh;
       tm.shift = sh; tm.ntx = nt(ph.nx); tm.nty = nt(ph.ny); tm.nbins = tm.ntx * tm.nty * nt(ph.nz);
     }
+    blocks_sample = persistent_blocks(k_sample, sizeof(unsigned) * tm.nbins, 1.0);
     rhomax = pipes[0].ctl->rhomax;
     CUDA_TRY(cudaEventCreate(&ev0)); CUDA_TRY(cudaEventCreate(&ev1));
     CUDA_TRY(cudaEventRecord(ev0, us));
@@ -307,6 +318,7 @@ struct Session {
     tm_us.begin(MC_K_AUX);
     k_pack_phantom<<<592, 256, 0, us>>>(ph.density, ph.material, nvox, (uint32_t *)(ws + L.vox), pipes[0].ctl);
     k_bricks<<<(g.nbricks + 255) / 256, 256, 0, us>>>(g.vox, g.nx, g.ny, g.nz, g.nbx, g.nby, g.nbricks, (uint32_t *)(ws + L.brick), pipes[0].ctl);
+    if (g.com_index) { k_com_mask<<<(unsigned)(((nvox + 31) / 32 + 255) / 256), 256, 0, us>>>(g.com_index, nvox, (uint32_t *)(ws + L.com_mask)); ++launches_us[MC_K_AUX]; }
     tm_us.end(MC_K_AUX); launches_us[MC_K_AUX] += 2;
     if (npipe > 1) {
       CUDA_TRY(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
@@ -334,7 +346,7 @@ struct Session {
       sa.p2 = g.com_index ? p.p2 : nullptr;
       sa.tm = tm; sa.tile_count = tm.nbins ? p.tile_count : nullptr;
       p.tm.begin(MC_K_SAMPLE);
-      const unsigned nblk = (unsigned)std::min<uint64_t>((count + kThreads - 1) / kThreads, (uint64_t)sms * 8);      // persistent: 8 CTAs of 256 per SM
+      const unsigned nblk = (unsigned)std::min<uint64_t>((count + kThreads - 1) / kThreads, (uint64_t)blocks_sample);     // persistent: one wave
       k_sample<<<nblk, kThreads, sizeof(unsigned) * tm.nbins, p.st>>>(sa);
       if (tm.nbins) {                                     // counting sort of the survivors by entry tile: counts -> cursors -> moves
         k_tile_scan<<<1, 1024, 0, p.st>>>(p.tile_count, p.tile_cursor, tm.nbins);

@@ -233,7 +233,8 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
     }
   }
   if (a.compact) {
-    // survivors packed with one queue-tail atomic per warp
+    // survivors packed with one queue-tail atomic per warp (pipelining the stores behind the atomic's latency was
+    // measured: no gain - the kernel is bound by instruction issue)
     const unsigned keep = __ballot_sync(kFull, live && pass);
     unsigned base = 0;
     if (lane == 0 && keep) base = atomicAdd(&a.ctl->n_pb, __popc(keep));
@@ -360,6 +361,15 @@ __global__ void k_pack_phantom(const float *density, const uint8_t *material, si
     for (int o = 16; o > 0; o >>= 1) b = fmaxf(b, __shfl_xor_sync(kFull, b, o));
     if ((threadIdx.x & 31) == 0 && b > 0.f) atomicMax((unsigned *)&c->rhomax[k], __float_as_uint(b));
   }
+}
+
+// One bit per voxel: com_index[v] != 0 (the commissioning tally's measurement voxels are few: PAPER.md:134).
+__global__ void k_com_mask(const int *com_index, size_t n, uint32_t *mask) {
+  const size_t w = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+  if (w * 32 >= n) return;
+  uint32_t m = 0u;
+  for (int b = 0; b < 32 && w * 32 + b < n; ++b) m |= (com_index[w * 32 + b] != 0 ? 1u : 0u) << b;
+  mask[w] = m;
 }
 
 // The brick table of the two-level phantom (Grid::brick): one thread per brick of 4x4x4 voxels (clipped at the grid's edge).

@@ -106,13 +106,13 @@ struct ScoreStage {
 };
 
 // Pending deposit: consecutive deposits into one voxel are merged before the atomic (integers: exact).
-template <bool COM>                                   // COM: the kernel variant that may carry a commissioning tally (= DBG)
+template <bool COM>                                   // COM: the kernel variants that may carry a commissioning tally (MODE_COM, MODE_DBG)
 struct Pending {
   int v; long long q; uint32_t col;                  // col: commissioning column of the lane's current history
   template <bool ON> __device__ __forceinline__ void flush(const Grid &g, const ScoreStage<ON> &st) {
     if (q) {
       st.add(g, v, (unsigned long long)q);
-      if (COM && g.com_index) {                      // only the stats/fingerprint kernel variants are launched with a tally
+      if (COM && g.com_index && ((__ldg(g.com_mask + (v >> 5)) >> (v & 31)) & 1u)) {
         const int row = __ldg(g.com_index + v);
         if (row > 0 && row <= g.com_rows) atomicAdd(g.com_dose + (size_t)col * g.com_rows + (row - 1), (unsigned long long)q);
       }
@@ -255,8 +255,12 @@ __device__ __forceinline__ TrackIn load_track(const TransportArgs &a, unsigned i
 // of holding the warp in a rejection loop.  Cross-sections come from the shared-memory table.
 enum { PH_IDLE = 0, PH_FLIGHT = 1, PH_KAHN = 2, PH_PAIR = 3 };
 
-template <bool DBG, bool STAGE>
+// MODE: kernel variant - MODE_PLAIN (what bench.py times), MODE_COM (plain + the commissioning tally: every track carries
+// the PSR column of its history), MODE_DBG (event counters, fingerprints, and the tally when asked for).
+enum { MODE_PLAIN = 0, MODE_COM = 1, MODE_DBG = 2 };
+template <int MODE, bool STAGE>
 __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ TransportArgs a) {
+  constexpr bool DBG = MODE == MODE_DBG, COM = MODE != MODE_PLAIN;
   extern __shared__ __align__(16) unsigned char s_raw[];           // [xs table | one StageRing per warp]
   float *s_xs = reinterpret_cast<float *>(s_raw);
   for (int i = threadIdx.x; i <= a.xs.n; i += kThreads) s_xs[kXsHead + i] = a.xs.data[kXsHead + i];
@@ -278,7 +282,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
   StageCursor stg; stg.head = stg.n = stg.base_raw = 0u; stg.pending = false;
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
-  Pending<DBG> pend; pend.v = 0; pend.q = 0; pend.col = 0u;
+  Pending<COM> pend; pend.v = 0; pend.q = 0; pend.col = 0u;
   int state = PH_IDLE; bool exhausted = false, collided = false, pend2 = false;
   float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, E = 0;
   int cvox = 0;                                          // voxel of the current position
@@ -302,7 +306,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
       const TrackIn t = load_track(a, idx, n1);
       if (t.ok) {
         x = t.x; y = t.y; z = t.z; u = t.u; v = t.v; w = t.w; E = t.E; h = t.h; nchild = 0; collided = false;
-        if (DBG && g.com_index) { pend.flush(g, stage); pend.col = t.col; }
+        if (COM && g.com_index) { pend.flush(g, stage); pend.col = t.col; }
         rng.init(h, t.track, t.blk);
         if (DBG) fnv.init(t.track);
         if (a.buffer_is_debug) tl.inc += (unsigned long long)quanta(E);
@@ -436,7 +440,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
     }
     // ---- secondaries, convergent: Compton electrons through the staging ring ...
     stage_push(a.eq, a.ctl, ring, stg, push_e, make_float4(x, y, z, eT), make_float4(ex, ey, ez, 0.f),
-               make_uint4((uint32_t)h, (uint32_t)(h >> 32), etrack, DBG ? pend.col : 0u));
+               make_uint4((uint32_t)h, (uint32_t)(h >> 32), etrack, COM ? pend.col : 0u));
     // ... and, in the rare iteration with a pair production in the warp, the e-/e+ through the same ring (the lane's
     // x, y, z, u, v, w, h, track and nchild are still those of the converting photon)
     const unsigned mp = __ballot_sync(kFull, push_p);
@@ -444,7 +448,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
 #pragma unroll
       for (int sl = 0; sl < 2; ++sl)
         stage_push(a.eq, a.ctl, ring, stg, pairT[sl] > 0.0f, make_float4(x, y, z, pairT[sl]), make_float4(u, v, w, 0.f),
-                   make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, (uint32_t)sl), DBG ? pend.col : 0u));
+                   make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, (uint32_t)sl), COM ? pend.col : 0u));
       // the two 0.511 MeV annihilation photons (tracks: slots 2, 3 of this conversion) stay in the lane: it continues
       // as the first at once and keeps the second in its shared-memory slot until the first has ended
       if (push_p) {
@@ -470,8 +474,9 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
 // ~1e-6 cm of a global coordinate.  In exact arithmetic this is the
 // same walk as floor((pos - o)/d) on global coordinates.  One loop iteration = one sub-step; the two
 // draws of a condensed step come from one Philox site (draw numbers are always even here).
-template <bool DBG, bool STAGE>
+template <int MODE, bool STAGE>
 __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant__ TransportArgs a) {
+  constexpr bool DBG = MODE == MODE_DBG, COM = MODE != MODE_PLAIN;
   extern __shared__ __align__(16) unsigned char s_raw[];           // [score staging table] when enabled
   const Grid &g = a.g;
   // a queue that overflowed holds slots that were never written (a reservation that straddled its end is dropped
@@ -484,7 +489,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
   SrcCursor sc; sc.next = sc.end = 0u;
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
-  Pending<DBG> pend; pend.v = 0; pend.q = 0; pend.col = 0u;
+  Pending<COM> pend; pend.v = 0; pend.q = 0; pend.col = 0u;
   bool active = false, exhausted = false;
   float lx = 0, ly = 0, lz = 0, u = 0, v = 0, w = 1, T = 0;      // offset inside voxel (vi,vj,vk), direction, energy
   float iu = 0, iv = 0, iw = 1;                                   // reciprocal direction cosines (refreshed when the direction changes)
@@ -502,7 +507,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
       if (t.ok) {
         float x = t.x, y = t.y, z = t.z;
         u = t.u; v = t.v; w = t.w; T = t.E; h = t.h; steps = 0; fresh = true;
-        if (DBG && g.com_index) { pend.flush(g, stage); pend.col = t.col; }
+        if (COM && g.com_index) { pend.flush(g, stage); pend.col = t.col; }
         rng.init(h, t.track, t.blk);
         if (DBG) { fnv.init(t.track); ++tl.st[ST_ETRACKS]; }
         if (a.buffer_is_debug) tl.inc += (unsigned long long)quanta(T);

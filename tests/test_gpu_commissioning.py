@@ -34,6 +34,9 @@ def test_tally_identity_determinism_and_oracle_parity(B, orc, cfg):
     # same bits for another batch size / one pipeline, and the 3-D tally is the one of a run without the matrix
     acc2, A2 = gpu_matrix(B, g, dph, c["beams"][0], N, seed, idx, rows, cols, batch=30_000, pipelines=1)
     assert np.array_equal(A, A2) and np.array_equal(acc, acc2)
+    # the tally's own kernel variant (MODE_COM, above) and the stats/fingerprint variant (MODE_DBG) give the same bits
+    acc3, A3 = gpu_matrix(B, g, dph, c["beams"][0], N, seed, idx, rows, cols, batch=1 << 15, flags=B.MC_FLAG_STATS)
+    assert np.array_equal(A, A3) and np.array_equal(acc, acc3)
     import torch
     plain = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
     g.dose(dph, c["beams"][0], N, seed, batch=1 << 16, dose_acc=plain)
@@ -80,3 +83,32 @@ def test_commissioning_loop_recovers_a_reweighted_beam(B, cfg):
     assert np.all(x >= 0)
     assert np.linalg.norm(fit - b) <= 1e-3 * np.linalg.norm(b)
     assert np.linalg.norm(A[:, used] @ np.ones(int(used.sum())) - b) > 30 * np.linalg.norm(fit - b)   # far better than the uncommissioned model
+
+
+def test_tally_costs_little(B, cfg):
+    """The commissioning tally runs in its own kernel variant (no counters, no fingerprints): on the paper's two commissioning
+    field sizes (40x40 and 5x5 cm2) the run with the tally stays within 15 % of the plain run's time."""
+    import torch
+    c = cfg("C4")
+    psr = c["psr"]
+    dph = B.DevicePhantom(c["phantom"])
+    idx, rows = com.measurement_index(c["phantom"]["nx"], c["phantom"]["ny"], c["phantom"]["nz"], c["phantom"]["dz"], depths_cm=(1.5, 10.0, 20.0))
+    cols = com.n_columns(psr["n_ebin"], psr["n_ring"])
+    d_idx = torch.as_tensor(np.ascontiguousarray(idx.reshape(-1), np.int32)).cuda()
+    N = 50_000_000
+    for field in (40.0, 5.0):
+        jaws = dict(c["jaws"], x1=-field / 2, x2=field / 2, y1=-field / 2, y2=field / 2)
+        g = B.Psl(psr, jaws, c["n_sectors"])
+        acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
+        A = torch.zeros((cols, rows), dtype=torch.int64, device="cuda")
+        ms = {}
+        for key, opt in (("plain", {}), ("tally", dict(com_index=d_idx, com_dose=A))):
+            best = 1e30
+            for _ in range(3):
+                acc.zero_()
+                g.dose(dph, c["beams"][0], N, 77, batch=1 << 22, dose_acc=acc, **opt)
+                best = min(best, B.stats()["ms_total"])
+            ms[key] = best
+        print("commissioning tally, %gx%g cm2 field, %g histories: plain %.1f ms (%.3e histories/s), with the tally %.1f ms (%.3e histories/s)"
+              % (field, field, N, ms["plain"], N / ms["plain"] * 1e3, ms["tally"], N / ms["tally"] * 1e3))
+        assert ms["tally"] <= 1.15 * ms["plain"]
