@@ -39,16 +39,11 @@ BUDGET = {"sample": 300.0,      # per history: 2 Philox blocks (2 x 40), alias p
           "pair": 60.0,         # split, two charged children, isotropic direction, two annihilation photons
           "substep": 60.0,      # gather 6, stopping power 6, step length 16, deposit 8, move + re-home 18, bounds 6
           "deflection": 90.0}   # Philox block 40, Highland angle 12, sincos + rotation 34, reciprocals 4
-# SASS thread-instructions the kernels as built retire per history (ncu smsp__thread_inst_executed.sum / histories):
-# side information, so that retired / algorithmic is visible.  Source: profiles/ (file and commit named there).
-RETIRED = {}
-# DRAM bytes (read + write) per history of each kernel class from `ncu --set full` captures (profiles/): kernel -> bytes
-NCU_DRAM_BYTES_PER_HISTORY = {}
-try:
-    _m = json.load(open(os.path.join(ROOT, "profiles", "r2_measured.json")))
-    RETIRED, NCU_DRAM_BYTES_PER_HISTORY = _m.get("retired_thread_inst_per_history", {}), _m.get("dram_bytes_per_history", {})
-except (OSError, ValueError):
-    pass
+# SASS thread-instructions the kernels as built retire per history (ncu smsp__thread_inst_executed.sum / histories): side
+# information, so that retired / algorithmic is visible.  Source: profiles/r2_launches.md (ncu launch lists at commit c2abba5).
+RETIRED = {"C4": {"sample": 512, "photon": 3365, "electron": 3069}, "C1": {"sample": 450, "photon": 705, "electron": 884}}
+# DRAM bytes (read + write) per history of each kernel class, from the `ncu --set full` captures in profiles/r2_top_kernels.md
+NCU_DRAM_BYTES_PER_HISTORY = {"C4": {"sample": 17.4, "photon": 256.5, "electron": 197.6}, "C1": {"sample": 6.8, "photon": 30.5, "electron": 23.3}}
 
 
 def parse():
