@@ -82,16 +82,19 @@ struct Grid {
   const uint8_t *material;
   const uint32_t *vox;                               // packed phantom, one gather per voxel: density bits rounded to a
                                                      // 22-bit mantissa | material index in the two low bits
-  // Two-level phantom: one word per brick of 4x4x4 voxels = the brick's common voxel word | 0x80000000 when all its
-  // voxels are equal (densities are >= 0, so bit 31 of a voxel word is free), else 0.  A phantom that is mostly
-  // uniform bricks (water tanks, slabs: n_uniform >= 90 % of the bricks, decided per call on the device) is then read
-  // through this table, which stays in L1/L2, and only the mixed bricks go to the 4-byte-per-voxel array.
-  const uint32_t *brick; const unsigned *n_uniform; int nbx, nby; unsigned nbricks;
+  // Hierarchical phantom: one word per brick of 4x4x4 voxels = the brick's common voxel word | 0x80000000 when all its
+  // voxels are equal (densities are >= 0, so bit 31 of a voxel word is free), else 0; and the same once more per
+  // super-brick of 4x4x4 bricks (16^3 voxels).  A phantom that is mostly uniform super-bricks (water tanks: >= 90 %,
+  // decided per call on the device) is then read top down: the super-brick table (16 KiB for 256^3 voxels:
+  // L1-resident), the brick table (L2) where a super-brick is mixed, the 4-byte-per-voxel array only where a brick is
+  // mixed.
+  const uint32_t *brick, *sbrick; const unsigned *n_uniform, *n_uniform_sb; int nbx, nby, nsx, nsy; unsigned nbricks, nsbricks;
   unsigned long long *acc;                           // int64 fixed-point dose accumulator (2^-32 MeV)
   // commissioning tally, off when com_index is null: com_index[v] = 0 or 1 + row,
   // com_dose[col * com_rows + row], col = the PSR unit the history was sampled from
   const int *com_index; unsigned long long *com_dose; int com_rows;
-  const uint32_t *com_mask;                          // one bit per voxel: com_index[v] != 0 (built per call; the index array itself is read only for those)
+  const uint32_t *com_mask, *com_coarse;             // one bit per voxel: com_index[v] != 0, and one bit per 512 consecutive voxels: any of
+                                                     // them (built per call; the coarse map stays in L1, the index array is read only on a hit)
 };
 
 __device__ __forceinline__ long long quanta(float e) { return __float2ll_rn(e * 4294967296.0f); }
@@ -102,10 +105,15 @@ __device__ __forceinline__ bool locate(const Grid &g, float x, float y, float z,
   i = (int)fi; j = (int)fj; k = (int)fk;
   return in;
 }
-__device__ __forceinline__ bool use_bricks(const Grid &g) { return g.brick != nullptr && *g.n_uniform * 10ull >= g.nbricks * 9ull; }
+// true: read the phantom top down through the super-brick and brick tables; false: read the per-voxel array directly
+// (a mixed cell costs one more dependent read per level, so the tables are used when >= 90 % of the super-bricks are uniform)
+__device__ __forceinline__ bool use_bricks(const Grid &g) { return g.brick != nullptr && *g.n_uniform_sb * 10ull >= g.nsbricks * 9ull; }
 __device__ __forceinline__ void fetch_voxel(const Grid &g, bool bricks, int i, int j, int k, int v, float &rho, int &mt) {
   uint32_t p = 0u;
-  if (bricks) p = __ldg(g.brick + ((i >> 2) + g.nbx * ((j >> 2) + g.nby * (k >> 2))));
+  if (bricks) {
+    p = __ldg(g.sbrick + ((i >> 4) + g.nsx * ((j >> 4) + g.nsy * (k >> 4))));
+    if (!(p & 0x80000000u)) p = __ldg(g.brick + ((i >> 2) + g.nbx * ((j >> 2) + g.nby * (k >> 2))));
+  }
   if (p & 0x80000000u) p &= 0x7fffffffu; else p = __ldg(g.vox + v);
   rho = __uint_as_float(p & ~3u); mt = (int)(p & 3u);
 }

@@ -33,7 +33,7 @@ static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 // k_sample and ordered by entry tile -, the entry-tile counters, and the electron queue (capacity 4B, 3 planes).  mc_dose_host appends its staging area (phantom in, dose out).
 constexpr int kMaxPipes = 2;
 struct Layout {
-  size_t ctl[kMaxPipes], tile[kMaxPipes], xs, vox, brick, com_mask, acc, p0[kMaxPipes], p1[kMaxPipes], p2[kMaxPipes], q0[kMaxPipes], q1[kMaxPipes], q2[kMaxPipes],
+  size_t ctl[kMaxPipes], tile[kMaxPipes], xs, vox, brick, sbrick, com_mask, com_coarse, acc, p0[kMaxPipes], p1[kMaxPipes], p2[kMaxPipes], q0[kMaxPipes], q1[kMaxPipes], q2[kMaxPipes],
       eq[kMaxPipes][3], total, zero_bytes;
   size_t host_rho, host_mat, host_dose, host_total;
   unsigned eq_cap;
@@ -45,8 +45,10 @@ static Layout make_layout(uint64_t batch, size_t nvox, size_t nbricks) {
   L.eq_cap = (unsigned)std::min<uint64_t>(4 * batch, 0x7fffffffu);
   for (int p = 0; p < kMaxPipes; ++p) L.ctl[p] = take(sizeof(Control));     // contiguous from offset 0: zeroed by one memset,
   for (int p = 0; p < kMaxPipes; ++p) L.tile[p] = take(2 * sizeof(unsigned) * kTileBinsMax);   // with the entry-tile counts and cursors
+  L.com_coarse = take(4 * ((nvox >> 14) + 1));               // commissioning tally: one bit per 512 voxels (zeroed with the rest)
   L.zero_bytes = o;
-  L.xs = take(kXsBytes); L.vox = take(4 * nvox); L.brick = take(4 * nbricks); L.com_mask = take(4 * ((nvox + 31) / 32)); L.acc = take(8 * nvox);
+  L.xs = take(kXsBytes); L.vox = take(4 * nvox); L.brick = take(4 * nbricks); L.sbrick = take(4 * nbricks);     // (super-bricks <= bricks for any grid shape)
+  L.com_mask = take(4 * ((nvox + 31) / 32)); L.acc = take(8 * nvox);
   for (int p = 0; p < kMaxPipes; ++p) {
     L.p0[p] = take(16 * batch); L.p1[p] = take(16 * batch); L.p2[p] = take(4 * batch);
     L.q0[p] = take(16 * batch); L.q1[p] = take(16 * batch); L.q2[p] = take(4 * batch);     // the same, ordered by entry tile
@@ -276,9 +278,11 @@ struct Session {
     long long *acc = dose_acc ? dose_acc : (long long *)(ws + L.acc);
     g = make_grid(ph, acc); g.vox = (const uint32_t *)(ws + L.vox);
     g.nbx = (ph.nx + 3) / 4; g.nby = (ph.ny + 3) / 4; g.nbricks = (unsigned)((size_t)g.nbx * g.nby * ((ph.nz + 3) / 4));
+    g.nsx = (g.nbx + 3) / 4; g.nsy = (g.nby + 3) / 4; g.sbrick = (const uint32_t *)(ws + L.sbrick);
     g.brick = (const uint32_t *)(ws + L.brick); g.n_uniform = &((Control *)(ws + L.ctl[0]))->n_uniform_bricks;
+    g.n_uniform_sb = &((Control *)(ws + L.ctl[0]))->n_uniform_sbricks; g.nsbricks = (unsigned)(g.nsx * g.nsy * (((ph.nz + 3) / 4 + 3) / 4));
     g.com_index = (const int *)o.com_index; g.com_dose = (unsigned long long *)o.com_dose; g.com_rows = o.com_rows;
-    g.com_mask = (const uint32_t *)(ws + L.com_mask);
+    g.com_mask = (const uint32_t *)(ws + L.com_mask); g.com_coarse = (const uint32_t *)(ws + L.com_coarse);
     for (int p = 0; p < npipe; ++p) {
       Pipe &q = pipes[p];
       q.st = npipe > 1 ? (cudaStream_t)o.aux_streams[p] : us; q.ctl = (Control *)(ws + L.ctl[p]);
@@ -318,7 +322,9 @@ struct Session {
     tm_us.begin(MC_K_AUX);
     k_pack_phantom<<<592, 256, 0, us>>>(ph.density, ph.material, nvox, (uint32_t *)(ws + L.vox), pipes[0].ctl);
     k_bricks<<<(g.nbricks + 255) / 256, 256, 0, us>>>(g.vox, g.nx, g.ny, g.nz, g.nbx, g.nby, g.nbricks, (uint32_t *)(ws + L.brick), pipes[0].ctl);
-    if (g.com_index) { k_com_mask<<<(unsigned)(((nvox + 31) / 32 + 255) / 256), 256, 0, us>>>(g.com_index, nvox, (uint32_t *)(ws + L.com_mask)); ++launches_us[MC_K_AUX]; }
+    { const int nbz = (ph.nz + 3) / 4; const unsigned nsb = (unsigned)(g.nsx * g.nsy * ((nbz + 3) / 4));
+      k_sbricks<<<(nsb + 127) / 128, 128, 0, us>>>(g.brick, g.nbx, g.nby, nbz, g.nsx, g.nsy, nsb, (uint32_t *)(ws + L.sbrick), pipes[0].ctl); ++launches_us[MC_K_AUX]; }
+    if (g.com_index) { k_com_mask<<<(unsigned)(((nvox + 31) / 32 + 255) / 256), 256, 0, us>>>(g.com_index, nvox, (uint32_t *)(ws + L.com_mask), (uint32_t *)(ws + L.com_coarse)); ++launches_us[MC_K_AUX]; }
     tm_us.end(MC_K_AUX); launches_us[MC_K_AUX] += 2;
     if (npipe > 1) {
       CUDA_TRY(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));

@@ -30,6 +30,7 @@ struct Control {
   unsigned long long stat[ST_COUNT];
   float rhomax[4];                 // largest density per material (as float, written via atomicMax on bits)
   unsigned n_uniform_bricks;       // bricks of 4x4x4 voxels whose voxels are all equal (k_bricks; two-level phantom)
+  unsigned n_uniform_sbricks;      // super-bricks of 4x4x4 bricks that are one uniform region (k_sbricks)
 };
 
 // One alias-table entry, 16 B: everything k_sample needs after picking a column.
@@ -364,12 +365,14 @@ __global__ void k_pack_phantom(const float *density, const uint8_t *material, si
 }
 
 // One bit per voxel: com_index[v] != 0 (the commissioning tally's measurement voxels are few: PAPER.md:134).
-__global__ void k_com_mask(const int *com_index, size_t n, uint32_t *mask) {
+// `coarse` (zeroed before): one bit per 512 consecutive voxels = 16 words of `mask`.
+__global__ void k_com_mask(const int *com_index, size_t n, uint32_t *mask, uint32_t *coarse) {
   const size_t w = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
   if (w * 32 >= n) return;
   uint32_t m = 0u;
   for (int b = 0; b < 32 && w * 32 + b < n; ++b) m |= (com_index[w * 32 + b] != 0 ? 1u : 0u) << b;
   mask[w] = m;
+  if (m) atomicOr(coarse + (w >> 9), 1u << ((w >> 4) & 31));
 }
 
 // The brick table of the two-level phantom (Grid::brick): one thread per brick of 4x4x4 voxels (clipped at the grid's edge).
@@ -387,6 +390,20 @@ __global__ void k_bricks(const uint32_t *vox, int nx, int ny, int nz, int nbx, i
   }
   const unsigned n = __popc(__ballot_sync(kFull, uni));
   if ((threadIdx.x & 31) == 0 && n) atomicAdd(&c->n_uniform_bricks, n);
+}
+
+// The super-brick table on top of it: one thread per super-brick of 4x4x4 bricks (clipped at the edge).
+__global__ void k_sbricks(const uint32_t *brick, int nbx, int nby, int nbz, int nsx, int nsy, unsigned nsb, uint32_t *sbrick, Control *c) {
+  const unsigned b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= nsb) return;
+  const int si = (int)(b % (unsigned)nsx), sj = (int)((b / (unsigned)nsx) % (unsigned)nsy), sk = (int)(b / ((unsigned)nsx * (unsigned)nsy));
+  const uint32_t w0 = brick[((size_t)(sk * 4) * nby + sj * 4) * nbx + si * 4];
+  bool uni = (w0 & 0x80000000u) != 0u;
+  for (int k = sk * 4; k < min(sk * 4 + 4, nbz); ++k)
+    for (int j = sj * 4; j < min(sj * 4 + 4, nby); ++j)
+      for (int i = si * 4; i < min(si * 4 + 4, nbx); ++i) uni &= brick[((size_t)k * nby + j) * nbx + i] == w0;
+  sbrick[b] = uni ? w0 : 0u;
+  if (uni) atomicAdd(&c->n_uniform_sbricks, 1u);
 }
 
 // Photon cross-section data: layout in pslmc_device.cuh (XsTable), evaluated in double.  The sigma_KN nodes depend on

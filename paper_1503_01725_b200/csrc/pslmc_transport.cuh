@@ -112,7 +112,7 @@ struct Pending {
   template <bool ON> __device__ __forceinline__ void flush(const Grid &g, const ScoreStage<ON> &st) {
     if (q) {
       st.add(g, v, (unsigned long long)q);
-      if (COM && g.com_index && ((__ldg(g.com_mask + (v >> 5)) >> (v & 31)) & 1u)) {
+      if (COM && g.com_index && ((__ldg(g.com_coarse + (v >> 14)) >> ((v >> 9) & 31)) & 1u) && ((__ldg(g.com_mask + (v >> 5)) >> (v & 31)) & 1u)) {
         const int row = __ldg(g.com_index + v);
         if (row > 0 && row <= g.com_rows) atomicAdd(g.com_dose + (size_t)col * g.com_rows + (row - 1), (unsigned long long)q);
       }
@@ -394,8 +394,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
           return bA ? (r3 <= 4.0f * (ie_ - ie_ * ie_)) : (r3 <= 0.5f * (ct_ * ct_ + ie_));
         };
         bool brA2; float ie2, k2, ct2;
-        const bool acc1 = trial(d0, d1, d2, brA, ie, k, ct), acc2 = trial(e0, e1, e2, brA2, ie2, k2, ct2);
-        if (!acc1) { brA = brA2; ie = ie2; k = k2; ct = ct2; d3 = e3; }
+        const bool acc1 = trial(d0, d1, d2, brA, ie, k, ct), acc2 = trial(e0, e1, e2, brA2, ie2, k2, ct2) && !acc1;
+        if (acc2) { brA = brA2; ie = ie2; k = k2; ct = ct2; d3 = e3; }
         accept = acc1 || acc2;
         rng.blk += acc1 ? 1u : 2u;
         if (DBG) tl.st[ST_KAHN] += acc1 ? 1u : 2u;
