@@ -17,6 +17,7 @@ struct Queue {
 };
 
 enum { SRC_BUFFER = 0, SRC_QUEUE = 1 };
+constexpr int kPhotonRefillMin = 8;            // k_photon likewise (r2: 1 -> 8 is 2-3 % of the kernel; 12, 16: slower)
 constexpr int kElectronRefillMin = 8;          // k_electron refills in groups of >= 8 idle lanes (measured best of 1, 4, 8, 16)
 constexpr unsigned kElectronChunk = 32;        // largest source chunk a k_electron warp reserves at once
 constexpr int kXsIntervals = 4096;
@@ -301,7 +302,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
       cvox = vox_index(g, vi, vj, vk); state = PH_FLIGHT;
     }
     // ---- refill idle lanes
-    const unsigned idx = refill_index<1, 128u>(a, state == PH_IDLE, n1, count, sc, exhausted);
+    const unsigned idx = refill_index<kPhotonRefillMin, 128u>(a, state == PH_IDLE, n1, count, sc, exhausted);
     if (idx != 0xffffffffu) {
       const TrackIn t = load_track(a, idx, n1);
       if (t.ok) {

@@ -110,3 +110,36 @@ def test_finalise_units(orc):
     acc = np.array([3 << 32, 5 << 32], np.int64)
     d = orc.finalise(ph, acc, 10)
     assert d[0] == pytest.approx(3.0 / (2.0 * 0.01 * 10)) and d[1] == 0.0
+
+
+def test_dose_list_and_strict_fingerprints(orc, cfg, opsl):
+    """orc_dose_list (the tally of a chosen set of histories) equals orc_dose over the same ids; the strict fingerprint
+    (FLAG_FP_VOXELS: also voxels, accepted Kahn trial and branch, sub-step kinds) changes no result, differs from the plain
+    one exactly for the histories that deposit or scatter, and tells apart two histories the plain one cannot."""
+    c = cfg("C0")
+    o, ph = opsl("C0"), orc.Phantom(c["phantom"])
+    beam, N, seed = c["beams"][0], 100_000, 1
+    a1, r1, f1 = o.dose(ph, beam, N, seed, h_begin=2000, h_end=2600, fingerprints=True)
+    ids = np.arange(2000, 2600)
+    a2, r2, f2 = orc.dose_list(o, ph, beam, N, seed, ids, fingerprints=True)
+    assert np.array_equal(a1, a2) and np.array_equal(f1, f2) and r1 == r2
+    # a permuted, thinned list: the same per-history fingerprints, the tally of exactly those histories
+    pick = np.random.default_rng(5).permutation(ids)[:200]
+    a3, _, f3 = orc.dose_list(o, ph, beam, N, seed, pick, fingerprints=True)
+    assert np.array_equal(f3, f1[pick - 2000])
+    a4 = np.zeros_like(a3)
+    for h in pick:
+        o.dose(ph, beam, N, seed, h_begin=int(h), h_end=int(h) + 1, acc=a4)
+    assert np.array_equal(a3, a4)
+    # strict fingerprints: same tally and counters; equal to the plain ones only for histories without a deposit or scatter
+    a5, r5, f5 = o.dose(ph, beam, N, seed, h_begin=2000, h_end=2600, flags=orc.FLAG_FP_VOXELS, fingerprints=True)
+    assert np.array_equal(a1, a5) and r1 == r5
+    same = f5 == f1
+    assert 0.2 < same.mean() < 0.8                              # jaw-rejected / missed / escaped-uncollided histories hash the same
+    for h in np.flatnonzero(same)[:20]:
+        t = np.zeros_like(a1)
+        o.dose(ph, beam, N, seed, h_begin=2000 + int(h), h_end=2001 + int(h), acc=t)
+        assert not t.any()                                      # ... and they deposit nothing
+    for h in np.flatnonzero(~same)[:20]:
+        _, rr, _ = o.dose(ph, beam, N, seed, h_begin=2000 + int(h), h_end=2001 + int(h))
+        assert rr["n_deposits"] > 0 or rr["n_compton"] > 0
