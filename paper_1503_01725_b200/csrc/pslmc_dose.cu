@@ -296,10 +296,7 @@ struct Session {
     // When the packed phantom + int64 grid (12 B per voxel) do not fit L2 the kernels are bound by random DRAM sectors and
     // fewer resident warps thrash less: measured on C4 (201 MB) 56.8 ms per 1e8 histories at 1.0, 53.1 at 0.75.
     const bool big = 12.0 * (double)nvox > 110e6;
-#ifndef PSLMC_GRID_SCALE_BIG
-#define PSLMC_GRID_SCALE_BIG 0.75
-#endif
-    init_blocks(big ? PSLMC_GRID_SCALE_BIG : 1.0);
+    init_blocks(big ? 0.75 : 1.0);                  // (r2, with the hierarchical phantom: 0.65 / 0.85 / 1.0 on C4 and 0.5-0.75 elsewhere are all slower)
     { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
     // Entry-tile ordering of every batch (the spatial inner loop): MC_FLAG_TILE_SORT.  Off by default:
     // measured on C4 it takes 10 % off the transport kernels' time and costs as much in the sort - photons
