@@ -127,3 +127,17 @@ def test_two_rank_sharding_is_bit_exact_gloo(tmp_path):
     outs = [p.communicate(timeout=300) for p in procs]
     assert all(p.returncode == 0 for p in procs), outs
     assert "OK" in outs[0][0]
+
+
+def test_flag_and_error_constants_match_header(binding):
+    """The binding's MC_FLAG_* / MC_ORDER_* values are the header's #defines (a mirror typed twice must not drift)."""
+    import re
+    text = open(os.path.join(ROOT, "include", "pslmc.h")).read()
+    defs = {m.group(1): int(m.group(2)) for m in re.finditer(r"#define\s+(MC_[A-Z_0-9]+)\s+(-?\d+)", text)}
+    flags = [k for k in defs if k.startswith("MC_FLAG_") or k.startswith("MC_ORDER_")]
+    assert len(flags) >= 11
+    for k in flags:
+        assert getattr(binding, k) == defs[k], k
+    assert defs["MC_E_WORKSPACE"] == -3 and defs["MC_E_OVERFLOW"] == -5 and defs["MC_OK"] == 0
+    vals = [defs[k] for k in defs if k.startswith("MC_FLAG_")]
+    assert len(set(vals)) == len(vals) and all(v & (v - 1) == 0 for v in vals)         # distinct single bits
