@@ -59,7 +59,7 @@ def parse():
     ap.add_argument("--no-all-configs", action="store_true", help="time the headline workload only")
     ap.add_argument("--order", default="sorted", choices=["sorted", "mixed"])
     ap.add_argument("--static-lanes", action="store_true")
-    ap.add_argument("--tile-sort", default="auto", choices=["auto", "on", "off"])
+    ap.add_argument("--tile-sort", default="off", choices=["on", "off"], help="ablation: order every batch by entry tile (MC_FLAG_TILE_SORT)")
     ap.add_argument("--pipelines", type=int, default=0, help="0 = two overlapping launch sequences, 1 = serial")
     return ap.parse_args()
 
@@ -225,7 +225,7 @@ class Workload:
         self.ws = B.workspace(self.psl.workspace_bytes(self.ph, args.batch, host=True))
         self.order = B.MC_ORDER_MIXED if args.order == "mixed" else B.MC_ORDER_SORTED
         self.flags = B.MC_FLAG_TIMING | (B.MC_FLAG_STATIC_LANES if args.static_lanes else 0) | \
-            {"auto": 0, "on": B.MC_FLAG_TILE_SORT, "off": B.MC_FLAG_NO_TILE_SORT}[args.tile_sort]
+            {"on": B.MC_FLAG_TILE_SORT, "off": 0}[args.tile_sort]
         self.hb, self.he = B.shard_range(self.n_total, rank, world)
         self.stream = torch.cuda.current_stream()
 

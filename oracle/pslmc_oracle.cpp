@@ -15,7 +15,8 @@
 //   sample_history      PAPER.md:82-92 S3 Eq. 4-5, :94-116 S4-S5 (focal geometry reading, or Eq. 6-7 as printed: NEXT-2), jaws :65/:92
 //   photon / electron   PAPER.md:161 (cut-offs); P1-P9 (Woodcock, Kahn, CSDA + Gaussian MS)
 //   deposit / ledgers   DESIGN.md S1 (int64 fixed point, 2^-32 MeV); commissioning tally PAPER.md:132-138 (NEXT-3)
-//   fingerprints        DESIGN.md F1
+//   fingerprints        DESIGN.md F1 (plain: the interaction sequence; FLAG_FP_VOXELS: the strict form used by the every-voxel parity test)
+//   orc_dose_list       the same path over a LIST of history ids (the tally of the diverged histories in that test); no arithmetic of its own
 //
 // Pins (tests/test_oracle_*.py, all `-m "not gpu"`): Philox vs cuRAND's host generator; ring/sector
 // weights vs closed forms; alias reconstruction; chi-square of sampled spectrum / fluence vs the
