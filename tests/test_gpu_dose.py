@@ -431,3 +431,24 @@ def test_full_size_sampled_parity_c2_c3_c4(name, beam, seed, B, orc, cfg):
     _, _, ofp = o.dose(oph, c["beams"][beam], N, seed, h_begin=N - 1000, h_end=N, acc=oacc, fingerprints=True)
     same += int((fp[N - 1000:].cpu().numpy().view(np.uint64) == ofp).sum()); total += 1000
     assert same / total >= 0.999, same / total
+
+
+def test_hierarchical_phantom_on_odd_grids(B, orc, cfg):
+    """The brick / super-brick tables on grids whose sizes are no multiples of 4 or 16 (clipped cells at the edges), uniform
+    (read through the tables) and with one foreign voxel per super-brick (mostly mixed super-bricks: read directly), and a slab
+    phantom whose faces cut through bricks: sequences, counters, ledgers and dose as the oracle's in all three."""
+    c = cfg("C1", False)
+    g, o = B.Psl(c["psr"], c["jaws"], 16), orc.Psl(c["psr"], c["jaws"], 16)
+    nx, ny, nz = 37, 26, 45
+    base = dict(nx=nx, ny=ny, nz=nz, dx=0.4, dy=0.5, dz=0.3, ox=-7.4, oy=-6.5, oz=0.0)
+    rho = np.ones((nz, ny, nx), np.float32); mat = np.zeros((nz, ny, nx), np.uint8)
+    uniform = dict(base, density=rho.reshape(-1).copy(), material=mat.reshape(-1).copy())
+    compare_with_oracle(B, orc, g, o, uniform, c["beams"][0], 200_000, 21, batch=1 << 15, frac_vox=0.98)
+    rho2 = rho.copy(); rho2[::16, ::16, ::16] = 1.0001                     # one voxel per super-brick differs: every super-brick mixed
+    speck = dict(base, density=rho2.reshape(-1).copy(), material=mat.reshape(-1).copy())
+    compare_with_oracle(B, orc, g, o, speck, c["beams"][0], 200_000, 21, batch=1 << 15, frac_vox=0.98)
+    rho3 = rho.copy(); mat3 = mat.copy()
+    rho3[10:17], mat3[10:17] = 1.85, 2                                     # slab faces inside bricks (10, 17 are no multiples of 4)
+    rho3[17:30], mat3[17:30] = 0.26, 1
+    slab = dict(base, density=rho3.reshape(-1).copy(), material=mat3.reshape(-1).copy())
+    compare_with_oracle(B, orc, g, o, slab, c["beams"][0], 200_000, 22, batch=1 << 15, frac_vox=0.98)
