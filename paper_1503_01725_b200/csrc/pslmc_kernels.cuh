@@ -29,7 +29,7 @@ struct Control {
   unsigned long long ledger[kLedgerSlots][4][2];   // [slot][incident,deposited,escaped,jaw][lo,hi] quanta
   unsigned long long stat[ST_COUNT];
   float rhomax[4];                 // largest density per material (as float, written via atomicMax on bits)
-  unsigned n_uniform_bricks;       // bricks of 4x4x4 voxels whose voxels are all equal (k_bricks; two-level phantom)
+  unsigned n_uniform_bricks;       // bricks of 4x4x4 voxels whose voxels are all equal (k_bricks; hierarchical phantom)
   unsigned n_uniform_sbricks;      // super-bricks of 4x4x4 bricks that are one uniform region (k_sbricks)
 };
 
