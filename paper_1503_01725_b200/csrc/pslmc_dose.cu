@@ -309,7 +309,7 @@ struct Session {
       while ((long long)nt(ph.nx) * nt(ph.ny) * nt(ph.nz) > kTileBinsMax) ++sh;
       tm.shift = sh; tm.ntx = nt(ph.nx); tm.nty = nt(ph.ny); tm.nbins = tm.ntx * tm.nty * nt(ph.nz);
     }
-    blocks_sample = persistent_blocks(k_sample, sizeof(unsigned) * tm.nbins, 0.6);      // (3 of 5 possible CTAs per SM: 8 % faster than a full wave - fewer warps on the buffer-tail atomic)
+    blocks_sample = persistent_blocks(k_sample, sizeof(unsigned) * tm.nbins, 0.6);      // (3 of the 5 possible CTAs per SM: 0-8 % faster than a full wave in the probes - fewer warps on the buffer-tail atomic)
     rhomax = pipes[0].ctl->rhomax;
     CUDA_TRY(cudaEventCreate(&ev0)); CUDA_TRY(cudaEventCreate(&ev1));
     CUDA_TRY(cudaEventRecord(ev0, us));
