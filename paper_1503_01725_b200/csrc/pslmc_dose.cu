@@ -309,7 +309,7 @@ struct Session {
       while ((long long)nt(ph.nx) * nt(ph.ny) * nt(ph.nz) > kTileBinsMax) ++sh;
       tm.shift = sh; tm.ntx = nt(ph.nx); tm.nty = nt(ph.ny); tm.nbins = tm.ntx * tm.nty * nt(ph.nz);
     }
-    blocks_sample = persistent_blocks(k_sample, sizeof(unsigned) * tm.nbins, 0.6);      // (3 of the 5 possible CTAs per SM: 0-8 % faster than a full wave in the probes - fewer warps on the buffer-tail atomic)
+    blocks_sample = persistent_blocks(k_sample, sizeof(unsigned) * tm.nbins, 1.0);      // (70 registers: 3 CTAs per SM)
     rhomax = pipes[0].ctl->rhomax;
     CUDA_TRY(cudaEventCreate(&ev0)); CUDA_TRY(cudaEventCreate(&ev1));
     CUDA_TRY(cudaEventRecord(ev0, us));
@@ -349,7 +349,7 @@ struct Session {
       sa.p2 = g.com_index ? p.p2 : nullptr;
       sa.tm = tm; sa.tile_count = tm.nbins ? p.tile_count : nullptr;
       p.tm.begin(MC_K_SAMPLE);
-      const unsigned nblk = (unsigned)std::min<uint64_t>((count + kThreads - 1) / kThreads, (uint64_t)blocks_sample);     // persistent: one wave
+      const unsigned nblk = (unsigned)std::min<uint64_t>((count + 2 * kThreads - 1) / (2 * kThreads), (uint64_t)blocks_sample);     // persistent; a CTA takes 512 histories per iteration
       k_sample<<<nblk, kThreads, sizeof(unsigned) * tm.nbins, p.st>>>(sa);
       if (tm.nbins) {                                     // counting sort of the survivors by entry tile: counts -> cursors -> moves
         k_tile_scan<<<1, 1024, 0, p.st>>>(p.tile_count, p.tile_cursor, tm.nbins);
@@ -634,7 +634,7 @@ extern "C" int mc_sample_debug(const psl_t *P, const beam_geom_t *beam, uint64_t
   sa.seed = seed; round_keys(seed, sa.ks); sa.first = first_history; sa.n_total = n_histories; sa.perm_a = 0; sa.count = (unsigned)count;
   sa.p0 = (float4 *)soa_out; sa.p1 = (float4 *)soa_out + count; sa.ctl = nullptr; sa.fp = nullptr; sa.compact = 0;
   int sms = 1; cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P->device);
-  k_sample<<<(unsigned)std::min<uint64_t>((count + kThreads - 1) / kThreads, (uint64_t)sms * 8), kThreads, 0, st>>>(sa);
+  k_sample<<<(unsigned)std::min<uint64_t>((count + 2 * kThreads - 1) / (2 * kThreads), (uint64_t)sms * 8), kThreads, 0, st>>>(sa);
   CUDA_TRY(cudaGetLastError());
   CUDA_TRY(cudaStreamSynchronize(st));
   return MC_OK;

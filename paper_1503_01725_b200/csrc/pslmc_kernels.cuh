@@ -100,7 +100,7 @@ __device__ __forceinline__ unsigned tile_bin(const TileMap &tm, int vi, int vj, 
 }
 
 // ------------------------------------------------------------------ k_sample
-// Persistent grid: a thread samples histories t = blockIdx.x*kThreads + threadIdx.x + i*gridDim.x*kThreads.  The
+// Persistent grid: a thread samples histories t = blockIdx.x*2*kThreads + {0, kThreads} + threadIdx.x + i*gridDim.x*2*kThreads.  The
 // (sub-source, energy bin) group of a history is found once per thread and then walked forward (sorted order:
 // history ids only grow), ledgers are summed in registers and flushed once per warp at the end: no barrier in the loop.
 __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ SampleArgs a) {
@@ -115,8 +115,12 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
   unsigned long long q_inc = 0, q_jaw = 0, q_esc = 0;
   unsigned n_miss = 0;
   int g = -1;                                              // group of the thread's previous history (sorted order)
-  for (unsigned t0 = blockIdx.x * kThreads; t0 < a.count; t0 += gridDim.x * kThreads) {
-  const unsigned t = t0 + threadIdx.x;
+  // two histories per thread and iteration (t and t + kThreads): one buffer-tail atomic per 64 histories of a warp
+  for (unsigned t0 = blockIdx.x * (2 * kThreads); t0 < a.count; t0 += gridDim.x * (2 * kThreads)) {
+  float4 O0[2], O1[2]; bool mine[2]; unsigned bins[2]; uint32_t cols[2];
+#pragma unroll
+  for (int rep = 0; rep < 2; ++rep) {
+  const unsigned t = t0 + rep * kThreads + threadIdx.x;
   const bool live = t < a.count;
   bool pass = false;
   float4 o0 = make_float4(0.f, 0.f, 0.f, 0.f), o1 = o0;
@@ -234,22 +238,29 @@ __global__ void __launch_bounds__(kThreads) k_sample(const __grid_constant__ Sam
     }
   }
   if (a.compact) {
-    // survivors packed with one queue-tail atomic per warp (pipelining the stores behind the atomic's latency was
-    // measured: no gain - the kernel is bound by instruction issue)
-    const unsigned keep = __ballot_sync(kFull, live && pass);
-    unsigned base = 0;
-    if (lane == 0 && keep) base = atomicAdd(&a.ctl->n_pb, __popc(keep));
-    base = __shfl_sync(kFull, base, 0);
-    if (live && pass) {
-      const unsigned dst = base + __popc(keep & ((1u << lane) - 1u));
-      o1.w = __uint_as_float(t | ((unsigned)ptype << 31));
-      __stcs(a.p0 + dst, o0); __stcs(a.p1 + dst, o1);         // write-once / read-once: streaming, keeps L2 for the phantom and the grid
-      if (a.p2) a.p2[dst] = com_col;
-      if (tiles) atomicAdd(&s_hist[bin], 1u);
-    }
+    o1.w = __uint_as_float(t | ((unsigned)ptype << 31));
+    O0[rep] = o0; O1[rep] = o1; mine[rep] = live && pass; bins[rep] = bin; cols[rep] = com_col;
   } else if (live) {
     o1.w = pass ? (float)g : -(float)g - 1.0f;
     a.p0[t] = o0; a.p1[t] = o1;
+  }
+  }
+  if (a.compact) {
+    // survivors of both histories packed with ONE queue-tail atomic per warp (deferring the stores behind the atomic's
+    // latency was measured: no gain)
+    const unsigned keep0 = __ballot_sync(kFull, mine[0]), keep1 = __ballot_sync(kFull, mine[1]);
+    const unsigned n0 = __popc(keep0), tot = n0 + __popc(keep1);
+    unsigned base = 0;
+    if (lane == 0 && tot) base = atomicAdd(&a.ctl->n_pb, tot);
+    base = __shfl_sync(kFull, base, 0);
+#pragma unroll
+    for (int rep = 0; rep < 2; ++rep)
+      if (mine[rep]) {
+        const unsigned dst = base + (rep ? n0 : 0u) + __popc((rep ? keep1 : keep0) & ((1u << lane) - 1u));
+        __stcs(a.p0 + dst, O0[rep]); __stcs(a.p1 + dst, O1[rep]);         // write-once / read-once: streaming, keeps L2 for the phantom and the grid
+        if (a.p2) a.p2[dst] = cols[rep];
+        if (tiles) atomicAdd(&s_hist[bins[rep]], 1u);
+      }
   }
   }
   // ledgers: incident, jaw-rejected and escaped (missed) energy, one 128-bit add per warp and ledger, spread over slots
