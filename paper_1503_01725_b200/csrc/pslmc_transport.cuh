@@ -19,7 +19,7 @@ struct Queue {
 enum { SRC_BUFFER = 0, SRC_QUEUE = 1 };
 constexpr int kPhotonRefillMin = 8;            // k_photon likewise (r2: 1 -> 8 is 2-3 % of the kernel; 12, 16: slower)
 constexpr int kElectronRefillMin = 8;          // k_electron refills in groups of >= 8 idle lanes (measured best of 1, 4, 8, 16)
-constexpr unsigned kElectronChunk = 32;        // largest source chunk a k_electron warp reserves at once
+constexpr unsigned kElectronChunk = 64;        // largest source chunk a k_electron warp reserves at once (r2: 32 -> 64 is 6 % of the kernel on C4: the cursor is one address for all warps)
 constexpr int kXsIntervals = 4096;
 constexpr size_t kAnnihBytes = 2 * sizeof(float4) * kThreads;   // k_photon: one pending annihilation photon per lane
 constexpr size_t kXsBytes = sizeof(float) * (kXsHead + kXsIntervals + 4);     // head + n + 1 nodes, padded to 16 bytes
