@@ -318,9 +318,9 @@ struct Session {
     tm_us.on = timing; tm_us.st = us;
     tm_us.begin(MC_K_AUX);
     k_pack_phantom<<<592, 256, 0, us>>>(ph.density, ph.material, nvox, (uint32_t *)(ws + L.vox), pipes[0].ctl);
-    k_bricks<<<(g.nbricks + 7) / 8, 256, 0, us>>>(g.vox, g.nx, g.ny, g.nz, g.nbx, g.nby, g.nbricks, (uint32_t *)(ws + L.brick), pipes[0].ctl);
+    k_bricks<<<(g.nbricks + 63) / 64, 64, 0, us>>>(g.vox, g.nx, g.ny, g.nz, g.nbx, g.nby, g.nbricks, (uint32_t *)(ws + L.brick), pipes[0].ctl);
     { const int nbz = (ph.nz + 3) / 4; const unsigned nsb = (unsigned)(g.nsx * g.nsy * ((nbz + 3) / 4));
-      k_sbricks<<<(nsb + 7) / 8, 256, 0, us>>>(g.brick, g.nbx, g.nby, nbz, g.nsx, g.nsy, nsb, (uint32_t *)(ws + L.sbrick), pipes[0].ctl); ++launches_us[MC_K_AUX]; }
+      k_sbricks<<<(nsb + 31) / 32, 32, 0, us>>>(g.brick, g.nbx, g.nby, nbz, g.nsx, g.nsy, nsb, (uint32_t *)(ws + L.sbrick), pipes[0].ctl); ++launches_us[MC_K_AUX]; }
     if (g.com_index) { k_com_mask<<<(unsigned)(((nvox + 31) / 32 + 255) / 256), 256, 0, us>>>(g.com_index, nvox, (uint32_t *)(ws + L.com_mask), (uint32_t *)(ws + L.com_coarse)); ++launches_us[MC_K_AUX]; }
     tm_us.end(MC_K_AUX); launches_us[MC_K_AUX] += 2;
     if (npipe > 1) {

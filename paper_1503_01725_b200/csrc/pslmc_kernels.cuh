@@ -386,37 +386,46 @@ __global__ void k_com_mask(const int *com_index, size_t n, uint32_t *mask, uint3
   if (m) atomicOr(coarse + (w >> 9), 1u << ((w >> 4) & 31));
 }
 
-// The brick table of the hierarchical phantom (Grid::brick): one WARP per brick of 4x4x4 voxels (clipped at the grid's
-// edge), two voxels per lane.
-__global__ void k_bricks(const uint32_t *vox, int nx, int ny, int nz, int nbx, int nby, unsigned nbricks, uint32_t *brick, Control *c) {
-  const unsigned b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31u;
-  if (b >= nbricks) return;                                // (whole warps)
-  const int bi = (int)(b % (unsigned)nbx), bj = (int)((b / (unsigned)nbx) % (unsigned)nby), bk = (int)(b / ((unsigned)nbx * (unsigned)nby));
-  const uint32_t w0 = vox[((size_t)(bk * 4) * ny + bj * 4) * nx + bi * 4];
-  bool same = true;
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    const int t = (int)lane + 32 * h, i = bi * 4 + (t & 3), j = bj * 4 + ((t >> 2) & 3), k = bk * 4 + (t >> 4);
-    if (i < nx && j < ny && k < nz) same &= vox[((size_t)k * ny + j) * nx + i] == w0;
-  }
-  const bool uni = __all_sync(kFull, same);
-  if (lane == 0) { brick[b] = uni ? (w0 | 0x80000000u) : 0u; if (uni) atomicAdd(&c->n_uniform_bricks, 1u); }
+// "All words of the 4x4x4 cell at (ci, cj, ck) of an array of (n0, n1, n2) words equal w0" - rows of four words are read as
+// one 16-byte load when they are aligned (n0 a multiple of 4) and the cell is not clipped in x.
+__device__ __forceinline__ bool cell_uniform(const uint32_t *w, int n0, int n1, int n2, int ci, int cj, int ck, uint32_t w0) {
+  bool uni = true;
+  const bool vec = (n0 & 3) == 0;                              // (then ci*4 + 4 <= n0 as well)
+  for (int k = ck * 4; k < min(ck * 4 + 4, n2); ++k)
+    for (int j = cj * 4; j < min(cj * 4 + 4, n1); ++j) {
+      const size_t row = ((size_t)k * n1 + j) * n0 + ci * 4;
+      if (vec) { const uint4 q = *reinterpret_cast<const uint4 *>(w + row); uni &= q.x == w0 && q.y == w0 && q.z == w0 && q.w == w0; }
+      else for (int i = 0; i < min(4, n0 - ci * 4); ++i) uni &= w[row + i] == w0;
+    }
+  return uni;
 }
 
-// The super-brick table on top of it: one warp per super-brick of 4x4x4 bricks (clipped at the edge).
-__global__ void k_sbricks(const uint32_t *brick, int nbx, int nby, int nbz, int nsx, int nsy, unsigned nsb, uint32_t *sbrick, Control *c) {
-  const unsigned b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31u;
-  if (b >= nsb) return;
-  const int si = (int)(b % (unsigned)nsx), sj = (int)((b / (unsigned)nsx) % (unsigned)nsy), sk = (int)(b / ((unsigned)nsx * (unsigned)nsy));
-  const uint32_t w0 = brick[((size_t)(sk * 4) * nby + sj * 4) * nbx + si * 4];
-  bool same = (w0 & 0x80000000u) != 0u;
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    const int t = (int)lane + 32 * h, i = si * 4 + (t & 3), j = sj * 4 + ((t >> 2) & 3), k = sk * 4 + (t >> 4);
-    if (i < nbx && j < nby && k < nbz) same &= brick[((size_t)k * nby + j) * nbx + i] == w0;
+// The brick table of the hierarchical phantom (Grid::brick): one thread per brick of 4x4x4 voxels (clipped at the grid's edge).
+__global__ void k_bricks(const uint32_t *vox, int nx, int ny, int nz, int nbx, int nby, unsigned nbricks, uint32_t *brick, Control *c) {
+  const unsigned b = blockIdx.x * blockDim.x + threadIdx.x;
+  bool uni = false;
+  if (b < nbricks) {
+    const int bi = (int)(b % (unsigned)nbx), bj = (int)((b / (unsigned)nbx) % (unsigned)nby), bk = (int)(b / ((unsigned)nbx * (unsigned)nby));
+    const uint32_t w0 = vox[((size_t)(bk * 4) * ny + bj * 4) * nx + bi * 4];
+    uni = cell_uniform(vox, nx, ny, nz, bi, bj, bk, w0);
+    brick[b] = uni ? (w0 | 0x80000000u) : 0u;
   }
-  const bool uni = __all_sync(kFull, same);
-  if (lane == 0) { sbrick[b] = uni ? w0 : 0u; if (uni) atomicAdd(&c->n_uniform_sbricks, 1u); }
+  const unsigned n = __popc(__ballot_sync(kFull, uni));
+  if ((threadIdx.x & 31) == 0 && n) atomicAdd(&c->n_uniform_bricks, n);
+}
+
+// The super-brick table on top of it: one thread per super-brick of 4x4x4 bricks (clipped at the edge).
+__global__ void k_sbricks(const uint32_t *brick, int nbx, int nby, int nbz, int nsx, int nsy, unsigned nsb, uint32_t *sbrick, Control *c) {
+  const unsigned b = blockIdx.x * blockDim.x + threadIdx.x;
+  bool uni = false;
+  if (b < nsb) {
+    const int si = (int)(b % (unsigned)nsx), sj = (int)((b / (unsigned)nsx) % (unsigned)nsy), sk = (int)(b / ((unsigned)nsx * (unsigned)nsy));
+    const uint32_t w0 = brick[((size_t)(sk * 4) * nby + sj * 4) * nbx + si * 4];
+    uni = (w0 & 0x80000000u) != 0u && cell_uniform(brick, nbx, nby, nbz, si, sj, sk, w0);
+    sbrick[b] = uni ? w0 : 0u;
+  }
+  const unsigned n = __popc(__ballot_sync(kFull, uni));
+  if ((threadIdx.x & 31) == 0 && n) atomicAdd(&c->n_uniform_sbricks, n);
 }
 
 // Photon cross-section data: layout in pslmc_device.cuh (XsTable), evaluated in double.  The sigma_KN nodes depend on
