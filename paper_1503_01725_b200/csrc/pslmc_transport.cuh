@@ -131,56 +131,70 @@ __device__ __forceinline__ void finish_track(const TransportArgs &a, unsigned lo
   if (DBG && a.fp) atomicAdd(a.fp + (h - a.fp_base), f.v);
 }
 
-// Warp-aggregated push through a per-warp shared-memory ring of 64 entries: lanes with `want` append
-// at consecutive ring positions (ballot + prefix sum); whenever the ring holds >= 32 entries the warp
-// takes 32 consecutive queue slots with ONE tail atomic and writes them as three coalesced 512-byte
-// rows.  No atomic and no global store in the common iteration; no holes in the queue.  Convergent calls.
+// Warp-aggregated push through a per-warp shared-memory ring of 64 entries: lanes with `want` append at consecutive ring
+// positions (ballot + prefix sum); whenever the ring holds >= 32 entries the warp writes 32 of them to the queue as three
+// coalesced 512-byte rows.  Queue slots are taken 64 at a time with ONE tail atomic (two flushes per atomic: the tail is
+// one address for every warp of the launch, and halving the atomics on it is worth more than the few null entries it
+// costs); the half of a reservation a warp has not used when the kernel ends is filled with null entries (energy 0),
+// which the consumer skips.  No atomic and no global store in the common iteration.  Convergent calls.
 struct StageRing { float4 a[64], b[64]; uint4 c[64]; };           // 3 KiB per warp
-struct StageCursor { unsigned head, n, base_raw; bool pending; };
-// The flush is split in two so that the tail atomic's latency is not waited for: stage_reserve issues
-// the atomic for 32 slots (result left in lane 0's register), stage_complete - one loop iteration later,
-// or at kernel exit - broadcasts it and writes the 32 oldest ring entries.
+struct StageCursor { unsigned head, n, base_raw, base, have; bool pending; };     // have: reserved slots not written yet (at `base`)
+// The atomic's latency is not waited for: stage_reserve issues it (result left in lane 0's register), stage_resolve -
+// one loop iteration later, or at kernel exit - broadcasts it.
 __device__ __forceinline__ void stage_reserve(const Queue &q, StageCursor &sc, unsigned n_out) {
   if ((threadIdx.x & 31u) == 0) sc.base_raw = atomicAdd(q.count, n_out);
-  sc.pending = true;
+  sc.pending = true; sc.have = n_out;
 }
-__device__ __forceinline__ void stage_complete(const Queue &q, Control *ctl, StageRing &r, StageCursor &sc, unsigned n_out) {
+__device__ __forceinline__ void stage_resolve(const Queue &q, Control *ctl, StageCursor &sc) {
+  sc.base = __shfl_sync(kFull, sc.base_raw, 0);
+  if (sc.base + sc.have > q.cap) { atomicOr(&ctl->overflow, 1u); sc.base = 0xffffffffu; }   // dropped whole; k_electron does not run on a queue that overflowed
+  sc.pending = false;
+}
+// Writes the n_real oldest ring entries (and null entries up to n_out) to the next n_out reserved slots.
+__device__ __forceinline__ void stage_write(const Queue &q, StageRing &r, StageCursor &sc, unsigned n_real, unsigned n_out) {
   const unsigned lane = threadIdx.x & 31u;
   __syncwarp();
-  const unsigned base = __shfl_sync(kFull, sc.base_raw, 0);
-  if (base + n_out > q.cap) atomicOr(&ctl->overflow, 1u);      // dropped whole; k_electron does not run on a queue that overflowed
-  else if (lane < n_out) {
+  if (sc.base != 0xffffffffu && lane < n_out) {
     const unsigned p = (sc.head + lane) & 63u;
-    __stcs(q.a + base + lane, r.a[p]); __stcs(q.b + base + lane, r.b[p]); __stcs(q.c + base + lane, r.c[p]);   // write-once / read-once: streaming
+    const bool real = lane < n_real;
+    // a null entry: an electron of 1e-30 MeV at a real entry's place - k_electron ends it in its first sub-step with a
+    // deposit of 0 quanta (plain and commissioning variants only: with counters or fingerprints no half is left open)
+    float4 A = r.a[real ? p : ((sc.head + sc.n - 1u) & 63u)]; if (!real) A.w = 1e-30f;
+    __stcs(q.a + sc.base + lane, A);                                                        // write-once / read-once: streaming
+    __stcs(q.b + sc.base + lane, real ? r.b[p] : make_float4(0.f, 0.f, 1.f, 0.f));
+    __stcs(q.c + sc.base + lane, real ? r.c[p] : make_uint4(0u, 0u, 0u, 0u));
   }
-  sc.head = (sc.head + n_out) & 63u; sc.n -= n_out; sc.pending = false;
+  if (sc.base != 0xffffffffu) sc.base += n_out;
+  sc.have -= n_out; sc.head = (sc.head + n_real) & 63u; sc.n -= n_real;
   __syncwarp();
 }
-// One call per loop iteration (convergent): finishes the flush reserved in the previous iteration, appends
-// this iteration's entries, and reserves the next flush once 32 are staged.  The ring never holds more
-// than 31 + 32 entries.
+// One call per loop iteration (convergent): resolves the reservation issued in the previous iteration, writes 32 entries
+// when the ring holds that many and slots are at hand, appends this iteration's entries, and reserves 64 more slots once
+// 32 entries are staged without any.  The ring never holds more than 31 + 32 entries.
 __device__ __forceinline__ void stage_push(const Queue &q, Control *ctl, StageRing &r, StageCursor &sc, bool want,
-                                           float4 A, float4 B, uint4 C) {
-  if (sc.pending) stage_complete(q, ctl, r, sc, 32u);
+                                           float4 A, float4 B, uint4 C, bool big) {
+  if (sc.n >= 32u && sc.have) { if (sc.pending) stage_resolve(q, ctl, sc); stage_write(q, r, sc, 32u, 32u); }
   const unsigned m = __ballot_sync(kFull, want);
-  if (!m) return;
-  const unsigned lane = threadIdx.x & 31u;
-  if (want) {
-    const unsigned p = (sc.head + sc.n + __popc(m & ((1u << lane) - 1u))) & 63u;
-    r.a[p] = A; r.b[p] = B; r.c[p] = C;
+  if (m) {
+    const unsigned lane = threadIdx.x & 31u;
+    if (want) {
+      const unsigned p = (sc.head + sc.n + __popc(m & ((1u << lane) - 1u))) & 63u;
+      r.a[p] = A; r.b[p] = B; r.c[p] = C;
+    }
+    sc.n += __popc(m);
   }
-  sc.n += __popc(m);
-  if (sc.n >= 32u) stage_reserve(q, sc, 32u);
+  if (sc.n >= 32u && !sc.have) stage_reserve(q, sc, big ? 64u : 32u);      // (big: the warp still has source to come, so the second half will be used)
 }
 __device__ __forceinline__ void stage_drain(const Queue &q, Control *ctl, StageRing &r, StageCursor &sc) {
-  if (sc.pending) stage_complete(q, ctl, r, sc, 32u);
-  if (sc.n) { const unsigned n = sc.n; stage_reserve(q, sc, n); stage_complete(q, ctl, r, sc, n); }
+  if (sc.pending) stage_resolve(q, ctl, sc);
+  while (sc.have) { const unsigned k = min(sc.n, 32u); stage_write(q, r, sc, k, 32u); }     // open halves: what is staged, then nulls
+  if (sc.n) { const unsigned n = sc.n; stage_reserve(q, sc, n); stage_resolve(q, ctl, sc); stage_write(q, r, sc, n, n); }
 }
 // Refill protocol shared by both kernels: lanes without a track take the next source indices.  A warp
 // takes `chunk` consecutive indices from the source cursor with ONE atomic and hands them out over
 // the next refills (warp-uniform cursor in `sc`).  Returns the source index for this lane or
 // 0xffffffff.  `exhausted` becomes true (warp-uniform) once the cursor passed the end.
-struct SrcCursor { unsigned next, end; };
+struct SrcCursor { unsigned next, end, chunk; };          // chunk: size of the last reservation (shrinks towards the end of the source)
 // Guided self-scheduling: the chunk shrinks with what was left at the warp's previous grab, so the
 // last chunks are small and the warps finish together.
 template <unsigned MAX_CHUNK>
@@ -213,7 +227,7 @@ __device__ __forceinline__ unsigned refill_index(const TransportArgs &a, bool id
     if (lane == 0) base = atomicAdd(a.src_head, chunk);
     base = __shfl_sync(kFull, base, 0);
     if (base >= count) { exhausted = true; return 0xffffffffu; }
-    sc.next = base; sc.end = min(base + chunk, count);
+    sc.next = base; sc.end = min(base + chunk, count); sc.chunk = chunk;
     prefetch_chunk(a, n1, sc.next, sc.end);
   }
   const unsigned rank = __popc(need & ((1u << lane) - 1u)), avail = sc.end - sc.next;
@@ -278,9 +292,9 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
   const bool bricks = use_bricks(g);
   const unsigned n1 = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
   const unsigned count = n1;
-  SrcCursor sc; sc.next = sc.end = 0u;
+  SrcCursor sc; sc.next = sc.end = sc.chunk = 0u;
   StageRing &ring = *reinterpret_cast<StageRing *>(s_raw + kXsBytes + sizeof(StageRing) * (threadIdx.x >> 5));
-  StageCursor stg; stg.head = stg.n = stg.base_raw = 0u; stg.pending = false;
+  StageCursor stg; stg.head = stg.n = stg.base_raw = stg.base = stg.have = 0u; stg.pending = false;
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
   Pending<COM> pend; pend.v = 0; pend.q = 0; pend.col = 0u;
@@ -440,8 +454,9 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
       }
     }
     // ---- secondaries, convergent: Compton electrons through the staging ring ...
+    const bool big = !DBG && !exhausted && sc.chunk >= 128u;   // not in the tail of the source: queue slots are taken 64 at a time
     stage_push(a.eq, a.ctl, ring, stg, push_e, make_float4(x, y, z, eT), make_float4(ex, ey, ez, 0.f),
-               make_uint4((uint32_t)h, (uint32_t)(h >> 32), etrack, COM ? pend.col : 0u));
+               make_uint4((uint32_t)h, (uint32_t)(h >> 32), etrack, COM ? pend.col : 0u), big);
     // ... and, in the rare iteration with a pair production in the warp, the e-/e+ through the same ring (the lane's
     // x, y, z, u, v, w, h, track and nchild are still those of the converting photon)
     const unsigned mp = __ballot_sync(kFull, push_p);
@@ -449,7 +464,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
 #pragma unroll
       for (int sl = 0; sl < 2; ++sl)
         stage_push(a.eq, a.ctl, ring, stg, pairT[sl] > 0.0f, make_float4(x, y, z, pairT[sl]), make_float4(u, v, w, 0.f),
-                   make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, (uint32_t)sl), COM ? pend.col : 0u));
+                   make_uint4((uint32_t)h, (uint32_t)(h >> 32), child_track(rng.track, nchild, (uint32_t)sl), COM ? pend.col : 0u), big);
       // the two 0.511 MeV annihilation photons (tracks: slots 2, 3 of this conversion) stay in the lane: it continues
       // as the first at once and keeps the second in its shared-memory slot until the first has ended
       if (push_p) {
@@ -487,7 +502,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_electron(const __grid_constant_
   const bool bricks = use_bricks(g);
   const unsigned n1 = a.src_kind == SRC_QUEUE ? min(*a.src_count, a.src.cap) : *a.src_count;
   const unsigned count = n1;
-  SrcCursor sc; sc.next = sc.end = 0u;
+  SrcCursor sc; sc.next = sc.end = sc.chunk = 0u;
   Tally tl; tl.inc = tl.dep = tl.esc = 0;
   if (DBG) { for (int s = 0; s < ST_COUNT; ++s) tl.st[s] = 0; }
   Pending<COM> pend; pend.v = 0; pend.q = 0; pend.col = 0u;
