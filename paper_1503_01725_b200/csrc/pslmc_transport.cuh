@@ -133,7 +133,7 @@ __device__ __forceinline__ void finish_track(const TransportArgs &a, unsigned lo
 
 // Warp-aggregated push through a per-warp shared-memory ring of 64 entries: lanes with `want` append at consecutive ring
 // positions (ballot + prefix sum); whenever the ring holds >= 32 entries the warp writes 32 of them to the queue as three
-// coalesced 512-byte rows.  Queue slots are taken 64 at a time with ONE tail atomic (two flushes per atomic: the tail is
+// coalesced 512-byte rows.  Queue slots are taken 128 at a time with ONE tail atomic (four flushes per atomic: the tail is
 // one address for every warp of the launch, and halving the atomics on it is worth more than the few null entries it
 // costs); the half of a reservation a warp has not used when the kernel ends is filled with null entries (energy 0),
 // which the consumer skips.  No atomic and no global store in the common iteration.  Convergent calls.
@@ -169,7 +169,7 @@ __device__ __forceinline__ void stage_write(const Queue &q, StageRing &r, StageC
   __syncwarp();
 }
 // One call per loop iteration (convergent): resolves the reservation issued in the previous iteration, writes 32 entries
-// when the ring holds that many and slots are at hand, appends this iteration's entries, and reserves 64 more slots once
+// when the ring holds that many and slots are at hand, appends this iteration's entries, and reserves 128 more slots once
 // 32 entries are staged without any.  The ring never holds more than 31 + 32 entries.
 __device__ __forceinline__ void stage_push(const Queue &q, Control *ctl, StageRing &r, StageCursor &sc, bool want,
                                            float4 A, float4 B, uint4 C, bool big) {
@@ -183,7 +183,7 @@ __device__ __forceinline__ void stage_push(const Queue &q, Control *ctl, StageRi
     }
     sc.n += __popc(m);
   }
-  if (sc.n >= 32u && !sc.have) stage_reserve(q, sc, big ? 64u : 32u);      // (big: the warp still has source to come, so the second half will be used)
+  if (sc.n >= 32u && !sc.have) stage_reserve(q, sc, big ? 128u : 32u);      // (big: the warp still has source to come, so the second half will be used)
 }
 __device__ __forceinline__ void stage_drain(const Queue &q, Control *ctl, StageRing &r, StageCursor &sc) {
   if (sc.pending) stage_resolve(q, ctl, sc);
@@ -454,7 +454,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_photon(const __grid_constant__ 
       }
     }
     // ---- secondaries, convergent: Compton electrons through the staging ring ...
-    const bool big = !DBG && !exhausted && sc.chunk >= 128u;   // not in the tail of the source: queue slots are taken 64 at a time
+    const bool big = !DBG && !exhausted && sc.chunk >= 128u;   // not in the tail of the source: queue slots are taken 128 at a time
     stage_push(a.eq, a.ctl, ring, stg, push_e, make_float4(x, y, z, eT), make_float4(ex, ey, ez, 0.f),
                make_uint4((uint32_t)h, (uint32_t)(h >> 32), etrack, COM ? pend.col : 0u), big);
     // ... and, in the rare iteration with a pair production in the warp, the e-/e+ through the same ring (the lane's
