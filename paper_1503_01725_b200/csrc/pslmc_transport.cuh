@@ -135,8 +135,9 @@ __device__ __forceinline__ void finish_track(const TransportArgs &a, unsigned lo
 // positions (ballot + prefix sum); whenever the ring holds >= 32 entries the warp writes 32 of them to the queue as three
 // coalesced 512-byte rows.  Queue slots are taken 128 at a time with ONE tail atomic (four flushes per atomic: the tail is
 // one address for every warp of the launch, and halving the atomics on it is worth more than the few null entries it
-// costs); the half of a reservation a warp has not used when the kernel ends is filled with null entries (energy 0),
-// which the consumer skips.  No atomic and no global store in the common iteration.  Convergent calls.
+// costs); the part of a reservation a warp has not used when the kernel ends is filled with null entries (electrons of
+// 1e-30 MeV, which k_electron ends in their first sub-step with a deposit of 0 quanta).  No atomic and no global store in
+// the common iteration.  Convergent calls.
 struct StageRing { float4 a[64], b[64]; uint4 c[64]; };           // 3 KiB per warp
 struct StageCursor { unsigned head, n, base_raw, base, have; bool pending; };     // have: reserved slots not written yet (at `base`)
 // The atomic's latency is not waited for: stage_reserve issues it (result left in lane 0's register), stage_resolve -
