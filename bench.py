@@ -41,9 +41,9 @@ BUDGET = {"sample": 300.0,      # per history: 2 Philox blocks (2 x 40), alias p
           "deflection": 90.0}   # Philox block 40, Highland angle 12, sincos + rotation 34, reciprocals 4
 # SASS thread-instructions the kernels as built retire per history (ncu smsp__thread_inst_executed.sum / histories): side
 # information, so that retired / algorithmic is visible.  Source: profiles/r2_launches.md (ncu launch lists of the end-of-round code).
-RETIRED = {"C4": {"sample": 553, "photon": 3392, "electron": 3070}, "C1": {"sample": 473, "photon": 712, "electron": 881}}
+RETIRED = {"C4": {"sample": 553, "photon": 3458, "electron": 3070}, "C1": {"sample": 473, "photon": 727, "electron": 882}}
 # DRAM bytes (read + write) per history of each kernel class, from the `ncu --set full` captures in profiles/r2_top_kernels.md
-NCU_DRAM_BYTES_PER_HISTORY = {"C4": {"sample": 17.4, "photon": 252.3, "electron": 197.9}, "C1": {"sample": 6.0, "photon": 31.1, "electron": 23.5}}
+NCU_DRAM_BYTES_PER_HISTORY = {"C4": {"sample": 17.6, "photon": 254.6, "electron": 197.8}, "C1": {"sample": 5.9, "photon": 30.3, "electron": 23.4}}
 
 
 def parse():
