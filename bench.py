@@ -224,23 +224,25 @@ class Workload:
         self.dose = torch.empty(nv, dtype=torch.float64, device="cuda")
         self.ws = B.workspace(self.psl.workspace_bytes(self.ph, args.batch, host=True))
         self.order = B.MC_ORDER_MIXED if args.order == "mixed" else B.MC_ORDER_SORTED
-        self.flags = B.MC_FLAG_TIMING | (B.MC_FLAG_STATIC_LANES if args.static_lanes else 0) | \
+        self.flags = (B.MC_FLAG_STATIC_LANES if args.static_lanes else 0) | \
             {"on": B.MC_FLAG_TILE_SORT, "off": 0}[args.tile_sort]
         self.hb, self.he = B.shard_range(self.n_total, rank, world)
         self.stream = torch.cuda.current_stream()
 
-    def step(self, pipelines=None):
+    def step(self, pipelines=None, timing=False):
+        """One pass of the whole path.  timing: per-kernel-class CUDA events inside the library (the serial pass only)."""
         B, a = self.B, self.args
         pipelines = a.pipelines if pipelines is None else pipelines
+        flags = self.flags | (B.MC_FLAG_TIMING if timing else 0)
         self.acc.zero_()
         if self.plan:
             nb = len(self.cfg["beams"])
             B.plan_dose([self.psl] * nb, self.ph, self.cfg["beams"], self.n_total, self.cfg["seed"], batch=a.batch, rank=self.rank,
-                        world=self.world, dose_out=self.dose, dose_acc=self.acc, workspace=self.ws, flags=self.flags,
+                        world=self.world, dose_out=self.dose, dose_acc=self.acc, workspace=self.ws, flags=flags,
                         stream=self.stream, pipelines=pipelines)
         else:
             self.psl.dose(self.ph, self.cfg["beams"][0], self.n_total, self.cfg["seed"], batch=a.batch, dose_out=self.dose,
-                          dose_acc=self.acc, workspace=self.ws, order=self.order, flags=self.flags, history_begin=self.hb,
+                          dose_acc=self.acc, workspace=self.ws, order=self.order, flags=flags, history_begin=self.hb,
                           history_end=self.he, stream=self.stream, pipelines=pipelines)
 
     def make_e2e(self):
@@ -262,7 +264,7 @@ class Workload:
             def run():
                 self.psl.dose_host(cfg["phantom"], cfg["beams"][0], self.n_total, cfg["seed"], batch=a.batch, dose_out=hout.numpy(),
                                    density=hd.numpy(), material=hm.numpy(), workspace=self.ws, order=self.order,
-                                   flags=self.flags & ~B.MC_FLAG_TIMING, history_begin=self.hb, history_end=self.he, stream=self.stream)
+                                   flags=self.flags, history_begin=self.hb, history_end=self.he, stream=self.stream)
         return run, 5 * self.ph.nvox, 8 * self.ph.nvox
 
 
@@ -300,7 +302,7 @@ def measure(w: Workload, steps: int, warmup: int, flush, dist=None):
     serial_ms = 0.0
     for _ in range(steps):
         flush.fill_(1)
-        w.step(pipelines=1)
+        w.step(pipelines=1, timing=True)
         s1 = B.stats()
         serial_ms += s1["ms_total"]
         for k in ms_class:
