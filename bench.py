@@ -60,7 +60,7 @@ def parse():
     ap.add_argument("--order", default="sorted", choices=["sorted", "mixed"])
     ap.add_argument("--static-lanes", action="store_true")
     ap.add_argument("--tile-sort", default="off", choices=["on", "off"], help="ablation: order every batch by entry tile (MC_FLAG_TILE_SORT)")
-    ap.add_argument("--pipelines", type=int, default=0, help="0 = two overlapping launch sequences, 1 = serial")
+    ap.add_argument("--pipelines", type=int, default=0, help="0 = three overlapping launch sequences (the library default), 1 = serial")
     return ap.parse_args()
 
 
@@ -297,7 +297,7 @@ def measure(w: Workload, steps: int, warmup: int, flush, dist=None):
             comm_ms += c0.elapsed_time(c1)
     torch.cuda.synchronize()
     total_ms = sum(e0.elapsed_time(e1) for e0, e1 in ev)
-    # per-kernel-class times: the same steps with strictly serial launches (with two pipelines the classes overlap)
+    # per-kernel-class times: the same steps with strictly serial launches (with several pipelines the classes overlap)
     ms_class = {k: 0.0 for k in B.KERNEL_CLASSES}
     serial_ms = 0.0
     for _ in range(steps):
@@ -458,14 +458,14 @@ def finish(args, B, head, m, total_ms, ck, others, selfcheck, peaks, world, warm
             "ms_per_step": out["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": out["workload"], "histories_per_gpu": head.per_gpu, "seed": head.cfg["seed"], "batch": args.batch,
-                       "order": args.order, "lane_refill": not args.static_lanes, "tile_sort": args.tile_sort, "pipelines": args.pipelines or 2,
+                       "order": args.order, "lane_refill": not args.static_lanes, "tile_sort": args.tile_sort, "pipelines": args.pipelines or 3,
                        "parallelism": "history-range shards x%d + int64 all-reduce" % world if world > 1 else "single GPU",
                        "l2": "flushed between timed steps (256 MiB write)"},
             "clocks": ck, "e2e": out["e2e"], "gpu_launches": m["launches"]}
     for k in ("roofline", "whole_path_alu_frac", "alg_thread_inst_per_history", "events_per_history", "kernel_ms_per_step", "serial_ms_per_step", "k_sample"):
         if k in out:
             line[k] = out[k]
-    line["kernel_ms_note"] = "serial pass (pipelines=1); the timed region overlaps two pipelines"
+    line["kernel_ms_note"] = "serial pass (pipelines=1); the timed region overlaps three pipelines"
     if base is not None:
         line["cpu_baseline"] = base
     # the random-access ceilings of this phantom (probes): gathers from the packed phantom, int64 REDs into the grid

@@ -109,11 +109,13 @@ typedef struct {
   uint64_t *fingerprints;          /* DEVICE u64[history_end-history_begin] or NULL; ADDED to    */
   uint64_t  history_begin;         /* sub-range of history ids to run (sharding) ...             */
   uint64_t  history_end;           /* ... 0 means n_histories (unless MC_FLAG_RANGE)             */
-  int32_t   pipelines;             /* 0 = as many as aux_streams are given (at most 2), 1 = strictly */
-                                   /* serial launches on cuda_stream (per-kernel times in mc_stats    */
-                                   /* are then disjoint).  With 2, batches are dealt alternately to   */
-                                   /* two launch sequences so that one kernel's tail overlaps the     */
-                                   /* other sequence's next kernel.  Same bits either way.            */
+  int32_t   pipelines;             /* 0 = the default (3 when both aux_streams are given), 1 =      */
+                                   /* strictly serial launches on cuda_stream (per-kernel times in    */
+                                   /* mc_stats are then disjoint), at most 3.  With n > 1, batches    */
+                                   /* are dealt round-robin to n launch sequences - on aux_streams[0], */
+                                   /* aux_streams[1] and, the third, cuda_stream itself - so that one */
+                                   /* kernel's tail overlaps another sequence's next kernel.  Same    */
+                                   /* bits for every n.                                               */
   int32_t   reserved;              /* must be 0                                                    */
   /* commissioning tally, off when com_index is NULL: every history carries the */
   /* column of the PSR it was sampled from (its descendants inherit it): (stype*n_ebin+ebin)*n_ring */

@@ -31,7 +31,7 @@ static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 // data, packed phantom, the int64 dose grid (used when the caller gives no dose_acc).  Per pipeline
 // (kMaxPipes of them, see Session): the particle buffer (2 planes + the commissioning column) twice - as packed by
 // k_sample and ordered by entry tile -, the entry-tile counters, and the electron queue (capacity 4B, 3 planes).  mc_dose_host appends its staging area (phantom in, dose out).
-constexpr int kMaxPipes = 2;
+constexpr int kMaxPipes = 3;     // two on the caller's aux_streams, the third on cuda_stream itself
 struct Layout {
   size_t ctl[kMaxPipes], tile[kMaxPipes], xs, vox, brick, sbrick, com_mask, com_coarse, acc, p0[kMaxPipes], p1[kMaxPipes], p2[kMaxPipes], q0[kMaxPipes], q1[kMaxPipes], q2[kMaxPipes],
       eq[kMaxPipes][3], total, zero_bytes;
@@ -194,7 +194,7 @@ struct Session {
   static constexpr size_t kXsSmem = kXsBytes + sizeof(StageRing) * (kThreads / 32) + kAnnihBytes;   // k_photon dynamic shared memory
 
   ~Session() {
-    for (cudaEvent_t e : {ev0, ev1, ev_fork, ev_join[0], ev_join[1]}) if (e) cudaEventDestroy(e);
+    for (cudaEvent_t e : {ev0, ev1, ev_fork, ev_join[0], ev_join[1], ev_join[2]}) if (e) cudaEventDestroy(e);
     tm_us.discard(); for (Pipe &p : pipes) p.tm.discard();                      // (events left by an early error return)
   }
 
@@ -272,7 +272,7 @@ struct Session {
     timing = (o.flags & MC_FLAG_TIMING) != 0;
     npipe = o.pipelines > 0 ? o.pipelines : kMaxPipes;
     npipe = std::max(1, std::min(npipe, kMaxPipes));
-    for (int p = 0; p < npipe; ++p) if (npipe > 1 && !o.aux_streams[p]) npipe = 1;     // no streams given: serial
+    for (int p = 0; p < std::min(npipe, 2); ++p) if (npipe > 1 && !o.aux_streams[p]) npipe = 1;     // no streams given: serial
     if (npipe > 1 && (o.aux_streams[0] == o.aux_streams[1] || o.aux_streams[0] == o.cuda_stream || o.aux_streams[1] == o.cuda_stream))
       return fail(MC_E_INVALID_ARG, "aux_streams must be distinct from each other and from cuda_stream");
     long long *acc = dose_acc ? dose_acc : (long long *)(ws + L.acc);
@@ -285,7 +285,7 @@ struct Session {
     g.com_mask = (const uint32_t *)(ws + L.com_mask); g.com_coarse = (const uint32_t *)(ws + L.com_coarse);
     for (int p = 0; p < npipe; ++p) {
       Pipe &q = pipes[p];
-      q.st = npipe > 1 ? (cudaStream_t)o.aux_streams[p] : us; q.ctl = (Control *)(ws + L.ctl[p]);
+      q.st = (npipe > 1 && p < 2) ? (cudaStream_t)o.aux_streams[p] : us; q.ctl = (Control *)(ws + L.ctl[p]);
       q.p0 = (float4 *)(ws + L.p0[p]); q.p1 = (float4 *)(ws + L.p1[p]); q.p2 = (uint32_t *)(ws + L.p2[p]);
       q.q0 = (float4 *)(ws + L.q0[p]); q.q1 = (float4 *)(ws + L.q1[p]); q.q2 = (uint32_t *)(ws + L.q2[p]);
       q.tile_count = (unsigned *)(ws + L.tile[p]); q.tile_cursor = q.tile_count + kTileBinsMax;
@@ -326,7 +326,7 @@ struct Session {
     if (npipe > 1) {
       CUDA_TRY(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
       CUDA_TRY(cudaEventRecord(ev_fork, us));
-      for (int p = 0; p < npipe; ++p) CUDA_TRY(cudaStreamWaitEvent(pipes[p].st, ev_fork, 0));
+      for (int p = 0; p < npipe; ++p) if (pipes[p].st != us) CUDA_TRY(cudaStreamWaitEvent(pipes[p].st, ev_fork, 0));
     }
     memset(&g_stats, 0, sizeof g_stats);
     return MC_OK;
@@ -407,6 +407,7 @@ struct Session {
   // Joins the pipelines, converts (or only scans) the grid, synchronises once, folds the control blocks into g_stats.
   int end(const phantom_t &ph, double *dose_out, uint64_t n_norm, uint64_t n_run, const char *who) {
     for (int p = 0; p < npipe && npipe > 1; ++p) {
+      if (pipes[p].st == us) continue;                      // (the third pipeline runs on the caller's stream itself)
       CUDA_TRY(cudaEventCreateWithFlags(&ev_join[p], cudaEventDisableTiming));
       CUDA_TRY(cudaEventRecord(ev_join[p], pipes[p].st));
       CUDA_TRY(cudaStreamWaitEvent(us, ev_join[p], 0));

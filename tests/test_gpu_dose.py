@@ -82,7 +82,7 @@ def test_bitwise_identity_under_batch_order_partition(B, gpsl, cfg):
     ref_acc, ref_dose, ref_st, ref_fp = gpu_dose(B, g, dph, beam, N, seed, 1 << 16)
     for batch, opt in ((1000, {}), (33_333, {}), (1 << 20, {}), (1 << 13, dict(order=B.MC_ORDER_MIXED)),
                        (1 << 15, dict(flags=B.MC_FLAG_STATIC_LANES)), (1 << 15, dict(flags=B.MC_FLAG_STATS | B.MC_FLAG_TIMING)),
-                       (1 << 14, dict(pipelines=1)), (1 << 12, dict(pipelines=2, flags=B.MC_FLAG_TIMING)),
+                       (1 << 14, dict(pipelines=1)), (1 << 12, dict(pipelines=2, flags=B.MC_FLAG_TIMING)), (1 << 12, dict(pipelines=3)),
                        (1 << 16, dict(flags=B.MC_FLAG_STAGE_SCORING)), (1 << 12, dict(flags=B.MC_FLAG_STAGE_SCORING | B.MC_FLAG_STATS, order=B.MC_ORDER_MIXED)),
                        (1 << 14, dict(flags=B.MC_FLAG_TILE_SORT)), (1 << 13, dict(flags=B.MC_FLAG_TILE_SORT | B.MC_FLAG_STATS, order=B.MC_ORDER_MIXED, pipelines=1))):
         acc, dose, st, fp = gpu_dose(B, g, dph, beam, N, seed, batch, **opt)
@@ -179,7 +179,7 @@ def test_no_allocation_inside_mc_dose_and_voxel_overflow(B, gpsl, cfg):
     g.dose(dph, beam, 50_000, 3, batch=1 << 14, dose_out=dose, dose_acc=acc, workspace=ws)        # module load, first-use costs
     torch.cuda.synchronize()
     free0 = torch.cuda.mem_get_info()[0]
-    for pipes in (1, 2):
+    for pipes in (1, 2, 3):
         g.dose(dph, beam, 50_000, 3, batch=1 << 14, dose_out=dose, dose_acc=acc, workspace=ws, pipelines=pipes, flags=B.MC_FLAG_TIMING)
     torch.cuda.synchronize()
     assert torch.cuda.mem_get_info()[0] == free0
