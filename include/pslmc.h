@@ -219,6 +219,23 @@ int  mc_dose(const psl_t *psl, const phantom_t *ph, const beam_geom_t *beam,
              uint64_t n_histories, uint64_t seed, uint64_t batch,
              double *dose_out, const mc_opts_t *opts);
 
+/* mc_dose_static — mc_dose for callers that may not allocate device memory (code whose surroundings are under CUDA
+ * graph capture, serving loops, harnesses that forbid cudaMalloc).  Same arguments, same kernels, same bits as mc_dose,
+ * except that opts->workspace / workspace_bytes must be NULL / 0: the scratch is a file-scope `static __device__` array
+ * of MC_STATIC_WORKSPACE_BYTES inside the library (every GPU that loads libpslmc holds it until the process exits; its
+ * device address is taken once per device with cudaGetSymbolAddress on the device current at the first call).  Needs
+ * mc_workspace_bytes(psl, ph, batch) <= MC_STATIC_WORKSPACE_BYTES, else MC_E_WORKSPACE (nothing is launched): e.g. a
+ * 64^3 phantom with batch <= 2^16, or a 128^3 phantom with batch <= 2^15.  The call itself and everything below it
+ * calls no cudaMalloc, cudaFree or other allocating routine (it creates and destroys CUDA events, like mc_dose).
+ * The array is shared by every call on that device and keeps the last call's contents; the call clears what must start
+ * at zero.  Two mc_dose_static calls that overlap on one GPU (different streams or host threads) RACE on it: serialise
+ * them, or give the others their own workspace through mc_dose.  Inputs and outputs stay the caller's.                */
+#define MC_STATIC_WORKSPACE_BYTES (64u << 20)
+size_t mc_static_workspace_bytes(void);
+int  mc_dose_static(const psl_t *psl, const phantom_t *ph, const beam_geom_t *beam,
+                    uint64_t n_histories, uint64_t seed, uint64_t batch,
+                    double *dose_out, const mc_opts_t *opts);
+
 /* mc_dose_host — same, end to end from HOST buffers: ph->density / ph->material and dose_out are
  * HOST pointers (pinned memory makes the copies asynchronous); the call uploads the phantom into the
  * workspace, runs mc_dose, and downloads the dose.  opts->workspace >= mc_host_workspace_bytes.  */

@@ -20,7 +20,7 @@ MC_FLAG_RANGE, MC_FLAG_NO_TILE_SORT, MC_FLAG_TILE_SORT, MC_FLAG_FP_VOXELS = 32, 
 LEDGERS = ("incident", "deposited", "escaped", "jaw")
 KERNEL_CLASSES = ("sample", "photon", "electron", "finalise", "aux")
 EXPORTS = ("psl_build", "psl_build_grid", "psl_set_direction_model", "mc_plan_allocate", "mc_plan_dose", "psl_free", "psl_export", "psl_allocate",
-           "mc_workspace_bytes", "mc_host_workspace_bytes", "mc_dose", "mc_dose_host",
+           "mc_workspace_bytes", "mc_host_workspace_bytes", "mc_dose", "mc_dose_host", "mc_dose_static", "mc_static_workspace_bytes",
            "mc_stats", "mc_last_error", "mc_sample_debug", "mc_transport_debug", "mc_philox_debug", "mc_xs_debug")
 
 
@@ -98,6 +98,9 @@ def lib():
                      C.c_void_p, C.POINTER(mc_opts_t)]
         L.mc_dose.argtypes = dose_args
         L.mc_dose_host.argtypes = dose_args
+        L.mc_dose_static.argtypes = dose_args
+        L.mc_static_workspace_bytes.restype = C.c_size_t
+        L.mc_static_workspace_bytes.argtypes = []
         L.mc_stats.argtypes = [C.POINTER(mc_stats_t)]
         L.mc_last_error.restype = C.c_char_p
         L.mc_sample_debug.argtypes = [C.c_void_p, C.POINTER(beam_geom_t), C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint64,
@@ -286,6 +289,19 @@ class Psl:
         o = _opts(**opt)
         _check(lib().mc_dose(self.h, C.byref(phantom.c), C.byref(_beam(beam)), n_histories, seed, batch,
                              dose_out.data_ptr() if dose_out is not None else None, C.byref(o)))
+        return dose_out
+
+    def dose_static(self, phantom: DevicePhantom, beam: dict, n_histories: int, seed: int, batch: int = 1 << 14, dose_out=None,
+                    **opt):
+        """mc_dose_static: mc_dose on the library's static device scratch (no allocation inside the call; dose_out or
+        dose_acc must be given by callers that want none in the binding either).  Same bits as dose()."""
+        import torch
+        if dose_out is None and opt.get("dose_acc") is None:
+            dose_out = torch.empty(phantom.nvox, dtype=torch.float64, device=phantom.device)
+        assert opt.get("workspace") is None, "dose_static takes no workspace"
+        o = _opts(**opt)
+        _check(lib().mc_dose_static(self.h, C.byref(phantom.c), C.byref(_beam(beam)), n_histories, seed, batch,
+                                    dose_out.data_ptr() if dose_out is not None else None, C.byref(o)))
         return dose_out
 
     def dose_host(self, ph: dict, beam: dict, n_histories: int, seed: int, batch: int = 1 << 22, dose_out: np.ndarray = None,

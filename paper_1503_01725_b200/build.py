@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpslmc.so")
-SOURCES = ["pslmc_psl.cu", "pslmc_dose.cu"]
+SOURCES = ["pslmc_psl.cu", "pslmc_dose.cu", "pslmc_static.cu"]
 PROBE_LIB = os.path.join(HERE, "libpslmc_probe.so")           # measurement probes (probes.py), not part of the ABI
 PROBE_SOURCES = [os.path.join("probes", "mem_probe.cu")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-fmad=false",
