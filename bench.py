@@ -41,9 +41,9 @@ BUDGET = {"sample": 300.0,      # per history: 2 Philox blocks (2 x 40), alias p
           "deflection": 90.0}   # Philox block 40, Highland angle 12, sincos + rotation 34, reciprocals 4
 # SASS thread-instructions the kernels as built retire per history (ncu smsp__thread_inst_executed.sum / histories): side
 # information, so that retired / algorithmic is visible.  Source: profiles/r2_launches.md (ncu launch lists of the end-of-round code).
-RETIRED = {"C4": {"sample": 553, "photon": 3458, "electron": 3070}, "C1": {"sample": 473, "photon": 727, "electron": 882}}
+RETIRED = {"C4": {"sample": 548, "photon": 3440, "electron": 3061}, "C1": {"sample": 471, "photon": 717, "electron": 875}}
 # DRAM bytes (read + write) per history of each kernel class, from the `ncu --set full` captures in profiles/r2_top_kernels.md
-NCU_DRAM_BYTES_PER_HISTORY = {"C4": {"sample": 17.6, "photon": 254.6, "electron": 197.8}, "C1": {"sample": 5.9, "photon": 30.3, "electron": 23.4}}
+NCU_DRAM_BYTES_PER_HISTORY = {"C4": {"sample": 27.9, "photon": 253.8, "electron": 176.3}, "C1": {"sample": 14.2, "photon": 34.4, "electron": 20.0}}
 
 
 def parse():
@@ -53,7 +53,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C4")
-    ap.add_argument("--batch", type=int, default=1 << 22)
+    ap.add_argument("--batch", type=int, default=1 << 24)
     ap.add_argument("--histories", type=int, default=0, help="override histories per GPU (default: the config's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-all-configs", action="store_true", help="time the headline workload only")

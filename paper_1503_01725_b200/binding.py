@@ -160,6 +160,7 @@ def stats() -> dict:
     return out
 
 
+DEFAULT_BATCH = 1 << 24        # histories per k_sample launch: 13.3 GB of workspace (3 pipelines x 264 B), measured best on C1-C4
 _aux = {}                                                # device index -> two torch streams for the pipelines (torch owns them)
 _ws = {}                                                 # device index -> cached torch workspace (torch owns the memory)
 
@@ -278,7 +279,7 @@ class Psl:
                                      _stream_ptr(stream)))
         return out
 
-    def dose(self, phantom: DevicePhantom, beam: dict, n_histories: int, seed: int, batch: int = 1 << 22, dose_out=None,
+    def dose(self, phantom: DevicePhantom, beam: dict, n_histories: int, seed: int, batch: int = DEFAULT_BATCH, dose_out=None,
              **opt):
         """mc_dose.  Returns dose_out (torch float64 on the device, MeV/g per history)."""
         import torch
@@ -304,7 +305,7 @@ class Psl:
                                     dose_out.data_ptr() if dose_out is not None else None, C.byref(o)))
         return dose_out
 
-    def dose_host(self, ph: dict, beam: dict, n_histories: int, seed: int, batch: int = 1 << 22, dose_out: np.ndarray = None,
+    def dose_host(self, ph: dict, beam: dict, n_histories: int, seed: int, batch: int = DEFAULT_BATCH, dose_out: np.ndarray = None,
                   density: np.ndarray = None, material: np.ndarray = None, **opt) -> np.ndarray:
         """mc_dose_host: host phantom arrays in, host dose out (copies inside the call)."""
         density = np.ascontiguousarray(ph["density"], np.float32) if density is None else density
@@ -352,7 +353,7 @@ def plan_allocate(psls, n_histories: int) -> np.ndarray:
     return out
 
 
-def plan_dose(psls, phantom, beams, n_histories: int, seed: int, batch: int = 1 << 22, rank: int = 0, world: int = 1,
+def plan_dose(psls, phantom, beams, n_histories: int, seed: int, batch: int = DEFAULT_BATCH, rank: int = 0, world: int = 1,
               dose_out=None, dose_acc=None, **opt):
     """mc_plan_dose: a multi-beam plan (PAPER.md:73-80 S1-S2) - Eq. 3 over all beams, beam i with seed + i, one int64 grid.
     With world > 1 this call runs shard `rank` of every beam's histories; the caller all-reduces the returned grid

@@ -67,7 +67,7 @@ def test_commissioning_loop_recovers_a_reweighted_beam(B, cfg):
         jaws = dict(c["jaws"], x1=-field / 2, x2=field / 2, y1=-field / 2, y2=field / 2)
         g = B.Psl(psr, jaws, c["n_sectors"])
         N = 20_000_000
-        _, A = gpu_matrix(B, g, dph, c["beams"][0], N, seed, idx, rows, cols, batch=1 << 22)
+        _, A = gpu_matrix(B, g, dph, c["beams"][0], N, seed, idx, rows, cols, batch=B.DEFAULT_BATCH)
         w_active = sum(gr["W"] for gr in g.export()["groups"])
         mats.append(A.T.astype(np.float64) * (w_active / N))                     # rows x cols, dose per particle of the whole plane
     A = np.vstack(mats)
@@ -106,7 +106,7 @@ def test_tally_costs_little(B, cfg):
             best = 1e30
             for _ in range(3):
                 acc.zero_()
-                g.dose(dph, c["beams"][0], N, 77, batch=1 << 22, dose_acc=acc, **opt)
+                g.dose(dph, c["beams"][0], N, 77, batch=B.DEFAULT_BATCH, dose_acc=acc, **opt)
                 best = min(best, B.stats()["ms_total"])
             ms[key] = best
         print("commissioning tally, %gx%g cm2 field, %g histories: plain %.1f ms (%.3e histories/s), with the tally %.1f ms (%.3e histories/s)"

@@ -301,7 +301,7 @@ def test_history_ids_beyond_32_bits(B, orc, gpsl, opsl, cfg):
 
 
 def test_full_size_c1_in_the_bench_configuration(B, orc, gpsl, opsl, cfg):
-    """BASELINE.json configs[1] at its full 1e7 histories in the launch configuration bench.py times (batch 2^22, two
+    """BASELINE.json configs[1] at its full 1e7 histories in the launch configuration bench.py times (the default batch and
     pipelines, sorted order): (a) the interaction sequences of sampled history ranges match the oracle history by
     history; (b) the dose grid is bit-identical to a serial small-batch run; (c) the ledger identities hold."""
     import torch
@@ -311,7 +311,7 @@ def test_full_size_c1_in_the_bench_configuration(B, orc, gpsl, opsl, cfg):
     dph, oph = B.DevicePhantom(c["phantom"]), orc.Phantom(c["phantom"])
     fp = torch.zeros(N, dtype=torch.int64, device="cuda")
     acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
-    gpsl("C1").dose(dph, c["beams"][0], N, seed, batch=1 << 22, dose_acc=acc, fingerprints=fp)
+    gpsl("C1").dose(dph, c["beams"][0], N, seed, batch=B.DEFAULT_BATCH, dose_acc=acc, fingerprints=fp)
     st = B.stats()
     L = st["ledger"]
     assert int(acc.sum().item()) == L["deposited"]
@@ -330,7 +330,7 @@ def test_full_size_c1_in_the_bench_configuration(B, orc, gpsl, opsl, cfg):
     assert same / total >= 0.999, same / total
     # (b) same bits without fingerprints (the plain kernel variants bench.py times), and serial with a small batch
     acc2 = torch.zeros_like(acc)
-    gpsl("C1").dose(dph, c["beams"][0], N, seed, batch=1 << 22, dose_acc=acc2)
+    gpsl("C1").dose(dph, c["beams"][0], N, seed, batch=B.DEFAULT_BATCH, dose_acc=acc2)
     assert torch.equal(acc, acc2)
     acc3 = torch.zeros_like(acc)
     gpsl("C1").dose(dph, c["beams"][0], N, seed, batch=1 << 18, dose_acc=acc3, pipelines=1)
@@ -354,7 +354,7 @@ def test_ledgers_beyond_64_bits(B, gpsl, cfg):
     acc2 = torch.zeros_like(acc)
     led = 0
     for hb, he in ((0, N // 2), (N // 2, N)):
-        gpsl("C0").dose(dph, c["beams"][0], N, 3, batch=1 << 22, dose_acc=acc2, history_begin=hb, history_end=he)
+        gpsl("C0").dose(dph, c["beams"][0], N, 3, batch=B.DEFAULT_BATCH, dose_acc=acc2, history_begin=hb, history_end=he)
         led += B.stats()["ledger"]["deposited"]
     assert torch.equal(acc, acc2) and led == L["deposited"]
 
@@ -417,7 +417,7 @@ def test_full_size_sampled_parity_c2_c3_c4(name, beam, seed, B, orc, cfg):
     dph, oph = B.DevicePhantom(c["phantom"]), orc.Phantom(c["phantom"])
     fp = torch.zeros(N, dtype=torch.int64, device="cuda")
     acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
-    g.dose(dph, c["beams"][beam], N, seed, batch=1 << 22, dose_acc=acc, fingerprints=fp)
+    g.dose(dph, c["beams"][beam], N, seed, batch=B.DEFAULT_BATCH, dose_acc=acc, fingerprints=fp)
     L = B.stats()["ledger"]
     assert int(acc.sum().item()) == L["deposited"]
     assert abs(L["deposited"] + L["escaped"] + L["jaw"] - L["incident"]) <= 1e-5 * L["incident"]

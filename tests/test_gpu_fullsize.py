@@ -144,7 +144,7 @@ PARITY = [("C1", 0, 10_000_000, 2), ("C2", 0, 10_000_000, 3), ("C3", 0, 10_000_0
 def test_dose_every_voxel_at_parity_size(name, beam, N, seed, orc):
     """SURVEY §8(d) parity runs: C1 full (1e7), C2 at 1e7, C3 beam 0 at 1e7, C4 at 1e7 - every voxel above 10 % of Dmax."""
     from paper_1503_01725_b200 import binding as B
-    r = explained_parity(B, orc, name, beam, N, seed, [(0, N)], batch=1 << 22, rel_tol=5e-3, sequence=True)
+    r = explained_parity(B, orc, name, beam, N, seed, [(0, N)], batch=B.DEFAULT_BATCH, rel_tol=5e-3, sequence=True)
     print("%s N=%g: identical interaction sequences %.6f; strict-identical histories %.6f (%d diverged); %d voxels above 10%% Dmax; without the diverged histories: "
           "%d voxels beyond 0.5%% (largest relative difference %.2e), %d of them not balanced by their face neighbours; full tallies: %d voxels "
           "beyond 0.5%% (largest %.2e); integral dose ratio %.7f"

@@ -39,7 +39,7 @@ def test_gamma_independent_seeds_c0(cfg):
 
     def gpu(seed):
         acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
-        g.dose(dph, c["beams"][0], N, seed, batch=1 << 22, dose_acc=acc)
+        g.dose(dph, c["beams"][0], N, seed, batch=B.DEFAULT_BATCH, dose_acc=acc)
         return acc.cpu().numpy().astype(np.float64).reshape(32, 32, 32)
 
     d_gpu, d_gpu2 = gpu(SEED_GPU), gpu(SEED_GPU2)
@@ -84,7 +84,7 @@ def test_gamma_gpu_vs_gpu_two_seeds(name, beam, n, cfg):
 
     def run(seed, hb, he):
         acc = torch.zeros(dph.nvox, dtype=torch.int64, device="cuda")
-        g.dose(dph, c["beams"][beam], n, seed, batch=1 << 22, dose_acc=acc, history_begin=hb, history_end=he)
+        g.dose(dph, c["beams"][beam], n, seed, batch=B.DEFAULT_BATCH, dose_acc=acc, history_begin=hb, history_end=he)
         return acc.cpu().numpy().astype(np.float64)
 
     d_a, d_b, d_c = (run(s, 0, n).reshape(shape) for s in (1001, 2002, 3003))
