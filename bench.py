@@ -41,9 +41,9 @@ BUDGET = {"sample": 300.0,      # per history: 2 Philox blocks (2 x 40), alias p
           "deflection": 90.0}   # Philox block 40, Highland angle 12, sincos + rotation 34, reciprocals 4
 # SASS thread-instructions the kernels as built retire per history (ncu smsp__thread_inst_executed.sum / histories): side
 # information, so that retired / algorithmic is visible.  Source: profiles/r2_launches.md (ncu launch lists of the end-of-round code).
-RETIRED = {"C4": {"sample": 548, "photon": 3440, "electron": 3061}, "C1": {"sample": 471, "photon": 717, "electron": 875}}
+RETIRED = {"C4": {"sample": 548, "photon": 3442, "electron": 3062}, "C1": {"sample": 471, "photon": 717, "electron": 874}}
 # DRAM bytes (read + write) per history of each kernel class, from the `ncu --set full` captures in profiles/r2_top_kernels.md
-NCU_DRAM_BYTES_PER_HISTORY = {"C4": {"sample": 27.9, "photon": 253.8, "electron": 176.3}, "C1": {"sample": 14.2, "photon": 34.4, "electron": 20.0}}
+NCU_DRAM_BYTES_PER_HISTORY = {"C4": {"sample": 27.8, "photon": 257.5, "electron": 177.8}, "C1": {"sample": 14.2, "photon": 34.6, "electron": 20.0}}
 
 
 def parse():

@@ -293,10 +293,13 @@ struct Session {
       q.eq.count = &q.ctl->n_eq; q.eq.cap = eq_cap;
       q.tm.on = timing; q.tm.st = q.st;
     }
-    // When the packed phantom + int64 grid (12 B per voxel) do not fit L2 the kernels are bound by random DRAM sectors and
-    // fewer resident warps thrash less: measured on C4 (201 MB) 56.8 ms per 1e8 histories at 1.0, 53.1 at 0.75.
+    // Persistent grids fill every CTA slot except in one case: a phantom whose packed words + int64 grid (12 B per voxel)
+    // do not fit L2, several pipelines and batches below 2^24.  There the launch tails are frequent and a grid of 0.75 leaves
+    // slots in which the next pipeline's CTAs start while this kernel drains (C4, three pipelines: 72.8 against 73.8 ms per 2e8
+    // at batch 2^22, 127 against 143 ms at 2^17).  Alone on the GPU a full grid is 8-11 % faster (C4 serial: 142.8 against
+    // 159.0 ms per 4e8), and with batches of 2^24 still 1 % (140.5 against 141.9 ms): profiles/r2_ablation_c4.md.
     const bool big = 12.0 * (double)nvox > 110e6;
-    init_blocks(big ? 0.75 : 1.0);                  // (r2, with the hierarchical phantom: 0.65 / 0.85 / 1.0 on C4 and 0.5-0.75 elsewhere are all slower)
+    init_blocks(big && npipe > 1 && batch < (1ull << 24) ? 0.75 : 1.0);
     { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
     // Entry-tile ordering of every batch (the spatial inner loop): MC_FLAG_TILE_SORT.  Off by default:
     // measured on C4 it takes 10 % off the transport kernels' time and costs as much in the sort - photons
