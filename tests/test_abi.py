@@ -141,3 +141,20 @@ def test_flag_and_error_constants_match_header(binding):
     assert defs["MC_E_WORKSPACE"] == -3 and defs["MC_E_OVERFLOW"] == -5 and defs["MC_OK"] == 0
     vals = [defs[k] for k in defs if k.startswith("MC_FLAG_")]
     assert len(set(vals)) == len(vals) and all(v & (v - 1) == 0 for v in vals)         # distinct single bits
+
+
+def test_static_workspace_size_matches_header(binding):
+    """mc_dose_static's scratch: the size the library reports is the header's MC_STATIC_WORKSPACE_BYTES (64 MiB), and the
+    device image really holds an array of that size (a host-only query and an ELF look: no GPU needed)."""
+    import re
+    import subprocess
+    text = open(os.path.join(ROOT, "include", "pslmc.h")).read()
+    m = re.search(r"#define\s+MC_STATIC_WORKSPACE_BYTES\s+\((\d+)u\s*<<\s*(\d+)\)", text)
+    assert m, "MC_STATIC_WORKSPACE_BYTES not found in pslmc.h"
+    want = int(m.group(1)) << int(m.group(2))
+    assert want == 64 << 20
+    assert binding.lib().mc_static_workspace_bytes() == want
+    elf = subprocess.run(["cuobjdump", "-elf", binding.LIB_PATH], capture_output=True, text=True)
+    if elf.returncode == 0:                                   # (cuobjdump ships with the CUDA toolkit of this image)
+        rows = [ln for ln in elf.stdout.splitlines() if "g_static_workspace" in ln and hex(want) in ln.lower()]
+        assert rows, "no %d-byte g_static_workspace symbol in the device ELF" % want
